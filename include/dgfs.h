@@ -1,0 +1,136 @@
+/*
+ * dgfs.h -- C ABI of the B200-native multi-species DGFS Boltzmann collision operator.
+ *
+ * What the library computes is the fast Fourier-spectral collision operator Q^(pq)(f^(p), f^(q))
+ * of arXiv 1903.04670 ("PAPER.md", cited as P:line):
+ *   - Eq. 1       right-hand side  sum_q Kn_pq^-1 Q^(pq)            -> dgfs_collide
+ *   - Eq. 2    definition of Q^(pq)
+ *   - Eq. 13-17 low-rank separated kernel modes
+ *   - Algorithm 1  precomputed tables a, b^(pq), c^(pq)          -> dgfs_create
+ *   - Algorithm 2  FFT -> phase -> 2 iFFT -> product -> FFT -> weighted sum,
+ *                              loss term as one convolution, prefactor beta   -> dgfs_collide[_pairs]
+ *   - 1-D RKDG transport around it (readings DG-1..4)      -> dgfs_step
+ *
+ * Conventions (identical to DESIGN.md "Boundary"):
+ *   - all floating point data is IEEE fp64;
+ *   - velocity node z = (ix*N + iy)*N + iz (iz fastest), c = (c[ix], c[iy], c[iz]),
+ *     c[j] = -L + (j + 1/2) * 2L/N (cell centred);
+ *   - distribution functions  f[nx][ns][N^3]  (point slowest, species, velocity node fastest);
+ *   - pointers documented "device" are CUDA device pointers on the context's device, pointers
+ *     documented "host" are ordinary host pointers; the library never takes ownership of either;
+ *   - `stream` is the caller's cudaStream_t passed as void* (NULL = legacy default stream);
+ *     dgfs_collide* / dgfs_step enqueue work on it and return without synchronising;
+ *   - every int-returning call returns DGFS_OK (0) or a negative DGFS_E* code, validates its
+ *     arguments before any launch, and records a message readable with dgfs_last_error();
+ *   - there is no CPU fallback: without a CUDA device dgfs_create fails with DGFS_ECUDA.
+ */
+#ifndef DGFS_H
+#define DGFS_H
+
+#include <stddef.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#define DGFS_OK        0
+#define DGFS_EINVAL   -1   /* invalid argument (message says which)            */
+#define DGFS_ECUDA    -2   /* CUDA runtime error (message carries the string)  */
+#define DGFS_ENOMEM   -3   /* device allocation failed                         */
+#define DGFS_ENOSUP   -4   /* valid request the library does not implement     */
+
+typedef struct dgfs_ctx dgfs_ctx;   /* opaque: owns device tables + workspace */
+
+/* Inputs of Algorithm 1 plus the physical parameters of Eq. 4-6. All host. */
+typedef struct dgfs_params {
+  int ns;                  /* number of species n (Eq. 1)                                        */
+  const double *mass;      /* [ns]     non-dimensional masses m_p > 0                             */
+  const double *omega;     /* [ns*ns]  viscosity index omega_pq (Eq. 4); gamma_pq = 2(1-omega_pq) */
+  const double *alpha;     /* [ns*ns]  VSS scattering parameter alpha_pq > 0; 1.0 = VHS           */
+  const double *kn;        /* [ns*ns]  Knudsen numbers Kn_pq (Eq. 5), or NULL => 1.0              */
+  const double *prefactor; /* [ns*ns]  beta_pq override (Eq. 6), or NULL => Eq. 6 from kn         */
+  int N;                   /* velocity points per dimension; supported: 8, 16, 24, 32, 48         */
+  int N_rho;               /* Gauss-Legendre radial nodes on [0, R]                       */
+  int M;                   /* points on the full sphere (reading S-1)                      */
+  double L;                /* velocity box [-L, L]^3                                              */
+  double R;                /* relative-velocity truncation radius; <= 0 => Eq. 9 with
+                              (max mass, min mass) (reading RAD-1)                                */
+  const double *sigma;     /* [M*3] unit vectors, or NULL => built-in rule for M in {6, 12, 32}   */
+  const double *w_sigma;   /* [M] weights summing to 4 pi; must be NULL iff sigma is NULL         */
+  int table_mode;          /* 0 = angular integrals of Eq. 16/17 evaluated exactly (default)
+                              1 = Algo 1's pre-computation sphere quadrature (needs *_pre)        */
+  int M_pre;               /* table_mode 1: number of pre-computation sphere points               */
+  const double *sigma_pre; /* [M_pre*3]                                                           */
+  const double *w_pre;     /* [M_pre]                                                             */
+  int device;              /* CUDA device ordinal                                                 */
+} dgfs_params;
+
+/* Algorithm 1: quadratures, truncation radius (Eq. 9), prefactors (Eq. 6) and the
+ * kernel-mode tables for every (radial node r, sphere point s, pair p,q), built on the device
+ * and kept there. Synchronous. On success *out owns the tables until dgfs_destroy. */
+int dgfs_create(const dgfs_params *p, dgfs_ctx **out);
+
+/* Frees tables and workspace. NULL is allowed. */
+void dgfs_destroy(dgfs_ctx *c);
+
+/* Message of the last failed call on this context (or of the last failed dgfs_create when
+ * c == NULL). The string is owned by the library and valid until the next call. */
+const char *dgfs_last_error(const dgfs_ctx *c);
+
+/* Right-hand side of Eq. 1 at nx spatial points, Algorithm 2 for all pairs:
+ *   Q[x][p][:] = sum_q beta_pq * Q^(pq)(f[x][p], f[x][q]).
+ * f: device, [nx][ns][N^3], read only.  Q: device, [nx][ns][N^3], overwritten; must not
+ * alias f.  nx >= 0 (0 is a no-op).  Workspace is grown on demand (see dgfs_reserve). */
+int dgfs_collide(dgfs_ctx *c, const double *f, double *Q, int nx, void *stream);
+
+/* Same, every pair separately: Qpq[x][p][q][:] = beta_pq * Q^(pq)(f[x][p], f[x][q]).
+ * Qpq: device, [nx][ns][ns][N^3]. */
+int dgfs_collide_pairs(dgfs_ctx *c, const double *f, double *Qpq, int nx, void *stream);
+
+/* Bytes of device workspace dgfs_collide* needs for a batch of nx points (tables excluded). */
+size_t dgfs_workspace_bytes(const dgfs_ctx *c, int nx);
+
+/* Allocate the workspace for batches of up to nx points now, so that later dgfs_collide* calls
+ * with <= nx points never allocate (required before capturing them into a CUDA graph). */
+int dgfs_reserve(dgfs_ctx *c, int nx);
+
+/* Read back what dgfs_create derived (host outputs; any pointer may be NULL):
+ * R (scalar), rho[N_rho], w_rho[N_rho], sigma[M*3], w_sigma[M], beta[ns*ns]. */
+int dgfs_get_quadrature(const dgfs_ctx *c, double *R, double *rho, double *w_rho,
+                        double *sigma, double *w_sigma, double *beta);
+
+/* Copy the kernel-mode tables of pair (p,q) to HOST buffers, in Algorithm 1's layout and meaning
+ * (for verification): a[N_rho][M][N^3] real, b[N_rho][M][N^3] complex interleaved
+ * (re,im) (Eq. 16), c[N^3] complex interleaved (Eq. 17). Any pointer may be
+ * NULL. The internal device tables are factored/compressed; this call expands them with the
+ * library's own kernels. */
+int dgfs_get_tables(dgfs_ctx *c, int p, int q, double *a, double *b, double *cc);
+
+/* FLOP count of one pair evaluation as executed (SURVEY 8(d) / DESIGN.md "Roofline"), for the
+ * benchmark's roofline line. */
+double dgfs_flops_per_pair_eval(const dgfs_ctx *c, int p, int q);
+
+/* 1-D mesh for dgfs_step: ne uniform elements on [x0, x1], nodal DG of polynomial degree
+ * `order` on K = order+1 Gauss-Lobatto-Legendre nodes, purely diffuse walls at both ends
+ * (Table 2; readings DG-1, DG-2). */
+typedef struct dgfs_mesh1d {
+  int ne;
+  int order;
+  double x0, x1;
+  double wall_T[2];        /* wall temperatures at x0 and x1                                  */
+  double wall_u[2][3];     /* wall velocities at x0 and x1                                    */
+} dgfs_mesh1d;
+
+/* nsteps explicit SSP-RK3 steps (reading DG-3) of Eq. 1 in one space dimension:
+ *   d/dt f = -c_x d/dx f + sum_q beta_pq Q^(pq),  upwind interface flux, diffuse walls.
+ * f: device, [ne][K][ns][N^3], updated in place. */
+int dgfs_step(dgfs_ctx *c, const dgfs_mesh1d *mesh, double *f, double dt, int nsteps, void *stream);
+
+/* The spatial right-hand side alone (verification of D1-D3): rhs = -c_x d/dx f with upwind
+ * fluxes and diffuse walls, no collisions.  f, rhs: device, [ne][K][ns][N^3]. */
+int dgfs_advect_rhs(dgfs_ctx *c, const dgfs_mesh1d *mesh, const double *f, double *rhs, void *stream);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* DGFS_H */

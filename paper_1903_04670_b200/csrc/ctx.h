@@ -1,0 +1,81 @@
+// ctx.h -- internal context of libdgfs (not part of the ABI).
+#pragma once
+#include <cuda_runtime.h>
+#include <string>
+#include <vector>
+#include "../../include/dgfs.h"
+#include "fft_reg.cuh"
+
+namespace dgfs {
+
+// Device-side view of the tables built by dgfs_create (Algorithm 1).
+// "SPEC layout" = spectral index order [lz][lx][ly] (ly fastest): the order in which the
+// warp-per-plane transforms produce and consume spectra.
+struct DevTables {
+  int ns, npairs, N, N3, N_rho, M, K2n;
+  // separable phase factors  e^{ +i mu_q rho'_r sigma_s,d v } (side 0, acts on f^_p) and
+  // e^{ -i mu_p rho'_r sigma_s,d v } (side 1, acts on f^_q)  == exp(+-i mu a_rs), Algo 2 steps 4-5
+  // with a_rs of Algo 1 step 7 split per axis.  d = 0 carries the folded
+  // normalisation: side 0: w_sigma_s / N^3, side 1: 1 / N^3.
+  const cplx* phase;            // [pair][r][s][side][3][N]
+  // b^(pq)_r(|k|^2) for pairs whose b does not depend on s (VHS, table_mode 0; Eq. 16)
+  const double* bvhs;           // [pair][r][K2n]
+  // full b^(pq)_rs(k) in SPEC layout for the other pairs (VSS or table_mode 1), else nullptr
+  const cplx* const* bfull;     // [pair] -> [r][s][N3]
+  const cplx* closs;            // [pair][N3]  c^(pq)(k), SPEC layout (Eq. 17)
+  const double* w_rho;          // [N_rho]
+  const double* beta;           // [pair]      beta_pq (Eq. 6)
+  const unsigned char* full;    // [pair]      1 = uses bfull and per-s forward transforms
+};
+
+}  // namespace dgfs
+
+struct dgfs_ctx {
+  int device = 0;
+  int ns = 0, N = 0, N_rho = 0, M = 0, npairs = 0, N3 = 0, K2n = 0;
+  double L = 0, R = 0;
+  int table_mode = 0;
+  bool any_full = false;
+  std::vector<double> mass, omega, alpha, kn, beta, gam, eta, rho, w_rho, sigma, w_sigma;
+  std::vector<double> sigma_pre, w_pre;
+  int M_pre_count() const { return (int)w_pre.size(); }
+  std::vector<unsigned char> full;
+  // device tables
+  dgfs::cplx* d_phase = nullptr;
+  double* d_bvhs = nullptr;
+  std::vector<dgfs::cplx*> h_bfull;      // device pointers, one per pair (or nullptr)
+  dgfs::cplx** d_bfull = nullptr;
+  dgfs::cplx* d_closs = nullptr;
+  double* d_w_rho = nullptr;
+  double* d_beta = nullptr;
+  double* d_rho = nullptr;
+  double* d_sigma = nullptr;
+  unsigned char* d_full = nullptr;
+  dgfs::DevTables tab{};
+  // workspace (grown on demand)
+  void* ws = nullptr;
+  size_t ws_bytes = 0;
+  size_t scratch_budget = 0;             // bytes allowed for the transposition scratch G
+  // DG operator storage (dgfs_step)
+  void* dg_ws = nullptr;
+  size_t dg_ws_bytes = 0;
+  std::string err;
+};
+
+namespace dgfs {
+
+int set_error(dgfs_ctx* c, int code, const std::string& msg);
+int check_cuda(dgfs_ctx* c, cudaError_t e, const char* what);
+
+// create.cu
+int build_tables(dgfs_ctx* c);
+// collide.cu
+struct ChunkPlan {
+  int nbx;                 // spatial points per chunk
+  size_t off_fhat, off_qg, off_g, off_t, total;
+};
+ChunkPlan plan_chunks(const dgfs_ctx* c, int nx);
+int run_collide(dgfs_ctx* c, const double* f, double* out, int nx, bool pairs_out, cudaStream_t st);
+int ensure_workspace(dgfs_ctx* c, size_t bytes);
+
+}  // namespace dgfs

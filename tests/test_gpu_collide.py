@@ -1,0 +1,194 @@
+"""Parity of the CUDA path (through the C ABI, via the ctypes binding) with the CPU oracle.
+
+Bar (BASELINE.json north_star): max|Q_gpu - Q_oracle| <= 1e-10 * max|Q_oracle| per (point, pair)
+array, fp64.  Tables: 1e-13 relative to the table's max.
+"""
+import numpy as np
+import pytest
+
+from workloads import get_config, make_points, make_dg_state, maxwellian
+
+pytestmark = pytest.mark.gpu
+
+TOL = 1e-10
+
+
+@pytest.fixture(scope="module")
+def torch_cuda():
+    import torch
+    if not torch.cuda.is_available():
+        pytest.fail("GPU tests need a CUDA device: there is no CPU fallback")
+    torch.cuda.set_device(0)
+    return torch
+
+
+def _oracle_tables(cfg, **kw):
+    from oracle.tables import precompute
+    return precompute(cfg.N, cfg.N_rho, cfg.M, cfg.L, cfg.mass, cfg.omega, cfg.alpha, **kw)
+
+
+def _gpu_op(cfg, **kw):
+    from paper_1903_04670_b200 import Dgfs
+    return Dgfs.from_config(cfg, device=0, **kw)
+
+
+def _pair_errs(Qg, Qo):
+    """max over velocity nodes, per (x, p, q), relative to that array's max."""
+    num = np.max(np.abs(Qg - Qo), axis=-1)
+    den = np.max(np.abs(Qo), axis=-1)
+    return num / den
+
+
+def _rand_cfg(name, ns, N, N_rho, M, alpha_diag, omega_diag, masses, seed):
+    from workloads.configs import Config, _mean_matrix
+    return Config(name, seed, tuple(masses), _mean_matrix(omega_diag), _mean_matrix(alpha_diag),
+                  N=N, L=5.5, N_rho=N_rho, M=M, nx=3, kind="bimaxwell")
+
+
+# ------------------------------------------------------------------------------ config c0, complete
+def test_c0_all_points_all_pairs(torch_cuda):
+    torch = torch_cuda
+    from oracle.collide import collide_pairs
+    cfg = get_config("c0")
+    f = make_points(cfg, range(cfg.nx))
+    Qo = collide_pairs(_oracle_tables(cfg), f)
+    with _gpu_op(cfg) as op:
+        fd = torch.from_numpy(f).cuda()
+        Qg = op.collide_pairs(fd).cpu().numpy()
+        Qs = op.collide(fd).cpu().numpy()
+    assert _pair_errs(Qg, Qo).max() < TOL
+    Qos = Qo.sum(axis=2)
+    assert (np.max(np.abs(Qs - Qos), axis=-1) / np.max(np.abs(Qos), axis=-1)).max() < TOL
+
+
+# ------------------------------------------------------------- every supported N, VHS and VSS pairs
+@pytest.mark.parametrize("N,N_rho,M,ns,alpha", [
+    (8, 5, 12, 3, (1.0, 1.2, 1.4)),       # mixed: pair (0,0) VHS, the rest VSS
+    (16, 4, 6, 2, (1.0, 1.0)),
+    (16, 3, 12, 2, (1.3, 1.0)),
+    (24, 3, 12, 2, (1.0, 1.0)),           # radix-3 path
+    (24, 2, 6, 2, (1.0, 1.45)),
+    (32, 3, 12, 2, (1.0, 1.0)),
+    (32, 2, 6, 2, (1.4, 1.4)),
+    (48, 2, 6, 2, (1.0, 1.0)),
+    (48, 1, 6, 2, (1.0, 1.2)),
+])
+def test_small_radial_rule_every_N(torch_cuda, N, N_rho, M, ns, alpha):
+    torch = torch_cuda
+    from oracle.collide import collide_pairs
+    masses = (1.0, 2.5, 1.7)[:ns]
+    omega = (0.5, 0.81, 0.7)[:ns]
+    cfg = _rand_cfg("t", ns, N, N_rho, M, alpha, omega, masses, seed=1000 + N)
+    f = make_points(cfg, range(cfg.nx))
+    # make the input rough (exercises the Nyquist planes / complex path)
+    rng = np.random.default_rng(N)
+    f *= 1.0 + 0.05 * rng.uniform(-1, 1, f.shape)
+    Qo = collide_pairs(_oracle_tables(cfg), f)
+    with _gpu_op(cfg) as op:
+        Qg = op.collide_pairs(torch.from_numpy(f).cuda()).cpu().numpy()
+    errs = _pair_errs(Qg, Qo)
+    assert errs.max() < TOL, errs
+
+
+# ------------------------------------------------------------------------------------------- tables
+@pytest.mark.parametrize("N,alpha,table_mode", [(8, (1.0, 1.0), 0), (8, (1.0, 1.4), 0), (16, (1.3, 1.2), 0),
+                                                (8, (1.0, 1.4), 1), (24, (1.0, 1.25), 0)])
+def test_tables_match_oracle(torch_cuda, N, alpha, table_mode):
+    from oracle.quadrature import sphere_rule
+    cfg = _rand_cfg("t", 2, N, 4, 12, alpha, (0.6, 0.8), (1.0, 2.0), seed=5)
+    kw = {}
+    if table_mode == 1:
+        sp, wp = sphere_rule(32)
+        kw = dict(table_mode=1, sigma_pre=sp, w_pre=wp)
+    # the same sphere points in the same order on both sides (inputs, not results)
+    sig, wsig = sphere_rule(cfg.M)
+    tab = _oracle_tables(cfg, sigma=sig, w_sigma=wsig, **kw)
+    with _gpu_op(cfg, sigma=sig, w_sigma=wsig, **kw) as op:
+        quad = op.quadrature()
+        assert abs(quad["R"] - tab.R) < 1e-14 * tab.R
+        np.testing.assert_allclose(quad["rho"], tab.rho, rtol=1e-13, atol=0)
+        np.testing.assert_allclose(quad["w_rho"], tab.w_rho, rtol=1e-13, atol=0)
+        np.testing.assert_allclose(quad["beta"], tab.beta, rtol=1e-13, atol=0)
+        for p in range(2):
+            for q in range(2):
+                a, b, c = op.tables(p, q)
+                assert np.max(np.abs(a - tab.a)) < 1e-13 * np.max(np.abs(tab.a))
+                assert np.max(np.abs(b - tab.b[p, q])) < 1e-13 * np.max(np.abs(tab.b[p, q])), (p, q)
+                assert np.max(np.abs(c - tab.c[p, q])) < 1e-13 * np.max(np.abs(tab.c[p, q])), (p, q)
+
+
+def test_builtin_sphere_rules_are_the_oracles_point_sets(torch_cuda):
+    from oracle.quadrature import sphere_rule
+    for M in (6, 12, 32):
+        cfg = _rand_cfg("t", 1, 8, 2, M, (1.0,), (0.5,), (1.0,), seed=5)
+        with _gpu_op(cfg) as op:
+            quad = op.quadrature()
+        sig, w = sphere_rule(M)
+        key = lambda s, ww: sorted((round(x, 12), round(y, 12), round(z, 12), round(v, 12)) for (x, y, z), v in zip(s, ww))
+        assert key(quad["sigma"], quad["w_sigma"]) == key(sig, w)
+
+
+# ----------------------------------------------------------------------- edge cases of the boundary
+def test_empty_batch_and_argument_errors(torch_cuda):
+    torch = torch_cuda
+    from paper_1903_04670_b200 import api
+    cfg = get_config("c0")
+    with _gpu_op(cfg) as op:
+        f = torch.zeros((1, cfg.ns, cfg.N ** 3), dtype=torch.float64, device="cuda")
+        Q = torch.full_like(f, 7.0)
+        api.dgfs_collide(op.ctx, f, Q, 0)                 # nx = 0: no-op
+        torch.cuda.synchronize()
+        assert float(Q.min()) == 7.0
+        with pytest.raises(api.DgfsError) as e:
+            api.dgfs_collide(op.ctx, f, f, 1)             # aliasing
+        assert e.value.code == api.DGFS_EINVAL
+        with pytest.raises(api.DgfsError):
+            api.dgfs_collide(op.ctx, f, Q, -1)
+        assert api.load_library().dgfs_collide(op.ctx, None, None, 1, None) == api.DGFS_EINVAL
+        op.collide(f, Q)                                   # f = 0 => Q = 0 exactly
+        torch.cuda.synchronize()
+        assert float(Q.abs().max()) == 0.0
+        assert op.workspace_bytes(4) > 0
+        op.reserve(4)
+
+
+def test_single_species_and_single_point(torch_cuda):
+    torch = torch_cuda
+    from oracle.collide import collide
+    cfg = _rand_cfg("t", 1, 16, 5, 12, (1.0,), (1.0,), (1.0,), seed=77)     # Maxwell molecules
+    f = make_points(cfg, [0])
+    Qo = collide(_oracle_tables(cfg), f)
+    with _gpu_op(cfg) as op:
+        Qg = op.collide(torch.from_numpy(f).cuda()).cpu().numpy()
+    assert np.max(np.abs(Qg - Qo)) < TOL * np.max(np.abs(Qo))
+
+
+def test_batch_is_consistent_with_single_point_calls_and_chunking(torch_cuda, monkeypatch):
+    """Points are independent: a batched call equals per-point calls bit for bit, also when
+    the workspace budget forces several chunks and a ragged last chunk."""
+    torch = torch_cuda
+    cfg = _rand_cfg("t", 2, 16, 3, 6, (1.0, 1.3), (0.6, 0.8), (1.0, 2.0), seed=9)
+    f = torch.from_numpy(make_points(cfg, range(7))).cuda()
+    with _gpu_op(cfg) as op:
+        Qb = op.collide_pairs(f).clone()
+        for x in (0, 3, 6):
+            Q1 = op.collide_pairs(f[x:x + 1].contiguous())
+            assert torch.equal(Q1[0], Qb[x])
+    monkeypatch.setenv("DGFS_SCRATCH_MB", "2")       # forces nbx = 1..2 points per chunk
+    with _gpu_op(cfg) as op:
+        Qc = op.collide_pairs(f)
+        assert torch.equal(Qc, Qb)
+
+
+def test_output_on_side_stream_and_repeatability(torch_cuda):
+    torch = torch_cuda
+    cfg = get_config("c0")
+    f = torch.from_numpy(make_points(cfg, range(cfg.nx))).cuda()
+    with _gpu_op(cfg) as op:
+        Q0 = op.collide(f).clone()
+        s = torch.cuda.Stream()
+        s.wait_stream(torch.cuda.current_stream())
+        with torch.cuda.stream(s):
+            Q1 = op.collide(f)
+        s.synchronize()
+        assert torch.equal(Q0, Q1)
