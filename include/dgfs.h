@@ -110,6 +110,19 @@ int dgfs_get_tables(dgfs_ctx *c, int p, int q, double *a, double *b, double *cc)
  * benchmark's roofline line. */
 double dgfs_flops_per_pair_eval(const dgfs_ctx *c, int p, int q);
 
+/* Instrumentation for the benchmark.  dgfs_launch_count: number of
+ * kernels this context has enqueued since dgfs_create.  dgfs_profile_enable(on != 0): from now on
+ * every kernel launch is bracketed by a pair of CUDA events recorded on the caller's stream, and
+ * launches, elapsed time and algorithmic FLOPs are accumulated per kernel class (a few
+ * microseconds of overhead per launch; off by default).  dgfs_profile_get: entry i of
+ * dgfs_profile_count; synchronises with the recorded events; *name is owned by the library.
+ * dgfs_profile_reset: zero the accumulators. */
+long long dgfs_launch_count(const dgfs_ctx *c);
+int dgfs_profile_enable(dgfs_ctx *c, int on);
+int dgfs_profile_count(const dgfs_ctx *c);
+int dgfs_profile_get(dgfs_ctx *c, int i, const char **name, long long *launches, double *ms, double *flops);
+int dgfs_profile_reset(dgfs_ctx *c);
+
 /* 1-D mesh for dgfs_step: ne uniform elements on [x0, x1], nodal DG of polynomial degree
  * `order` on K = order+1 Gauss-Lobatto-Legendre nodes, purely diffuse walls at both ends
  * (Table 2; readings DG-1, DG-2). */

@@ -18,6 +18,8 @@ ABI_SYMBOLS = (
     "dgfs_create", "dgfs_destroy", "dgfs_last_error", "dgfs_collide", "dgfs_collide_pairs",
     "dgfs_workspace_bytes", "dgfs_reserve", "dgfs_get_quadrature", "dgfs_get_tables",
     "dgfs_flops_per_pair_eval", "dgfs_step", "dgfs_advect_rhs",
+    "dgfs_launch_count", "dgfs_profile_enable", "dgfs_profile_count", "dgfs_profile_get",
+    "dgfs_profile_reset",
 )
 
 DGFS_OK, DGFS_EINVAL, DGFS_ECUDA, DGFS_ENOMEM, DGFS_ENOSUP = 0, -1, -2, -3, -4
@@ -99,6 +101,16 @@ def load_library():
     lib.dgfs_get_tables.restype = ip
     lib.dgfs_flops_per_pair_eval.argtypes = [vp, ip, ip]
     lib.dgfs_flops_per_pair_eval.restype = C.c_double
+    lib.dgfs_launch_count.argtypes = [vp]
+    lib.dgfs_launch_count.restype = C.c_longlong
+    lib.dgfs_profile_enable.argtypes = [vp, ip]
+    lib.dgfs_profile_enable.restype = ip
+    lib.dgfs_profile_count.argtypes = [vp]
+    lib.dgfs_profile_count.restype = ip
+    lib.dgfs_profile_get.argtypes = [vp, ip, C.POINTER(C.c_char_p), C.POINTER(C.c_longlong), _dp, _dp]
+    lib.dgfs_profile_get.restype = ip
+    lib.dgfs_profile_reset.argtypes = [vp]
+    lib.dgfs_profile_reset.restype = ip
     lib.dgfs_step.argtypes = [vp, C.POINTER(_Mesh), vp, C.c_double, ip, vp]
     lib.dgfs_step.restype = ip
     lib.dgfs_advect_rhs.argtypes = [vp, C.POINTER(_Mesh), vp, vp, vp]
@@ -216,6 +228,28 @@ def dgfs_get_tables(ctx, p, q, N, N_rho, M, want=("a", "b", "c")):
     return a, b, c
 
 
+def dgfs_launch_count(ctx):
+    return int(load_library().dgfs_launch_count(ctx))
+
+
+def dgfs_profile_enable(ctx, on):
+    _check(ctx, load_library().dgfs_profile_enable(ctx, int(bool(on))))
+
+
+def dgfs_profile_reset(ctx):
+    _check(ctx, load_library().dgfs_profile_reset(ctx))
+
+
+def dgfs_profile_count(ctx):
+    return int(load_library().dgfs_profile_count(ctx))
+
+
+def dgfs_profile_get(ctx, i):
+    name, n, ms, fl = C.c_char_p(), C.c_longlong(), C.c_double(), C.c_double()
+    _check(ctx, load_library().dgfs_profile_get(ctx, int(i), C.byref(name), C.byref(n), C.byref(ms), C.byref(fl)))
+    return dict(name=name.value.decode(), launches=n.value, ms=ms.value, flops=fl.value)
+
+
 def dgfs_step(ctx, mesh, f, dt, nsteps):
     m = mesh._c()
     _check(ctx, load_library().dgfs_step(ctx, C.byref(m), _dev(f, "f"), float(dt), int(nsteps), _stream_ptr()))
@@ -292,6 +326,17 @@ class Dgfs:
 
     def flops_per_pair_eval(self, p, q):
         return dgfs_flops_per_pair_eval(self.ctx, p, q)
+
+    def launch_count(self):
+        return dgfs_launch_count(self.ctx)
+
+    def profile(self, on=None, reset=False):
+        """Per-kernel-class accumulators (list of dicts); `on` switches the event bracketing."""
+        if on is not None:
+            dgfs_profile_enable(self.ctx, on)
+        if reset:
+            dgfs_profile_reset(self.ctx)
+        return [dgfs_profile_get(self.ctx, i) for i in range(dgfs_profile_count(self.ctx))]
 
     def reserve(self, nx):
         dgfs_reserve(self.ctx, nx)

@@ -352,24 +352,41 @@ static int collide_impl(dgfs_ctx* c, const double* f, double* out, int nx, bool 
   }
   const int pen_blocks = (N2 + 127) / 128;
   const int plane_blocks = (N + W - 1) / W;
+  // algorithmic FLOPs per spatial point of each r-loop kernel (FFT3 = 15 N^3 log2 N,
+  // a 1-D pass is a third of it): phases 12 N^3, product 6 N^3, accumulate 8 N^3 (complex b) / 4 N^3 (real b)
+  const double fft3 = 15.0 * N3 * log2((double)N);
+  double fl_shift = 0, fl_zprod = 0, fl_acc = 0;
+  for (int pr = 0; pr < np; ++pr) {
+    const double M = c->M;
+    fl_shift += M * (2.0 * fft3 * 2.0 / 3.0 + 12.0 * N3);
+    fl_zprod += M * (2.0 * fft3 / 3.0 + 6.0 * N3) + (c->full[pr] ? M : 1.0) * fft3 / 3.0;
+    fl_acc += (c->full[pr] ? M * (fft3 * 2.0 / 3.0 + 8.0 * N3) : (fft3 * 2.0 / 3.0 + 4.0 * N3));
+  }
   for (int x0 = 0; x0 < nx; x0 += pl.nbx) {
     const int nb = (nx - x0 < pl.nbx) ? nx - x0 : pl.nbx;
     const int items = nb * np;
     const double* fc = f + (size_t)x0 * ns * N3;
     // S1: f^ for every species of every point of the chunk (R-2: once per species, not per pair)
-    k_zfwd_real<N><<<dim3(pen_blocks, nb * ns), 128, 0, st>>>(fc, T);
-    k_plane_fwd<N, W, 0><<<dim3(plane_blocks, nb * ns), 32 * W, smem_plane, st>>>(c->tab, T, 1, fhat, 0);
+    { ProfScope ps(c->prof, st, "k_zfwd_real", nb * ns * fft3 / 3.0);
+      k_zfwd_real<N><<<dim3(pen_blocks, nb * ns), 128, 0, st>>>(fc, T); }
+    { ProfScope ps(c->prof, st, "k_plane_fwd<store>", nb * ns * fft3 * 2.0 / 3.0);
+      k_plane_fwd<N, W, 0><<<dim3(plane_blocks, nb * ns), 32 * W, smem_plane, st>>>(c->tab, T, 1, fhat, 0); }
     cudaMemsetAsync(QG, 0, (size_t)items * N3 * sizeof(cplx), st);
     for (int r = 0; r < c->N_rho; ++r) {
-      k_shift_xy<N, W><<<dim3(N, items), 32 * W, smem_plane, st>>>(c->tab, fhat, G, r);
-      k_z_prod<N><<<dim3(pen_blocks, items), 256, smem_z, st>>>(c->tab, G, T, tsl);
-      k_plane_fwd<N, W, 1><<<dim3(plane_blocks, items), 32 * W, smem_plane, st>>>(c->tab, T, tsl, QG, r);
+      { ProfScope ps(c->prof, st, "k_shift_xy", nb * fl_shift);
+        k_shift_xy<N, W><<<dim3(N, items), 32 * W, smem_plane, st>>>(c->tab, fhat, G, r); }
+      { ProfScope ps(c->prof, st, "k_z_prod", nb * fl_zprod);
+        k_z_prod<N><<<dim3(pen_blocks, items), 256, smem_z, st>>>(c->tab, G, T, tsl); }
+      { ProfScope ps(c->prof, st, "k_plane_fwd<accumulate>", nb * fl_acc);
+        k_plane_fwd<N, W, 1><<<dim3(plane_blocks, items), 32 * W, smem_plane, st>>>(c->tab, T, tsl, QG, r); }
     }
-    k_final_xy<N><<<dim3(N, items), 64, smem_final, st>>>(c->tab, fhat, QG, G);
-    if (pairs_out)
-      k_z_final<N, false><<<dim3(pen_blocks, items), 128, 0, st>>>(c->tab, G, fc, out + (size_t)x0 * np * N3);
-    else
-      k_z_final<N, true><<<dim3(pen_blocks, nb * ns), 128, 0, st>>>(c->tab, G, fc, out + (size_t)x0 * ns * N3);
+    { ProfScope ps(c->prof, st, "k_final_xy", items * (2.0 * fft3 * 2.0 / 3.0 + 6.0 * N3));
+      k_final_xy<N><<<dim3(N, items), 64, smem_final, st>>>(c->tab, fhat, QG, G); }
+    { ProfScope ps(c->prof, st, "k_z_final", items * (2.0 * fft3 / 3.0 + 5.0 * N3));
+      if (pairs_out)
+        k_z_final<N, false><<<dim3(pen_blocks, items), 128, 0, st>>>(c->tab, G, fc, out + (size_t)x0 * np * N3);
+      else
+        k_z_final<N, true><<<dim3(pen_blocks, nb * ns), 128, 0, st>>>(c->tab, G, fc, out + (size_t)x0 * ns * N3); }
   }
   return check_cuda(c, cudaGetLastError(), "collide launch");
 }
@@ -416,6 +433,32 @@ extern "C" int dgfs_reserve(dgfs_ctx* c, int nx) {
   if (nx == 0) return DGFS_OK;
   cudaSetDevice(c->device);
   return ensure_workspace(c, plan_chunks(c, nx).total);
+}
+extern "C" long long dgfs_launch_count(const dgfs_ctx* c) { return c ? c->prof.total_launches : 0; }
+extern "C" int dgfs_profile_enable(dgfs_ctx* c, int on) {
+  if (!c) return DGFS_EINVAL;
+  c->prof.on = on != 0;
+  return DGFS_OK;
+}
+extern "C" int dgfs_profile_count(const dgfs_ctx* c) { return c ? (int)c->prof.entries.size() : 0; }
+extern "C" int dgfs_profile_get(dgfs_ctx* c, int i, const char** name, long long* launches, double* ms, double* flops) {
+  if (!c) return DGFS_EINVAL;
+  if (i < 0 || i >= (int)c->prof.entries.size()) return set_error(c, DGFS_EINVAL, "dgfs_profile_get: index out of range");
+  cudaSetDevice(c->device);
+  c->prof.drain();
+  const ProfEntry& e = c->prof.entries[i];
+  if (name) *name = e.name.c_str();
+  if (launches) *launches = e.launches;
+  if (ms) *ms = e.ms;
+  if (flops) *flops = e.flops;
+  return DGFS_OK;
+}
+extern "C" int dgfs_profile_reset(dgfs_ctx* c) {
+  if (!c) return DGFS_EINVAL;
+  cudaSetDevice(c->device);
+  c->prof.drain();
+  for (auto& e : c->prof.entries) { e.launches = 0; e.ms = 0; e.flops = 0; }
+  return DGFS_OK;
 }
 extern "C" double dgfs_flops_per_pair_eval(const dgfs_ctx* c, int p, int q) {
   if (!c || p < 0 || q < 0 || p >= c->ns || q >= c->ns) return 0.0;

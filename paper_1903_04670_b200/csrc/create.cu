@@ -188,16 +188,16 @@ __global__ void k_bfull_series(cplx* out, int p, int q, int N, int N_rho, int M,
       for (int n = 0; n <= nmax; ++n) { jn[n] = tterm * (1.0 - z * z / (2.0 * (2 * n + 3))); tterm *= z / (2 * n + 3); }
     } else {
       int nstart = nmax + 40;
-      double fp1 = 0.0, f = 1e-280, norm = 0.0;
+      double fp1 = 0.0, f = 1e-120, norm = 0.0;
       for (int n = nstart; n >= 0; --n) {
         // j_{n-1} = (2n+1)/z j_n - j_{n+1}
         if (n <= nmax) jn[n] = f;
         norm += (2 * n + 1) * f * f;
         double fm1 = (2 * n + 1) / z * f - fp1;
         fp1 = f; f = fm1;
-        if (fabs(f) > 1e250) {   // rescale to avoid overflow
-          f *= 1e-250; fp1 *= 1e-250; norm *= 1e-250 * 1e-250;
-          for (int m = n; m <= nmax; ++m) jn[m] *= 1e-250;
+        if (fabs(f) > 1e120) {   // rescale so that f^2 in the norm cannot overflow
+          f *= 1e-120; fp1 *= 1e-120; norm *= 1e-240;
+          for (int m = n; m <= nmax; ++m) jn[m] *= 1e-120;
         }
       }
       double scale = rsqrt(norm);
@@ -481,6 +481,8 @@ extern "C" void dgfs_destroy(dgfs_ctx* c) {
   cudaFree(c->d_rho); cudaFree(c->d_sigma); cudaFree(c->d_full); cudaFree(c->d_bfull);
   for (auto p : c->h_bfull) cudaFree(p);
   cudaFree(c->ws); cudaFree(c->dg_ws);
+  c->prof.drain();
+  for (auto e : c->prof.pool) cudaEventDestroy(e);
   delete c;
 }
 

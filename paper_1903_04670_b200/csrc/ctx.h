@@ -30,8 +30,54 @@ struct DevTables {
 
 }  // namespace dgfs
 
+namespace dgfs {
+// per-kernel-class accumulators behind dgfs_profile_* (include/dgfs.h)
+struct ProfEntry {
+  std::string name;
+  long long launches = 0;
+  double ms = 0.0, flops = 0.0;
+  std::vector<std::pair<cudaEvent_t, cudaEvent_t>> pending;
+};
+struct Profiler {
+  bool on = false;
+  long long total_launches = 0;
+  std::vector<ProfEntry> entries;
+  std::vector<cudaEvent_t> pool;
+  int find(const char* name) {
+    for (size_t i = 0; i < entries.size(); ++i) if (entries[i].name == name) return (int)i;
+    entries.emplace_back(); entries.back().name = name; return (int)entries.size() - 1;
+  }
+  cudaEvent_t get_event() {
+    if (!pool.empty()) { cudaEvent_t e = pool.back(); pool.pop_back(); return e; }
+    cudaEvent_t e; cudaEventCreate(&e); return e;
+  }
+  void drain() {
+    for (auto& en : entries) {
+      for (auto& pr : en.pending) {
+        cudaEventSynchronize(pr.second);
+        float t = 0; cudaEventElapsedTime(&t, pr.first, pr.second);
+        en.ms += t; pool.push_back(pr.first); pool.push_back(pr.second);
+      }
+      en.pending.clear();
+    }
+  }
+};
+// RAII bracket around one launch
+struct ProfScope {
+  Profiler& P; cudaStream_t st; int id = -1; cudaEvent_t e0{}, e1{};
+  ProfScope(Profiler& p, cudaStream_t s, const char* name, double flops) : P(p), st(s) {
+    ++P.total_launches;
+    if (!P.on) return;
+    id = P.find(name); P.entries[id].launches++; P.entries[id].flops += flops;
+    e0 = P.get_event(); e1 = P.get_event(); cudaEventRecord(e0, st);
+  }
+  ~ProfScope() { if (id >= 0) { cudaEventRecord(e1, st); P.entries[id].pending.emplace_back(e0, e1); } }
+};
+}  // namespace dgfs
+
 struct dgfs_ctx {
   int device = 0;
+  dgfs::Profiler prof;
   int ns = 0, N = 0, N_rho = 0, M = 0, npairs = 0, N3 = 0, K2n = 0;
   double L = 0, R = 0;
   int table_mode = 0;
