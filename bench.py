@@ -21,10 +21,9 @@ if ROOT not in sys.path:
 
 METRIC = "collision evals/s (spatial pts x species pairs) at N=32"
 UNIT = "pair-evals/s"
-# FP64 DFMA pipe: 148 SMs x 64 DFMA/clk/SM x 2 flop x 1.965 GHz; measured
-# with a dependent-free DFMA kernel on this pool's B200: 34.2 TFLOP/s (profiles/r01_peaks.md)
+# FP64 DFMA pipe: 148 SMs x 64 DFMA/clk/SM x 2 flop x 1.965 GHz.  The same
+# pipe is also measured live with dgfs_measure_fp64_peak (dependency-free DFMA chains) and reported.
 FP64_PEAK_NOMINAL_TFLOPS = 148 * 64 * 2 * 1.965e9 / 1e12
-FP64_PEAK_MEASURED_TFLOPS = 34.2
 PAPER_P100_PAIR_EVALS_PER_S = 1.0 / 0.01057      # Table 1 P:316 (N=32, N_rho=32, M=12), 1 x P100
 
 
@@ -213,20 +212,22 @@ def main():
     value = evals_per_step / (ms_per_step * 1e-3)
 
     # ---------------- end to end: pinned host -> device -> collide -> pinned host ----------------
+    # dgfs_collide_host: HOST pointers in and out; the library's own streams carry the copies and the
+    # kernels, and the call returns when Q is in host memory, so the region is timed on the host
+    # clock between two device synchronisations (CUDA events on torch's stream would not see it).
+    del f_dev, q_dev
+    torch.cuda.empty_cache()
+
     def e2e_step():
-        f_dev.copy_(f_host, non_blocking=True)
-        op.collide(f_dev, q_dev)
-        q_host.copy_(q_dev, non_blocking=True)
+        op.collide_host(f_host, q_host)
 
     e2e_step()
     barrier()
-    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-    e0.record(stream)
+    t0 = time.perf_counter()
     for _ in range(args.steps):
         e2e_step()
-    e1.record(stream)
     barrier()
-    t = torch.tensor([e0.elapsed_time(e1)], dtype=torch.float64, device="cuda")
+    t = torch.tensor([(time.perf_counter() - t0) * 1e3], dtype=torch.float64, device="cuda")
     if world > 1:
         dist.all_reduce(t, op=dist.ReduceOp.MAX)
     e2e_ms = float(t.item()) / args.steps
@@ -239,6 +240,8 @@ def main():
         ksum = sum(p["ms"] for p in prof)
         achieved = top["flops"] / (top["ms"] * 1e-3) / 1e12
         flops_step = sum(op.flops_per_pair_eval(p, q) for p in range(cfg.ns) for q in range(cfg.ns)) * nx
+        from paper_1903_04670_b200 import dgfs_measure_fp64_peak
+        FP64_PEAK_MEASURED_TFLOPS = dgfs_measure_fp64_peak(local, 2.0)[1]
         roofline = {
             "bound": "alu", "kernel": top["name"], "achieved": achieved, "peak": FP64_PEAK_NOMINAL_TFLOPS,
             "unit": "TFLOP/s", "frac": achieved / FP64_PEAK_NOMINAL_TFLOPS,
@@ -246,6 +249,7 @@ def main():
                            "MEASURED_PEAKS.json has no fp64 entry",
             "frac_of_measured_dfma_peak": achieved / FP64_PEAK_MEASURED_TFLOPS,
             "measured_dfma_peak": FP64_PEAK_MEASURED_TFLOPS,
+            "measured_dfma_peak_how": "dgfs_measure_fp64_peak: dependency-free DFMA chains, 2 s sustained, same box",
             "kernel_share_of_step": top["ms"] / ksum,
             "launch_ms": top["ms"] / top["launches"], "launches": top["launches"],
             "flops_per_launch": top["flops"] / top["launches"],
@@ -270,7 +274,8 @@ def main():
             "dtype": "f64", "data": "synthetic", "config": workload_desc(cfg, nx, world),
             "clocks": sampler.summary(),
             "e2e": {"value": evals_per_step / (e2e_ms * 1e-3), "unit": UNIT, "ms_per_step": e2e_ms,
-                    "h2d_bytes_per_step": nbytes, "d2h_bytes_per_step": nbytes},
+                    "h2d_bytes_per_step": nbytes, "d2h_bytes_per_step": nbytes,
+                    "call": "dgfs_collide_host (C ABI, pinned host buffers in and out, host clock)"},
             "gpu_launches": launches,
             "roofline": roofline,
             "cpu_baseline": cpu,

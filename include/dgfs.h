@@ -87,6 +87,13 @@ int dgfs_collide(dgfs_ctx *c, const double *f, double *Q, int nx, void *stream);
  * Qpq: device, [nx][ns][ns][N^3]. */
 int dgfs_collide_pairs(dgfs_ctx *c, const double *f, double *Qpq, int nx, void *stream);
 
+/* End-to-end form of dgfs_collide with HOST buffers (pageable or pinned): f_host [nx][ns][N^3] is
+ * copied to the device in slabs, collided (same kernels as dgfs_collide) and Q_host [nx][ns][N^3]
+ * is copied back; uploads, kernels and downloads of consecutive slabs overlap on the library's own
+ * streams.  Synchronous: on return Q_host is complete.  This is the call bench.py's "e2e" line
+ * times.  The device staging buffers are owned by the context and grown on demand. */
+int dgfs_collide_host(dgfs_ctx *c, const double *f_host, double *Q_host, int nx);
+
 /* Bytes of device workspace dgfs_collide* needs for a batch of nx points (tables excluded). */
 size_t dgfs_workspace_bytes(const dgfs_ctx *c, int nx);
 
@@ -122,6 +129,12 @@ int dgfs_profile_enable(dgfs_ctx *c, int on);
 int dgfs_profile_count(const dgfs_ctx *c);
 int dgfs_profile_get(dgfs_ctx *c, int i, const char **name, long long *launches, double *ms, double *flops);
 int dgfs_profile_reset(dgfs_ctx *c);
+
+/* Roofline denominator: throughput of the plain FP64 pipe of `device`
+ * measured with dependency-free DFMA chains for about `seconds` (0 < seconds <= 30): best single
+ * launch (*tflops_burst) and the average over the whole interval (*tflops_sustained). Host outputs,
+ * either may be NULL.  Synchronous; needs no context. */
+int dgfs_measure_fp64_peak(int device, double seconds, double *tflops_burst, double *tflops_sustained);
 
 /* 1-D mesh for dgfs_step: ne uniform elements on [x0, x1], nodal DG of polynomial degree
  * `order` on K = order+1 Gauss-Lobatto-Legendre nodes, purely diffuse walls at both ends

@@ -19,7 +19,7 @@ ABI_SYMBOLS = (
     "dgfs_workspace_bytes", "dgfs_reserve", "dgfs_get_quadrature", "dgfs_get_tables",
     "dgfs_flops_per_pair_eval", "dgfs_step", "dgfs_advect_rhs",
     "dgfs_launch_count", "dgfs_profile_enable", "dgfs_profile_count", "dgfs_profile_get",
-    "dgfs_profile_reset",
+    "dgfs_profile_reset", "dgfs_collide_host", "dgfs_measure_fp64_peak",
 )
 
 DGFS_OK, DGFS_EINVAL, DGFS_ECUDA, DGFS_ENOMEM, DGFS_ENOSUP = 0, -1, -2, -3, -4
@@ -91,6 +91,10 @@ def load_library():
         fn = getattr(lib, name)
         fn.argtypes = [vp, vp, vp, ip, vp]
         fn.restype = ip
+    lib.dgfs_collide_host.argtypes = [vp, vp, vp, ip]
+    lib.dgfs_collide_host.restype = ip
+    lib.dgfs_measure_fp64_peak.argtypes = [ip, C.c_double, _dp, _dp]
+    lib.dgfs_measure_fp64_peak.restype = ip
     lib.dgfs_workspace_bytes.argtypes = [vp, ip]
     lib.dgfs_workspace_bytes.restype = C.c_size_t
     lib.dgfs_reserve.argtypes = [vp, ip]
@@ -194,6 +198,34 @@ def dgfs_collide(ctx, f, Q, nx):
 
 def dgfs_collide_pairs(ctx, f, Qpq, nx):
     _check(ctx, load_library().dgfs_collide_pairs(ctx, _dev(f, "f"), _dev(Qpq, "Qpq"), int(nx), _stream_ptr()))
+
+
+def _host(t, who, n):
+    """Host fp64 buffer (numpy array or CPU torch tensor, contiguous) -> void*."""
+    if isinstance(t, np.ndarray):
+        if t.dtype != np.float64 or not t.flags.c_contiguous or t.size != n:
+            raise ValueError("%s must be a C-contiguous float64 array of %d values" % (who, n))
+        return C.c_void_p(t.ctypes.data)
+    import torch
+    if not (isinstance(t, torch.Tensor) and not t.is_cuda and t.dtype == torch.float64 and t.is_contiguous()
+            and t.numel() == n):
+        raise ValueError("%s must be a contiguous fp64 host tensor of %d values" % (who, n))
+    return C.c_void_p(t.data_ptr())
+
+
+def dgfs_collide_host(ctx, f_host, Q_host, nx, ns, N3):
+    """dgfs_collide with HOST buffers: copies in, kernels and copies out all inside the call."""
+    n = int(nx) * int(ns) * int(N3)
+    _check(ctx, load_library().dgfs_collide_host(ctx, _host(f_host, "f_host", n), _host(Q_host, "Q_host", n), int(nx)))
+
+
+def dgfs_measure_fp64_peak(device=0, seconds=1.0):
+    """(burst, sustained) TFLOP/s of the FP64 DFMA pipe, measured by the library."""
+    a, b = C.c_double(), C.c_double()
+    rc = load_library().dgfs_measure_fp64_peak(int(device), float(seconds), C.byref(a), C.byref(b))
+    if rc != DGFS_OK:
+        raise DgfsError(rc, "dgfs_measure_fp64_peak failed")
+    return a.value, b.value
 
 
 def dgfs_workspace_bytes(ctx, nx):
@@ -307,15 +339,12 @@ class Dgfs:
         return out
 
     def collide_host(self, f_host, out_host=None):
-        """End-to-end call with HOST numpy/torch buffers: H2D copy, collide, D2H copy."""
-        import torch
-        fh = torch.as_tensor(f_host)
-        fd = fh.to("cuda", non_blocking=True)
-        Q = self.collide(fd)
+        """End-to-end call with HOST numpy / CPU-torch buffers (dgfs_collide_host)."""
+        nx = int(f_host.shape[0])
         if out_host is None:
-            return Q.cpu()
-        out_host.copy_(Q, non_blocking=True)
-        torch.cuda.current_stream().synchronize()
+            out_host = np.empty((nx, self.ns, self.N3)) if isinstance(f_host, np.ndarray) else f_host.new_empty(
+                (nx, self.ns, self.N3))
+        dgfs_collide_host(self.ctx, f_host, out_host, nx, self.ns, self.N3)
         return out_host
 
     def quadrature(self):

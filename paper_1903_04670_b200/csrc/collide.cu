@@ -423,6 +423,61 @@ extern "C" int dgfs_collide(dgfs_ctx* c, const double* f, double* Q, int nx, voi
 extern "C" int dgfs_collide_pairs(dgfs_ctx* c, const double* f, double* Qpq, int nx, void* stream) {
   return collide_common(c, f, Qpq, nx, stream, true, "dgfs_collide_pairs");
 }
+// Host-buffer form: slabs of `hp_pts` points go host -> device -> kernels -> host on three streams,
+// double buffered, so that the copies of slab i+1 / i-1 overlap the kernels of slab i.
+extern "C" int dgfs_collide_host(dgfs_ctx* c, const double* f_host, double* Q_host, int nx) {
+  if (!c) return DGFS_EINVAL;
+  if (nx < 0) return set_error(c, DGFS_EINVAL, "dgfs_collide_host: nx must be >= 0");
+  if (nx == 0) return DGFS_OK;
+  if (!f_host || !Q_host) return set_error(c, DGFS_EINVAL, "dgfs_collide_host: f_host and Q_host must not be NULL");
+  cudaError_t e = cudaSetDevice(c->device);
+  if (e != cudaSuccess) return check_cuda(c, e, "cudaSetDevice");
+  const size_t per_pt = (size_t)c->ns * c->N3;
+  int slab = (int)((size_t)(128u << 20) / (per_pt * sizeof(double)));      // ~128 MiB per slab buffer
+  if (slab < 1) slab = 1;
+  if (slab > nx) slab = nx;
+  int rc;
+  if (!c->hp_stream[0]) {
+    for (int i = 0; i < 3; ++i) {
+      if ((rc = check_cuda(c, cudaStreamCreateWithFlags(&c->hp_stream[i], cudaStreamNonBlocking), "stream create"))) return rc;
+      for (int b = 0; b < 2; ++b)
+        if ((rc = check_cuda(c, cudaEventCreateWithFlags(&c->hp_ev[i][b], cudaEventDisableTiming), "event create"))) return rc;
+    }
+  }
+  if (slab > c->hp_pts) {
+    cudaDeviceSynchronize();
+    for (int b = 0; b < 2; ++b) {
+      cudaFree(c->hp_f[b]); cudaFree(c->hp_q[b]); c->hp_f[b] = c->hp_q[b] = nullptr;
+    }
+    c->hp_pts = 0;
+    for (int b = 0; b < 2; ++b) {
+      if ((rc = check_cuda(c, cudaMalloc((void**)&c->hp_f[b], slab * per_pt * sizeof(double)), "host-pipe slab allocation"))) return rc;
+      if ((rc = check_cuda(c, cudaMalloc((void**)&c->hp_q[b], slab * per_pt * sizeof(double)), "host-pipe slab allocation"))) return rc;
+    }
+    c->hp_pts = slab;
+  }
+  if ((rc = ensure_workspace(c, plan_chunks(c, slab).total))) return rc;
+  cudaStream_t s_in = c->hp_stream[0], s_k = c->hp_stream[1], s_out = c->hp_stream[2];
+  int i = 0;
+  for (int x0 = 0; x0 < nx; x0 += slab, ++i) {
+    const int n = (nx - x0 < slab) ? nx - x0 : slab, b = i & 1;
+    const size_t bytes = (size_t)n * per_pt * sizeof(double);
+    if (i >= 2) cudaStreamWaitEvent(s_in, c->hp_ev[1][b], 0);             // kernels of slab i-2 have read hp_f[b]
+    cudaMemcpyAsync(c->hp_f[b], f_host + (size_t)x0 * per_pt, bytes, cudaMemcpyHostToDevice, s_in);
+    cudaEventRecord(c->hp_ev[0][b], s_in);
+    cudaStreamWaitEvent(s_k, c->hp_ev[0][b], 0);
+    if (i >= 2) cudaStreamWaitEvent(s_k, c->hp_ev[2][b], 0);              // download of slab i-2 has read hp_q[b]
+    if ((rc = run_collide(c, c->hp_f[b], c->hp_q[b], n, false, s_k))) return rc;
+    cudaEventRecord(c->hp_ev[1][b], s_k);
+    cudaStreamWaitEvent(s_out, c->hp_ev[1][b], 0);
+    cudaMemcpyAsync(Q_host + (size_t)x0 * per_pt, c->hp_q[b], bytes, cudaMemcpyDeviceToHost, s_out);
+    cudaEventRecord(c->hp_ev[2][b], s_out);
+  }
+  for (int k = 0; k < 3; ++k)
+    if ((rc = check_cuda(c, cudaStreamSynchronize(c->hp_stream[k]), "dgfs_collide_host"))) return rc;
+  return DGFS_OK;
+}
+
 extern "C" size_t dgfs_workspace_bytes(const dgfs_ctx* c, int nx) {
   if (!c || nx <= 0) return 0;
   return plan_chunks(c, nx).total;

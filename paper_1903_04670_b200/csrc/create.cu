@@ -481,6 +481,11 @@ extern "C" void dgfs_destroy(dgfs_ctx* c) {
   cudaFree(c->d_rho); cudaFree(c->d_sigma); cudaFree(c->d_full); cudaFree(c->d_bfull);
   for (auto p : c->h_bfull) cudaFree(p);
   cudaFree(c->ws); cudaFree(c->dg_ws);
+  for (int b = 0; b < 2; ++b) { cudaFree(c->hp_f[b]); cudaFree(c->hp_q[b]); }
+  for (int i = 0; i < 3; ++i) {
+    if (c->hp_stream[i]) cudaStreamDestroy(c->hp_stream[i]);
+    for (int b = 0; b < 2; ++b) if (c->hp_ev[i][b]) cudaEventDestroy(c->hp_ev[i][b]);
+  }
   c->prof.drain();
   for (auto e : c->prof.pool) cudaEventDestroy(e);
   delete c;

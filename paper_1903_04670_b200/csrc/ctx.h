@@ -102,6 +102,12 @@ struct dgfs_ctx {
   void* ws = nullptr;
   size_t ws_bytes = 0;
   size_t scratch_budget = 0;             // bytes allowed for the transposition scratch G
+  // dgfs_collide_host: two device slabs each for f and Q, three streams, per-slab events
+  double* hp_f[2] = {nullptr, nullptr};
+  double* hp_q[2] = {nullptr, nullptr};
+  int hp_pts = 0;
+  cudaStream_t hp_stream[3] = {nullptr, nullptr, nullptr};
+  cudaEvent_t hp_ev[3][2] = {};
   // DG operator storage (dgfs_step)
   void* dg_ws = nullptr;
   size_t dg_ws_bytes = 0;

@@ -192,3 +192,26 @@ def test_output_on_side_stream_and_repeatability(torch_cuda):
             Q1 = op.collide(f)
         s.synchronize()
         assert torch.equal(Q0, Q1)
+
+
+def test_host_buffer_call_matches_device_call(torch_cuda):
+    """dgfs_collide_host (HOST pointers, slabs pipelined on the library's streams) == dgfs_collide."""
+    torch = torch_cuda
+    cfg = get_config("c0")
+    xs = [i % cfg.nx for i in range(37)]          # ragged against any slab size
+    f = make_points(cfg, xs)
+    with _gpu_op(cfg) as op:
+        Qd = op.collide(torch.from_numpy(f).cuda()).cpu().numpy()
+        Qh = op.collide_host(f)                                    # numpy, pageable
+        fh = torch.from_numpy(f).pin_memory()
+        Qp = op.collide_host(fh, torch.empty_like(fh).pin_memory()).numpy()   # pinned torch
+        from paper_1903_04670_b200 import DgfsError
+        with pytest.raises(ValueError):
+            op.collide_host(f.astype(np.float32))
+    assert np.array_equal(Qd, Qh) and np.array_equal(Qd, Qp)
+
+
+def test_fp64_peak_probe_is_plausible(torch_cuda):
+    from paper_1903_04670_b200 import dgfs_measure_fp64_peak
+    burst, sustained = dgfs_measure_fp64_peak(0, 0.2)
+    assert 5.0 < sustained <= burst < 60.0
