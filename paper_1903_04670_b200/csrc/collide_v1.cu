@@ -1,0 +1,492 @@
+// collide_v1.cu -- v1 pipeline of dgfs_collide for pairs whose b_rs does not depend on s (VHS,
+// table_mode 0): Algorithm 2 of PAPER.md with the exact rearrangements of DESIGN.md
+// section 5 (R-1, R-2, R-4, R-5, R-6, R-7).
+//
+// What is computed per pair (p,q), point x and radial node r (steps 2-8):
+//   S_r(c) = sum_s w_s Re[ A_rs(c) B_rs(c) ],   A_rs = ifft3(e^{+i mu_q a_rs} f^_p),  B_rs = ifft3(e^{-i mu_p a_rs} f^_q)
+//   QG    += w_r b_r(|k|) fft3(S_r)
+// Re[.] is exact here: b_r is real and even in k, so Im(A B) only feeds the imaginary part that step 10
+// discards.  f_p, f_q are real, hence A = a_r + i a_i with REAL fields a_r, a_i, where a_i comes
+// from the three Nyquist planes only (the shift multiplier has no conjugate partner there).  Writing each
+// 1-D factor as h_d + J s_d (v1_tables.h), with J standing for the imaginary unit that breaks the
+// Hermitian symmetry,
+//   a_r <- h_x h_y h_z - s_x s_y h_z - s_x h_y s_z - h_x s_y s_z        (spectral multipliers of f^_p)
+//   a_i <- s_x h_y h_z + h_x s_y h_z + h_x h_y s_z - s_x s_y s_z
+// and the same for B.  Two real fields share one complex transform: Z = a_r + i b_r, W = a_i + i b_i,
+// Re(A B) = Re Z Im Z - Re W Im W.
+//
+// Kernels per radial node (all spatial points of a chunk at once):
+//   k_zshift  inverse z pass of h_z f^ for every DISTINCT z shift (the sphere rules share sigma_z values:
+//             18 arrays instead of 96 at c2), on the Hermitian half of the (lx,ly) plane (R-7)
+//   k_nyq     the Nyquist-plane fields: three 2-D transforms and three 1-D sums per (pair, s)
+//   k_xy      per (pair, cz plane): for every s the inverse x,y passes of the packed field in one warp
+//             (lane = pencil, FFTs in registers, one transposition through shared memory), the product
+//             and the sum over s in registers; writes the real plane S_r(., ., cz)
+//   k_zfwd_real / k_plane_fwd<accumulate> (kernels_v0.cuh): fft3(S_r), QG += w_r b_r .
+// Steps 1 and 10 reuse the v0 kernels.
+#include <cmath>
+#include <cstdio>
+#include <cstdlib>
+#include "ctx.h"
+#include "kernels_v0.cuh"
+
+namespace dgfs {
+
+// ---------------------------------------------------------------- create-time tables ------------
+static void split_factor(double theta, int N, double scale, cplx* h, double* s) {
+  const int H = N / 2;
+  for (int j = 0; j < N; ++j) {
+    const int v = j - (j >= H ? N : 0);
+    h[j] = make_double2(cos(theta * v) * scale, sin(theta * v) * scale);
+  }
+  h[H] = make_double2(cos(theta * H) * scale, 0.0);
+  *s = -sin(theta * H) * scale;
+}
+
+template <class T>
+static int upload(dgfs_ctx* c, T** d, const std::vector<T>& h, const char* what) {
+  int rc = check_cuda(c, cudaMalloc((void**)d, h.size() * sizeof(T)), what);
+  if (rc) return rc;
+  return check_cuda(c, cudaMemcpy(*d, h.data(), h.size() * sizeof(T), cudaMemcpyHostToDevice), what);
+}
+
+int build_tables_v1(dgfs_ctx* c) {
+  const int ns = c->ns, np = c->npairs, N = c->N, Nr = c->N_rho, M = c->M;
+  const double pi = 3.14159265358979323846;
+  // distinct (species, kappa) with kappa = +mu_q sigma_z (side A acts on f^_p) or -mu_p sigma_z (side B on f^_q)
+  std::vector<double> zk;
+  c->v1_zsp.clear(); c->v1_zmap.assign((size_t)np * M * 2, 0);
+  auto zjob = [&](int sp, double kappa) {
+    for (size_t k = 0; k < zk.size(); ++k)
+      if (c->v1_zsp[k] == sp && fabs(zk[k] - kappa) <= 1e-15) return (int)k;
+    c->v1_zsp.push_back(sp); zk.push_back(kappa);
+    return (int)zk.size() - 1;
+  };
+  for (int p = 0; p < ns; ++p) for (int q = 0; q < ns; ++q) {
+    const double mu_q = c->mass[q] / (c->mass[p] + c->mass[q]), mu_p = c->mass[p] / (c->mass[p] + c->mass[q]);
+    for (int s = 0; s < M; ++s) {
+      c->v1_zmap[((size_t)(p * ns + q) * M + s) * 2 + 0] = zjob(p, mu_q * c->sigma[3 * s + 2]);
+      c->v1_zmap[((size_t)(p * ns + q) * M + s) * 2 + 1] = zjob(q, -mu_p * c->sigma[3 * s + 2]);
+    }
+  }
+  const int nz = (int)zk.size();
+  c->v1_nz = nz;
+  std::vector<cplx> hz((size_t)Nr * nz * N), hxy((size_t)np * Nr * M * 2 * 2 * N);
+  std::vector<double> szv((size_t)Nr * nz), sxy((size_t)np * Nr * M * 2 * 2);
+  for (int r = 0; r < Nr; ++r) {
+    const double rp = pi * c->rho[r] / c->L;
+    for (int k = 0; k < nz; ++k)
+      // the job's own kappa stands for every (pair, s, side) mapped to it (they agree to 1e-15)
+      split_factor(zk[k] * rp, N, 1.0 / N, &hz[((size_t)r * nz + k) * N], &szv[(size_t)r * nz + k]);
+    for (int p = 0; p < ns; ++p) for (int q = 0; q < ns; ++q) {
+      const double mu_q = c->mass[q] / (c->mass[p] + c->mass[q]), mu_p = c->mass[p] / (c->mass[p] + c->mass[q]);
+      for (int s = 0; s < M; ++s) for (int side = 0; side < 2; ++side) {
+        const double kap = side == 0 ? mu_q : -mu_p;
+        const size_t e = (((size_t)(p * ns + q) * Nr + r) * M + s) * 2 + side;
+        const double wx = (side == 0 ? c->w_sigma[s] : 1.0) / N;
+        split_factor(kap * rp * c->sigma[3 * s + 0], N, wx, &hxy[e * 2 * N], &sxy[e * 2]);
+        split_factor(kap * rp * c->sigma[3 * s + 1], N, 1.0 / N, &hxy[e * 2 * N + N], &sxy[e * 2 + 1]);
+      }
+    }
+  }
+  int rc;
+  if ((rc = upload(c, &c->d_v1_zsp, c->v1_zsp, "upload z-job species"))) return rc;
+  if ((rc = upload(c, &c->d_v1_zmap, c->v1_zmap, "upload z-job map"))) return rc;
+  if ((rc = upload(c, &c->d_v1_hz, hz, "upload z factors"))) return rc;
+  if ((rc = upload(c, &c->d_v1_szv, szv, "upload z scalars"))) return rc;
+  if ((rc = upload(c, &c->d_v1_hxy, hxy, "upload x,y factors"))) return rc;
+  if ((rc = upload(c, &c->d_v1_sxy, sxy, "upload x,y scalars"))) return rc;
+  V1Tables& t = c->v1;
+  t.nz = nz; t.zsp = c->d_v1_zsp; t.zmap = c->d_v1_zmap; t.hz = c->d_v1_hz; t.szv = c->d_v1_szv;
+  t.hxy = c->d_v1_hxy; t.sxy = c->d_v1_sxy;
+  return DGFS_OK;
+}
+
+void free_tables_v1(dgfs_ctx* c) {
+  cudaFree(c->d_v1_zsp); cudaFree(c->d_v1_zmap); cudaFree(c->d_v1_hz); cudaFree(c->d_v1_szv);
+  cudaFree(c->d_v1_hxy); cudaFree(c->d_v1_sxy);
+}
+
+// ---------------------------------------------------------------- device code -------------------
+// Half-packed spectrum (R-7): f^ of a real field is Hermitian, so columns ly = 0 .. H-1 suffice when
+// column 0 carries column H in its imaginary unit:  fhh[lz][lx][m] = f^(lx, m, lz) for m >= 1,
+// f^(lx, 0, lz) + i f^(lx, H, lz) for m = 0.  Both packed columns are spectra (in lx, lz) of real
+// fields, so they separate again as Re / Im once the x and z transforms are done.
+template <int N>
+__global__ void __launch_bounds__(256) k_pack_half(const cplx* __restrict__ fhat, cplx* __restrict__ fhh, int narr) {
+  constexpr int H = N / 2;
+  const size_t total = (size_t)narr * N * N * H;
+  for (size_t i = blockIdx.x * (size_t)blockDim.x + threadIdx.x; i < total; i += (size_t)gridDim.x * blockDim.x) {
+    const int m = (int)(i % H);
+    const size_t row = i / H;                       // (array, lz, lx)
+    cplx v = fhat[row * N + m];
+    if (m == 0) { cplx w = fhat[row * N + H]; v.x -= w.y; v.y += w.x; }
+    fhh[i] = v;
+  }
+}
+
+// Inverse z pass of h_z f^ for z job k = blockIdx.y of point blockIdx.z; thread per (lx, m) pencil.
+// in: fhh[xl][species][lz][lx][m];  out: Gz[xl][k][cz][lx][m].
+template <int N>
+__global__ void __launch_bounds__(128) k_zshift(V1Tables t, int ns, const cplx* __restrict__ fhh, cplx* __restrict__ Gz, int r) {
+  constexpr int H = N / 2, NP = N * H;
+  const int pid = blockIdx.x * 128 + threadIdx.x;
+  if (pid >= NP) return;
+  const int k = blockIdx.y, xl = blockIdx.z;
+  const cplx* src = fhh + ((size_t)xl * ns + t.zsp[k]) * (size_t)(N * NP) + pid;
+  const cplx* hz = t.hz + ((size_t)r * t.nz + k) * N;
+  cplx v[N];
+#pragma unroll
+  for (int i = 0; i < N; ++i) v[i] = cmul(src[(size_t)i * NP], __ldg(&hz[i]));
+  fft_reg<N, +1>(v);
+  cplx* dst = Gz + ((size_t)xl * t.nz + k) * (size_t)(N * NP) + pid;
+#pragma unroll
+  for (int i = 0; i < N; ++i) dst[(size_t)i * NP] = v[i];
+}
+
+// x * (a + i b) for packed side B:  i * x
+__device__ __forceinline__ cplx cmul_i(cplx x) { return make_double2(-x.y, x.x); }
+
+// Nyquist-plane fields of one (item = point x pair, s): block (s, item), 4 warps.
+//   warp 0: uz[cy][cx]  = ifft_xy[ h_x h_y s_z f^(., ., H) ]        warp 1: uxp[cz][cy] = ifft_yz[ s_x h_y h_z f^(H, ., .) ] - (-1)^{cy+cz} s_x s_y s_z f^(H,H,H)
+//   warp 2: uy[cz][cx]  = ifft_xz[ h_x s_y h_z f^(., H, .) ]        warp 3: the 1-D corrections vyh, vxp, vzp
+// every field packed as (side A) + i (side B); each side's field is real.
+template <int N>
+__global__ void __launch_bounds__(128) k_nyq(V1Tables t, DevTables tab, const cplx* __restrict__ fhat, cplx* __restrict__ nyq, int r) {
+  constexpr int H = N / 2, N2 = N * N, N3 = N2 * N;
+  typedef NyqLayout<N> NL;
+  extern __shared__ cplx sm[];
+  const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+  const int s = blockIdx.x, item = blockIdx.y;
+  const int pair = item % tab.npairs, xl = item / tab.npairs;
+  const int p = pair / tab.ns, q = pair % tab.ns;
+  const cplx* FA = fhat + ((size_t)xl * tab.ns + p) * N3;
+  const cplx* FB = fhat + ((size_t)xl * tab.ns + q) * N3;
+  const size_t e = (((size_t)pair * tab.N_rho + r) * tab.M + s) * 2;
+  const cplx *hxA = t.hxy + e * 2 * N, *hyA = hxA + N, *hxB = hxA + 2 * N, *hyB = hxA + 3 * N;
+  const double sxA = t.sxy[e * 2], syA = t.sxy[e * 2 + 1], sxB = t.sxy[e * 2 + 2], syB = t.sxy[e * 2 + 3];
+  const int kA = t.zmap[((size_t)pair * tab.M + s) * 2], kB = t.zmap[((size_t)pair * tab.M + s) * 2 + 1];
+  const cplx *hzA = t.hz + ((size_t)r * t.nz + kA) * N, *hzB = t.hz + ((size_t)r * t.nz + kB) * N;
+  const double szA = t.szv[(size_t)r * t.nz + kA], szB = t.szv[(size_t)r * t.nz + kB];
+  cplx* out = nyq + ((size_t)item * tab.M + s) * NL::STRIDE;
+  cplx* buf = sm + (size_t)warp * (N * (N + 1));
+  auto pack = [](cplx fa, cplx ha, double sa, cplx fb, cplx hb, double sb) {
+    cplx a = cmul(fa, ha), b = cmul(fb, hb);
+    return make_double2(sa * a.x - sb * b.y, sa * a.y + sb * b.x);
+  };
+  auto none = [](cplx x, int) { return x; };
+  if (warp == 0) {
+    warp_plane_fft<N, +1>(
+        buf, lane,
+        [&](int lx, int ly) {
+          const size_t i = (size_t)H * N2 + lx * N + ly;
+          return pack(FA[i], cmul(hxA[lx], hyA[ly]), szA, FB[i], cmul(hxB[lx], hyB[ly]), szB);
+        },
+        none, [&](int cy, int cx, cplx val) { out[NL::UZ + cy * N + cx] = val; });
+  } else if (warp == 1) {
+    const double tA = sxA * syA * szA * FA[(size_t)H * N2 + H * N + H].x, tB = sxB * syB * szB * FB[(size_t)H * N2 + H * N + H].x;
+    warp_plane_fft<N, +1>(
+        buf, lane,
+        [&](int lz, int ly) {
+          const size_t i = (size_t)lz * N2 + H * N + ly;
+          return pack(FA[i], cmul(hzA[lz], hyA[ly]), sxA, FB[i], cmul(hzB[lz], hyB[ly]), sxB);
+        },
+        none,
+        [&](int cy, int cz, cplx val) {
+          const double sg = ((cy + cz) & 1) ? -1.0 : 1.0;
+          out[NL::UXP + cz * N + cy] = make_double2(val.x - sg * tA, val.y - sg * tB);
+        });
+  } else if (warp == 2) {
+    warp_plane_fft<N, +1>(
+        buf, lane,
+        [&](int lz, int lx) {
+          const size_t i = (size_t)lz * N2 + lx * N + H;
+          return pack(FA[i], cmul(hzA[lz], hxA[lx]), syA, FB[i], cmul(hzB[lz], hxB[lx]), syB);
+        },
+        none, [&](int cx, int cz, cplx val) { out[NL::UY + cz * N + cx] = val; });
+  } else {
+    cplx* roots = buf;            // e^{2 pi i k / N}
+    cplx* inx = buf + N;
+    cplx* inz = buf + 2 * N;
+    for (int k = lane; k < N; k += 32) {
+      double sn, cs; sincospi(2.0 * k / N, &sn, &cs);
+      roots[k] = make_double2(cs, sn);
+      // vxp: column ly = H of plane lz = H;  vzp: the (H,H) pencil along lz
+      const size_t ix = (size_t)H * N2 + k * N + H, iz = (size_t)k * N2 + H * N + H;
+      inx[k] = pack(FA[ix], hxA[k], syA * szA, FB[ix], hxB[k], syB * szB);
+      inz[k] = pack(FA[iz], hzA[k], sxA * syA, FB[iz], hzB[k], sxB * syB);
+      // vyh: row lx = H of plane lz = H in lane format (side, m), without the y factor
+      const int side = k / H, m = k % H;
+      const cplx* F = side ? FB : FA;
+      const double sc = side ? sxB * szB : sxA * szA;
+      const size_t iy = (size_t)H * N2 + H * N;
+      cplx v = F[iy + m];
+      if (m == 0) v = make_double2(v.x, F[iy + H].x);
+      out[NL::VYH + k] = make_double2(sc * v.x, sc * v.y);
+    }
+    __syncwarp();
+    for (int c = lane; c < N; c += 32) {
+      cplx ax = make_double2(0, 0), az = make_double2(0, 0);
+      for (int l = 0; l < N; ++l) {
+        const cplx w = roots[(l * c) % N];
+        ax = cfma(inx[l], w, ax);
+        az = cfma(inz[l], w, az);
+      }
+      out[NL::VXP + c] = ax;
+      out[NL::VZP + c] = az;
+    }
+  }
+}
+
+// The r-loop's main kernel: block (cz, item), W warps; warp w handles s = w, w + W, ...
+//   pass 1 (lane = (side, m), m = Hermitian-half column): v[lx] = Gz_side(lx, m, cz) h_x,side[lx]; inverse x
+//           pass in registers; y factor of the lane's column; transposition through shared memory
+//   pass 2 (lane = cx): rebuild the 32 packed columns X[ly] = Y_A + i Y_B (mirror half by conjugation),
+//           inverse y pass, Z = a_r + i b_r; W from the Nyquist fields; acc[cy] += Re Z Im Z - Re W Im W
+// out: S[item][cz][cy][cx] (real).
+template <int N, int W>
+__global__ void __launch_bounds__(32 * W) k_xy(V1Tables t, DevTables tab, const cplx* __restrict__ Gz,
+                                               const cplx* __restrict__ nyq, double* __restrict__ S, int r) {
+  constexpr int H = N / 2, P = N + 1, NH = N * H, N2 = N * N;
+  typedef NyqLayout<N> NL;
+  static_assert(N <= 32, "one lane per pencil");
+  extern __shared__ cplx sm[];
+  const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+  const int cz = blockIdx.x, item = blockIdx.y;
+  const int pair = item % tab.npairs, xl = item / tab.npairs;
+  cplx* buf = sm + (size_t)warp * (N * P);
+  const bool act = lane < N;
+  const int ln = act ? lane : 0;
+  const int side = ln / H, m = ln % H;
+  const double szs = (cz & 1) ? -1.0 : 1.0;
+  const double sxb = (ln & 1) ? -1.0 : 1.0;
+  double acc[N];
+#pragma unroll
+  for (int j = 0; j < N; ++j) acc[j] = 0.0;
+  for (int s = warp; s < tab.M; s += W) {
+    const int k = t.zmap[((size_t)pair * tab.M + s) * 2 + side];
+    const cplx* g = Gz + ((size_t)xl * t.nz + k) * (size_t)(N * NH) + (size_t)cz * NH + m;
+    const cplx* hx = t.hxy + ((((size_t)pair * tab.N_rho + r) * tab.M + s) * 2 + side) * 2 * N;
+    const cplx* nq = nyq + ((size_t)item * tab.M + s) * NL::STRIDE;
+    if (act) {
+      cplx v[N];
+#pragma unroll
+      for (int i = 0; i < N; ++i) v[i] = cmul(g[i * H], __ldg(&hx[i]));
+      {
+        const cplx c1 = nq[NL::VYH + ln];
+        v[H].x = fma(-szs, c1.x, v[H].x);
+        v[H].y = fma(-szs, c1.y, v[H].y);
+      }
+      fft_reg<N, +1>(v);
+      // y factor: complex h_y[m] for m >= 1; for the packed lane m = 0 the real parts of h_y[0], h_y[H]
+      // scale Re (column 0) and Im (column H) separately
+      const cplx hy0 = __ldg(&hx[N + m]);
+      const double hyH = __ldg(&hx[N + H]).x;
+      const double ya = hy0.x, yb = (m == 0) ? 0.0 : -hy0.y, yc = (m == 0) ? 0.0 : hy0.y, yd = (m == 0) ? hyH : hy0.x;
+#pragma unroll
+      for (int i = 0; i < N; ++i)
+        buf[i * P + ln] = make_double2(fma(v[i].x, ya, v[i].y * yb), fma(v[i].x, yc, v[i].y * yd));
+    }
+    __syncwarp();
+    if (act) {
+      const cplx* row = buf + ln * P;
+      cplx X[N];
+      {
+        const cplx a0 = row[0], b0 = row[H];
+        const cplx vx = nq[NL::VXP + ln], vz = nq[NL::VZP + cz];
+        X[0] = make_double2(a0.x, b0.x);
+        X[H] = make_double2(a0.y - szs * vx.x - sxb * vz.x, b0.y - szs * vx.y - sxb * vz.y);
+      }
+#pragma unroll
+      for (int mm = 1; mm < H; ++mm) {
+        const cplx ya = row[mm], yb = row[H + mm];
+        X[mm] = make_double2(ya.x - yb.y, ya.y + yb.x);
+        X[N - mm] = make_double2(ya.x + yb.y, yb.x - ya.y);
+      }
+      fft_reg<N, +1>(X);
+      const cplx uyv = nq[NL::UY + cz * N + ln];
+      const cplx* uxp = nq + NL::UXP + cz * N;
+      const cplx* uz = nq + NL::UZ + ln;
+#pragma unroll
+      for (int j = 0; j < N; ++j) {
+        const cplx ux = __ldg(&uxp[j]);
+        const cplx uzv = uz[j * N];
+        const double syj = (j & 1) ? -1.0 : 1.0;
+        const double wx = fma(sxb, ux.x, fma(szs, uzv.x, syj * uyv.x));
+        const double wy = fma(sxb, ux.y, fma(szs, uzv.y, syj * uyv.y));
+        acc[j] = fma(X[j].x, X[j].y, fma(-wx, wy, acc[j]));
+      }
+    }
+    __syncwarp();
+  }
+  // sum the W partial planes through shared memory and write S(., ., cz)
+  __syncthreads();
+  double* red = reinterpret_cast<double*>(sm);            // [W][N][N] doubles <= W * N * P cplx
+  if (act) {
+#pragma unroll
+    for (int j = 0; j < N; ++j) red[(warp * N + j) * N + ln] = acc[j];
+  }
+  __syncthreads();
+  double* o = S + ((size_t)item * N + cz) * N2;
+  for (int e2 = threadIdx.x; e2 < N2; e2 += 32 * W) {
+    double sum = 0.0;
+#pragma unroll
+    for (int w = 0; w < W; ++w) sum += red[w * N2 + e2];
+    o[e2] = sum;
+  }
+}
+
+// forward z pass of the real field S[item][cz][cy][cx] (thread per (cy,cx) pencil) -> T[item][kz][cy][cx]
+template <int N>
+__global__ void __launch_bounds__(128) k_zfwd_planes(const double* __restrict__ S, cplx* __restrict__ T) {
+  constexpr int N2 = N * N, N3 = N2 * N;
+  const int pid = blockIdx.x * 128 + threadIdx.x;
+  if (pid >= N2) return;
+  const double* src = S + (size_t)blockIdx.y * N3 + pid;
+  cplx v[N];
+#pragma unroll
+  for (int i = 0; i < N; ++i) v[i] = make_double2(src[(size_t)i * N2], 0.0);
+  fft_reg<N, -1>(v);
+  cplx* dst = T + (size_t)blockIdx.y * N3 + pid;
+#pragma unroll
+  for (int k = 0; k < N; ++k) dst[(size_t)k * N2] = v[k];
+}
+
+// ---------------------------------------------------------------- host orchestration ------------
+namespace {
+struct PlanV1 {
+  int nbx;
+  size_t off_fhat, off_fhh, off_qg, off_gz, off_nyq, off_s, off_t, total;
+};
+PlanV1 plan_v1(const dgfs_ctx* c, int nx) {
+  PlanV1 pl{};
+  const size_t N = c->N, N3 = c->N3, arr = N3 * sizeof(cplx);
+  int nbx = c->v1_chunk;
+  if (nbx > nx) nbx = nx;
+  if (nbx < 1) nbx = 1;
+  if ((size_t)nbx * c->npairs > 65535) nbx = 65535 / c->npairs;
+  pl.nbx = nbx;
+  const size_t items = (size_t)nbx * c->npairs;
+  const size_t nyq_stride = 4 * N + 3 * N * N;
+  size_t gz = (size_t)nbx * c->v1_nz * (arr / 2), g2 = items * 2 * arr;
+  size_t off = 0;
+  auto take = [&](size_t bytes) { size_t o = off; off += (bytes + 255) & ~(size_t)255; return o; };
+  pl.off_fhat = take((size_t)nbx * c->ns * arr);
+  pl.off_fhh = take((size_t)nbx * c->ns * (arr / 2));
+  pl.off_qg = take(items * arr);
+  pl.off_gz = take(gz > g2 ? gz : g2);
+  pl.off_nyq = take(items * c->M * nyq_stride * sizeof(cplx));
+  pl.off_s = take(items * N3 * sizeof(double));
+  pl.off_t = take(items * arr);
+  pl.total = off;
+  return pl;
+}
+}  // namespace
+
+size_t workspace_bytes_v1(const dgfs_ctx* c, int nx) { return plan_v1(c, nx).total; }
+
+// algorithmic FLOPs of the executed algorithm: a 1-D transform of length N counts
+// 5 N log2 N, pointwise work counts the real operations of the formulas in this file's header.
+namespace {
+struct FlopsV1 { double zshift, nyq, xy, zfwd, acc, per_r, tail; };
+FlopsV1 flops_v1(const dgfs_ctx* c) {
+  const double N = c->N, N2 = N * N, N3 = N2 * N, H = N / 2, M = c->M;
+  const double fft1 = 5.0 * N * log2(N), fft3 = 3.0 * N2 * fft1;
+  FlopsV1 f{};
+  f.zshift = (double)c->v1_nz / c->npairs * N * H * (fft1 + 6.0 * N);   // per item
+  f.nyq = M * (3.0 * (2.0 * N * fft1 + 28.0 * N2) + 16.0 * N2);
+  f.xy = M * N * (2.0 * N * fft1 + 28.0 * N2);
+  f.zfwd = N2 * fft1;
+  f.acc = 2.0 * N2 * fft1 + 4.0 * N3;
+  f.per_r = f.zshift + f.nyq + f.xy + f.zfwd + f.acc;
+  f.tail = 2.0 * fft3 + 11.0 * N3 + fft3 / c->ns;
+  return f;
+}
+}  // namespace
+
+double flops_per_pair_eval_v1(const dgfs_ctx* c) {
+  const FlopsV1 f = flops_v1(c);
+  return c->N_rho * f.per_r + f.tail;
+}
+
+template <int N>
+static int collide_v1_impl(dgfs_ctx* c, const double* f, double* out, int nx, bool pairs_out, cudaStream_t st) {
+  constexpr int N2 = N * N, N3 = N2 * N, H = N / 2;
+  constexpr int W = 4;
+  const PlanV1 pl = plan_v1(c, nx);
+  int rc = ensure_workspace(c, pl.total);
+  if (rc) return rc;
+  char* ws = (char*)c->ws;
+  cplx* fhat = (cplx*)(ws + pl.off_fhat);
+  cplx* fhh = (cplx*)(ws + pl.off_fhh);
+  cplx* QG = (cplx*)(ws + pl.off_qg);
+  cplx* Gz = (cplx*)(ws + pl.off_gz);
+  cplx* nyq = (cplx*)(ws + pl.off_nyq);
+  double* S = (double*)(ws + pl.off_s);
+  cplx* T = (cplx*)(ws + pl.off_t);
+  const int ns = c->ns, np = c->npairs, nz = c->v1_nz;
+  const size_t smem_plane = plane_smem_per_warp<N>() * W;
+  const size_t smem_final = plane_smem_per_warp<N>() * 2;
+  const size_t smem_xy = sizeof(cplx) * (size_t)W * N * (N + 1);
+  const size_t smem_nyq = sizeof(cplx) * (size_t)4 * N * (N + 1);
+  static bool attr_done = false;
+  if (!attr_done) {
+    cudaFuncSetAttribute(k_plane_fwd<N, W, 0>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_plane);
+    cudaFuncSetAttribute(k_plane_fwd<N, W, 1>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_plane);
+    cudaFuncSetAttribute(k_final_xy<N>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_final);
+    cudaFuncSetAttribute(k_xy<N, W>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_xy);
+    cudaFuncSetAttribute(k_nyq<N>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_nyq);
+    attr_done = true;
+  }
+  const int pen_blocks = (N2 + 127) / 128;
+  const int hpen_blocks = (N * H + 127) / 128;
+  const int plane_blocks = (N + W - 1) / W;
+  const double fft3 = 15.0 * N3 * log2((double)N);
+  const FlopsV1 fl = flops_v1(c);
+  for (int x0 = 0; x0 < nx; x0 += pl.nbx) {
+    const int nb = (nx - x0 < pl.nbx) ? nx - x0 : pl.nbx;
+    const int items = nb * np;
+    const double* fc = f + (size_t)x0 * ns * N3;
+    // step 1, once per species (R-2), plus the half-packed copy
+    { ProfScope ps(c->prof, st, "k_zfwd_real", nb * ns * fft3 / 3.0);
+      k_zfwd_real<N><<<dim3(pen_blocks, nb * ns), 128, 0, st>>>(fc, T); }
+    { ProfScope ps(c->prof, st, "k_plane_fwd<store>", nb * ns * fft3 * 2.0 / 3.0);
+      k_plane_fwd<N, W, 0><<<dim3(plane_blocks, nb * ns), 32 * W, smem_plane, st>>>(c->tab, T, 1, fhat, 0); }
+    { ProfScope ps(c->prof, st, "k_pack_half", 0.0);
+      k_pack_half<N><<<(nb * ns * N2 * H + 255) / 256, 256, 0, st>>>(fhat, fhh, nb * ns); }
+    cudaMemsetAsync(QG, 0, (size_t)items * N3 * sizeof(cplx), st);
+    for (int r = 0; r < c->N_rho; ++r) {
+      { ProfScope ps(c->prof, st, "k_zshift", items * fl.zshift);
+        k_zshift<N><<<dim3(hpen_blocks, nz, nb), 128, 0, st>>>(c->v1, ns, fhh, Gz, r); }
+      { ProfScope ps(c->prof, st, "k_nyq", items * fl.nyq);
+        k_nyq<N><<<dim3(c->M, items), 128, smem_nyq, st>>>(c->v1, c->tab, fhat, nyq, r); }
+      { ProfScope ps(c->prof, st, "k_xy", items * fl.xy);
+        k_xy<N, W><<<dim3(N, items), 32 * W, smem_xy, st>>>(c->v1, c->tab, Gz, nyq, S, r); }
+      { ProfScope ps(c->prof, st, "k_zfwd_planes", items * fl.zfwd);
+        k_zfwd_planes<N><<<dim3(pen_blocks, items), 128, 0, st>>>(S, T); }
+      { ProfScope ps(c->prof, st, "k_plane_fwd<accumulate>", items * fl.acc);
+        k_plane_fwd<N, W, 1><<<dim3(plane_blocks, items), 32 * W, smem_plane, st>>>(c->tab, T, 1, QG, r); }
+    }
+    // step 10
+    { ProfScope ps(c->prof, st, "k_final_xy", items * (2.0 * fft3 * 2.0 / 3.0 + 6.0 * N3));
+      k_final_xy<N><<<dim3(N, items), 64, smem_final, st>>>(c->tab, fhat, QG, Gz); }
+    { ProfScope ps(c->prof, st, "k_z_final", items * (2.0 * fft3 / 3.0 + 5.0 * N3));
+      if (pairs_out)
+        k_z_final<N, false><<<dim3(pen_blocks, items), 128, 0, st>>>(c->tab, Gz, fc, out + (size_t)x0 * np * N3);
+      else
+        k_z_final<N, true><<<dim3(pen_blocks, nb * ns), 128, 0, st>>>(c->tab, Gz, fc, out + (size_t)x0 * ns * N3); }
+  }
+  return check_cuda(c, cudaGetLastError(), "collide (v1) launch");
+}
+
+int run_collide_v1(dgfs_ctx* c, const double* f, double* out, int nx, bool pairs_out, cudaStream_t st) {
+  switch (c->N) {
+    case 8: return collide_v1_impl<8>(c, f, out, nx, pairs_out, st);
+    case 16: return collide_v1_impl<16>(c, f, out, nx, pairs_out, st);
+    case 24: return collide_v1_impl<24>(c, f, out, nx, pairs_out, st);
+    case 32: return collide_v1_impl<32>(c, f, out, nx, pairs_out, st);
+  }
+  return set_error(c, DGFS_ENOSUP, "v1 pipeline: unsupported N");
+}
+
+}  // namespace dgfs

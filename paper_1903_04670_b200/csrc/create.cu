@@ -470,6 +470,16 @@ extern "C" int dgfs_create(const dgfs_params* P, dgfs_ctx** out) {
   c->scratch_budget = (size_t)(env ? atol(env) : 3072) << 20;
   int rc = build_tables(c);
   if (rc != DGFS_OK) { g_create_error = c->err; dgfs_destroy(c); return rc; }
+  // pipeline choice: v1 (collide_v1.cu) needs b independent of s for every pair and one lane per pencil;
+  // DGFS_PIPELINE=v0 forces the stage-per-kernel pipeline (used by the parity tests to cover both)
+  const char* pipe = getenv("DGFS_PIPELINE");
+  c->use_v1 = !c->any_full && N <= 32 && !(pipe && std::string(pipe) == "v0");
+  if (c->use_v1) {
+    const char* ch = getenv("DGFS_V1_CHUNK");
+    if (ch && atoi(ch) > 0) c->v1_chunk = atoi(ch);
+    rc = build_tables_v1(c);
+    if (rc != DGFS_OK) { g_create_error = c->err; dgfs_destroy(c); return rc; }
+  }
   *out = c;
   return DGFS_OK;
 }
@@ -481,6 +491,7 @@ extern "C" void dgfs_destroy(dgfs_ctx* c) {
   cudaFree(c->d_rho); cudaFree(c->d_sigma); cudaFree(c->d_full); cudaFree(c->d_bfull);
   for (auto p : c->h_bfull) cudaFree(p);
   cudaFree(c->ws); cudaFree(c->dg_ws);
+  free_tables_v1(c);
   for (int b = 0; b < 2; ++b) { cudaFree(c->hp_f[b]); cudaFree(c->hp_q[b]); }
   for (int i = 0; i < 3; ++i) {
     if (c->hp_stream[i]) cudaStreamDestroy(c->hp_stream[i]);

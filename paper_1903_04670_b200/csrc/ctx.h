@@ -5,6 +5,7 @@
 #include <vector>
 #include "../../include/dgfs.h"
 #include "fft_reg.cuh"
+#include "v1_tables.h"
 
 namespace dgfs {
 
@@ -98,6 +99,15 @@ struct dgfs_ctx {
   double* d_sigma = nullptr;
   unsigned char* d_full = nullptr;
   dgfs::DevTables tab{};
+  // v1 pipeline (collide_v1.cu): tables built by build_tables_v1, used when no pair needs the full b table
+  bool use_v1 = false;
+  int v1_chunk = 8;                      // spatial points per launch group (sized for the L2)
+  int v1_nz = 0;
+  std::vector<int> v1_zsp, v1_zmap;
+  int *d_v1_zsp = nullptr, *d_v1_zmap = nullptr;
+  dgfs::cplx *d_v1_hz = nullptr, *d_v1_hxy = nullptr;
+  double *d_v1_szv = nullptr, *d_v1_sxy = nullptr;
+  dgfs::V1Tables v1{};
   // workspace (grown on demand)
   void* ws = nullptr;
   size_t ws_bytes = 0;
@@ -129,5 +139,11 @@ struct ChunkPlan {
 ChunkPlan plan_chunks(const dgfs_ctx* c, int nx);
 int run_collide(dgfs_ctx* c, const double* f, double* out, int nx, bool pairs_out, cudaStream_t st);
 int ensure_workspace(dgfs_ctx* c, size_t bytes);
+// collide_v1.cu
+int build_tables_v1(dgfs_ctx* c);
+void free_tables_v1(dgfs_ctx* c);
+size_t workspace_bytes_v1(const dgfs_ctx* c, int nx);
+int run_collide_v1(dgfs_ctx* c, const double* f, double* out, int nx, bool pairs_out, cudaStream_t st);
+double flops_per_pair_eval_v1(const dgfs_ctx* c);
 
 }  // namespace dgfs

@@ -1,0 +1,36 @@
+// v1_tables.h -- create-time tables of the v1 collision pipeline (internal, not part of the ABI).
+//
+// The shift e^{i theta.l} of Algorithm 2 steps 4-5 (a_rs of Algo 1 step 7,
+// P:185, is linear in l) is a product of three 1-D factors.  Each factor is split into the part that
+// keeps the spectrum of a real field Hermitian ("h": e^{i theta_d v} for |v| < N/2, cos(theta_d N/2)
+// on the Nyquist index) and the part that does not ("s" = -sin(theta_d N/2), Nyquist index only);
+// DESIGN.md section 5, R-6.  1/N per axis (unnormalised inverse transforms, reading C-3) and the
+// sphere weight w_s (side A, x axis) are folded into both parts.
+#pragma once
+#include "fft_reg.cuh"
+
+namespace dgfs {
+
+struct V1Tables {
+  int nz;                    // number of distinct z shifts ("z jobs") per radial node
+  const int* zsp;            // [nz]                 species whose spectrum the job shifts
+  const int* zmap;           // [pair][s][side]      -> z job
+  const cplx* hz;            // [r][nz][N]           Hermitian-preserving z factor (1/N folded)
+  const double* szv;         // [r][nz]              anti-Hermitian z scalar (1/N folded)
+  const cplx* hxy;           // [pair][r][s][side][2][N]   x factors then y factors
+  const double* sxy;         // [pair][r][s][side][2]      anti-Hermitian x, y scalars
+};
+
+// per (item, s) block of Nyquist-plane fields written by k_nyq, in units of cplx
+template <int N>
+struct NyqLayout {
+  static constexpr int VYH = 0;            // [N]     lane format, x-Nyquist row correction (no y factor)
+  static constexpr int VXP = N;            // [N]     packed (A + iB), y-Nyquist column correction
+  static constexpr int VZP = 2 * N;        // [N]     packed, (H,H) element correction per cz
+  static constexpr int UXP = 4 * N;        // [cz][cy]
+  static constexpr int UY = 4 * N + N * N; // [cz][cx]
+  static constexpr int UZ = 4 * N + 2 * N * N;   // [cy][cx]
+  static constexpr int STRIDE = 4 * N + 3 * N * N;
+};
+
+}  // namespace dgfs

@@ -74,6 +74,44 @@ def test_c0_all_points_all_pairs(torch_cuda):
     (48, 1, 6, 2, (1.0, 1.2)),
 ])
 def test_small_radial_rule_every_N(torch_cuda, N, N_rho, M, ns, alpha):
+    _small_radial_rule(torch_cuda, N, N_rho, M, ns, alpha)
+
+
+@pytest.mark.parametrize("N,N_rho,M,ns", [(8, 3, 6, 2), (16, 2, 12, 2), (32, 2, 12, 2)])
+def test_v0_pipeline_on_vhs_pairs(torch_cuda, monkeypatch, N, N_rho, M, ns):
+    """All-VHS configurations default to the v1 pipeline; DGFS_PIPELINE=v0 keeps the stage-per-kernel
+    pipeline (the one VSS pairs and N = 48 use) covered on the same inputs."""
+    monkeypatch.setenv("DGFS_PIPELINE", "v0")
+    _small_radial_rule(torch_cuda, N, N_rho, M, ns, (1.0,) * ns)
+
+
+@pytest.mark.parametrize("N,N_rho,M,ns,noise", [
+    (8, 4, 32, 2, 0.3),        # 32-point rule: 11 distinct sigma_z values
+    (8, 3, 12, 3, 0.5),        # 9 pairs, strongly rough input: the Nyquist-plane terms are O(1) of the result
+    (16, 2, 32, 1, 0.3),       # single species: sides A and B share their z shifts
+    (32, 2, 6, 2, 0.3),        # octahedron: sigma with two zero components
+])
+def test_v1_nyquist_terms(torch_cuda, N, N_rho, M, ns, noise):
+    _small_radial_rule(torch_cuda, N, N_rho, M, ns, (1.0,) * ns, noise=noise)
+
+
+def test_v1_user_sphere_rule_without_symmetry(torch_cuda):
+    """A caller-supplied sigma set with no shared sigma_z values (every z shift is its own job)."""
+    torch = torch_cuda
+    from oracle.collide import collide_pairs
+    rng = np.random.default_rng(5)
+    M = 7
+    sig = rng.normal(size=(M, 3)); sig /= np.linalg.norm(sig, axis=1)[:, None]
+    w = rng.uniform(0.5, 1.5, M); w *= 4 * np.pi / w.sum()
+    cfg = _rand_cfg("t", 2, 16, 3, M, (1.0, 1.0), (0.5, 0.9), (1.0, 3.0), seed=21)
+    f = make_points(cfg, range(cfg.nx)) * (1.0 + 0.2 * rng.uniform(-1, 1, (cfg.nx, 2, 16 ** 3)))
+    Qo = collide_pairs(_oracle_tables(cfg, sigma=sig, w_sigma=w), f)
+    with _gpu_op(cfg, sigma=sig, w_sigma=w) as op:
+        Qg = op.collide_pairs(torch.from_numpy(f).cuda()).cpu().numpy()
+    assert _pair_errs(Qg, Qo).max() < TOL
+
+
+def _small_radial_rule(torch_cuda, N, N_rho, M, ns, alpha, noise=0.05):
     torch = torch_cuda
     from oracle.collide import collide_pairs
     masses = (1.0, 2.5, 1.7)[:ns]
@@ -82,7 +120,7 @@ def test_small_radial_rule_every_N(torch_cuda, N, N_rho, M, ns, alpha):
     f = make_points(cfg, range(cfg.nx))
     # make the input rough (exercises the Nyquist planes / complex path)
     rng = np.random.default_rng(N)
-    f *= 1.0 + 0.05 * rng.uniform(-1, 1, f.shape)
+    f *= 1.0 + noise * rng.uniform(-1, 1, f.shape)
     Qo = collide_pairs(_oracle_tables(cfg), f)
     with _gpu_op(cfg) as op:
         Qg = op.collide_pairs(torch.from_numpy(f).cuda()).cpu().numpy()
@@ -178,6 +216,23 @@ def test_batch_is_consistent_with_single_point_calls_and_chunking(torch_cuda, mo
     with _gpu_op(cfg) as op:
         Qc = op.collide_pairs(f)
         assert torch.equal(Qc, Qb)
+
+
+def test_v1_batch_consistency_and_chunking(torch_cuda, monkeypatch):
+    """Same as above for the v1 pipeline (all pairs VHS): chunk of 8 points by default, 3 here, ragged tail."""
+    torch = torch_cuda
+    cfg = _rand_cfg("t", 2, 16, 3, 12, (1.0, 1.0), (0.6, 0.8), (1.0, 2.0), seed=9)
+    f = torch.from_numpy(make_points(cfg, range(11))).cuda()
+    with _gpu_op(cfg) as op:
+        Qb = op.collide_pairs(f).clone()
+        Qs = op.collide(f).clone()
+        for x in (0, 7, 8, 10):
+            Q1 = op.collide_pairs(f[x:x + 1].contiguous())
+            assert torch.equal(Q1[0], Qb[x])
+    monkeypatch.setenv("DGFS_V1_CHUNK", "3")
+    with _gpu_op(cfg) as op:
+        assert torch.equal(op.collide_pairs(f), Qb)
+        assert torch.equal(op.collide(f), Qs)
 
 
 def test_output_on_side_stream_and_repeatability(torch_cuda):
