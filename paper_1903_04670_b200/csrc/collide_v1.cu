@@ -18,10 +18,11 @@
 // Kernels per radial node (all spatial points of a chunk at once):
 //   k_zshift  inverse z pass of h_z f^ for every DISTINCT z shift (the sphere rules share sigma_z values:
 //             18 arrays instead of 96 at c2), on the Hermitian half of the (lx,ly) plane (R-7)
-//   k_nyq     the Nyquist-plane fields: three 2-D transforms and three 1-D sums per (pair, s)
+//   k_nyq1d / k_nyq2   the Nyquist-plane fields: three 1-D sums and three 2-D transforms per (pair, s)
 //   k_xy      per (pair, cz plane): for every s the inverse x,y passes of the packed field in one warp
 //             (lane = pencil, FFTs in registers, one transposition through shared memory), the product
-//             and the sum over s in registers; writes the real plane S_r(., ., cz)
+//             and the sum over s in registers; writes the real plane sum_s Re Z Im Z (., ., cz)
+//   k_wterm   subtracts sum_s Re W Im W
 //   k_zfwd_real / k_plane_fwd<accumulate> (kernels_v0.cuh): fft3(S_r), QG += w_r b_r .
 // Steps 1 and 10 reuse the v0 kernels.
 #include <cmath>
@@ -113,7 +114,8 @@ void free_tables_v1(dgfs_ctx* c) {
 // f^(lx, 0, lz) + i f^(lx, H, lz) for m = 0.  Both packed columns are spectra (in lx, lz) of real
 // fields, so they separate again as Re / Im once the x and z transforms are done.
 template <int N>
-__global__ void __launch_bounds__(256) k_pack_half(const cplx* __restrict__ fhat, cplx* __restrict__ fhh, int narr) {
+__global__ void __launch_bounds__(256) k_pack_half(const cplx* __restrict__ fhat, cplx* __restrict__ fhh,
+                                                   cplx* __restrict__ nyqy, int narr) {
   constexpr int H = N / 2;
   const size_t total = (size_t)narr * N * N * H;
   for (size_t i = blockIdx.x * (size_t)blockDim.x + threadIdx.x; i < total; i += (size_t)gridDim.x * blockDim.x) {
@@ -122,6 +124,15 @@ __global__ void __launch_bounds__(256) k_pack_half(const cplx* __restrict__ fhat
     cplx v = fhat[row * N + m];
     if (m == 0) { cplx w = fhat[row * N + H]; v.x -= w.y; v.y += w.x; }
     fhh[i] = v;
+  }
+  // the ly = H plane, half-packed along lx:  nyqy[arr][lz][m] = f^(m, H, lz), m = 0 carrying f^(H, H, lz)
+  const size_t total2 = (size_t)narr * N * H;
+  for (size_t i = blockIdx.x * (size_t)blockDim.x + threadIdx.x; i < total2; i += (size_t)gridDim.x * blockDim.x) {
+    const int m = (int)(i % H);
+    const size_t pl = i / H;                        // (array, lz)
+    cplx v = fhat[(pl * N + m) * N + H];
+    if (m == 0) { cplx w = fhat[(pl * N + H) * N + H]; v.x -= w.y; v.y += w.x; }
+    nyqy[i] = v;
   }
 }
 
@@ -144,196 +155,384 @@ __global__ void __launch_bounds__(128) k_zshift(V1Tables t, int ns, const cplx* 
   for (int i = 0; i < N; ++i) dst[(size_t)i * NP] = v[i];
 }
 
-// x * (a + i b) for packed side B:  i * x
-__device__ __forceinline__ cplx cmul_i(cplx x) { return make_double2(-x.y, x.x); }
+// 16-byte asynchronous copy global -> shared (LDGSTS): the data of the next plane job lands in shared
+// memory while the warp is still in the FFTs of the current one, without holding registers.
+__device__ __forceinline__ void cp_async16(void* smem, const void* gmem) {
+  const unsigned sa = (unsigned)__cvta_generic_to_shared(smem);
+  asm volatile("cp.async.cg.shared.global [%0], [%1], 16;\n" ::"r"(sa), "l"(gmem));
+}
+__device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;\n" ::); }
+__device__ __forceinline__ void cp_async_wait_all() { asm volatile("cp.async.wait_group 0;\n" ::: "memory"); }
 
-// Nyquist-plane fields of one (item = point x pair, s): block (s, item), 4 warps.
-//   warp 0: uz[cy][cx]  = ifft_xy[ h_x h_y s_z f^(., ., H) ]        warp 1: uxp[cz][cy] = ifft_yz[ s_x h_y h_z f^(H, ., .) ] - (-1)^{cy+cz} s_x s_y s_z f^(H,H,H)
-//   warp 2: uy[cz][cx]  = ifft_xz[ h_x s_y h_z f^(., H, .) ]        warp 3: the 1-D corrections vyh, vxp, vzp
-// every field packed as (side A) + i (side B); each side's field is real.
+// Per-warp shared memory of a plane job: the N x (N+1) tile (input columns, then the transposition) and
+// the job's small tables.
 template <int N>
-__global__ void __launch_bounds__(128) k_nyq(V1Tables t, DevTables tab, const cplx* __restrict__ fhat, cplx* __restrict__ nyq, int r) {
+struct JobSmem {
+  static constexpr int P = N + 1;
+  static constexpr int TILE = N * P;
+  static constexpr int HI = TILE;            // [2][N]  factor along the pass-1 index, per side
+  static constexpr int HM = TILE + 2 * N;    // [2][N]  factor along the pass-2 index, per side
+  static constexpr int VYH = TILE + 4 * N;   // [N]     lane format
+  static constexpr int VXP = TILE + 5 * N;   // [N]
+  static constexpr int VZP = TILE + 6 * N;   // [1]
+  static constexpr int WORDS = TILE + 6 * N + 2;
+};
+
+// 1-D Nyquist corrections of one (item, s) per warp (file header: the s s h, s h s, h s s and s s s terms):
+//   vyh[(side, m)] = s_x s_z f^(H, m, H)                 row lx = H of plane lz = H, lane format, y factor not applied
+//   vxp[cx] = sum_lx e^{2 pi i lx cx / N} h_x s_y s_z f^(lx, H, H)      vzp[cz] = sum_lz e^{..} s_x s_y h_z f^(H, H, lz)
+//   vt = s_x s_y s_z f^(H, H, H)                         all packed (side A) + i (side B)
+template <int N>
+__global__ void __launch_bounds__(128) k_nyq1d(V1Tables t, DevTables tab, const cplx* __restrict__ fhat,
+                                               cplx* __restrict__ nyq, int r, int njobs) {
   constexpr int H = N / 2, N2 = N * N, N3 = N2 * N;
   typedef NyqLayout<N> NL;
-  extern __shared__ cplx sm[];
+  __shared__ cplx sm1[4][3 * N];
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
-  const int s = blockIdx.x, item = blockIdx.y;
+  const int job = blockIdx.x * 4 + warp;
+  if (job >= njobs) return;
+  const int s = job % tab.M, item = job / tab.M;
   const int pair = item % tab.npairs, xl = item / tab.npairs;
   const int p = pair / tab.ns, q = pair % tab.ns;
   const cplx* FA = fhat + ((size_t)xl * tab.ns + p) * N3;
   const cplx* FB = fhat + ((size_t)xl * tab.ns + q) * N3;
   const size_t e = (((size_t)pair * tab.N_rho + r) * tab.M + s) * 2;
-  const cplx *hxA = t.hxy + e * 2 * N, *hyA = hxA + N, *hxB = hxA + 2 * N, *hyB = hxA + 3 * N;
+  const cplx *hxA = t.hxy + e * 2 * N, *hxB = hxA + 2 * N;
   const double sxA = t.sxy[e * 2], syA = t.sxy[e * 2 + 1], sxB = t.sxy[e * 2 + 2], syB = t.sxy[e * 2 + 3];
   const int kA = t.zmap[((size_t)pair * tab.M + s) * 2], kB = t.zmap[((size_t)pair * tab.M + s) * 2 + 1];
   const cplx *hzA = t.hz + ((size_t)r * t.nz + kA) * N, *hzB = t.hz + ((size_t)r * t.nz + kB) * N;
   const double szA = t.szv[(size_t)r * t.nz + kA], szB = t.szv[(size_t)r * t.nz + kB];
   cplx* out = nyq + ((size_t)item * tab.M + s) * NL::STRIDE;
-  cplx* buf = sm + (size_t)warp * (N * (N + 1));
   auto pack = [](cplx fa, cplx ha, double sa, cplx fb, cplx hb, double sb) {
     cplx a = cmul(fa, ha), b = cmul(fb, hb);
     return make_double2(sa * a.x - sb * b.y, sa * a.y + sb * b.x);
   };
-  auto none = [](cplx x, int) { return x; };
-  if (warp == 0) {
-    warp_plane_fft<N, +1>(
-        buf, lane,
-        [&](int lx, int ly) {
-          const size_t i = (size_t)H * N2 + lx * N + ly;
-          return pack(FA[i], cmul(hxA[lx], hyA[ly]), szA, FB[i], cmul(hxB[lx], hyB[ly]), szB);
-        },
-        none, [&](int cy, int cx, cplx val) { out[NL::UZ + cy * N + cx] = val; });
-  } else if (warp == 1) {
-    const double tA = sxA * syA * szA * FA[(size_t)H * N2 + H * N + H].x, tB = sxB * syB * szB * FB[(size_t)H * N2 + H * N + H].x;
-    warp_plane_fft<N, +1>(
-        buf, lane,
-        [&](int lz, int ly) {
-          const size_t i = (size_t)lz * N2 + H * N + ly;
-          return pack(FA[i], cmul(hzA[lz], hyA[ly]), sxA, FB[i], cmul(hzB[lz], hyB[ly]), sxB);
-        },
-        none,
-        [&](int cy, int cz, cplx val) {
-          const double sg = ((cy + cz) & 1) ? -1.0 : 1.0;
-          out[NL::UXP + cz * N + cy] = make_double2(val.x - sg * tA, val.y - sg * tB);
-        });
-  } else if (warp == 2) {
-    warp_plane_fft<N, +1>(
-        buf, lane,
-        [&](int lz, int lx) {
-          const size_t i = (size_t)lz * N2 + lx * N + H;
-          return pack(FA[i], cmul(hzA[lz], hxA[lx]), syA, FB[i], cmul(hzB[lz], hxB[lx]), syB);
-        },
-        none, [&](int cx, int cz, cplx val) { out[NL::UY + cz * N + cx] = val; });
-  } else {
-    cplx* roots = buf;            // e^{2 pi i k / N}
-    cplx* inx = buf + N;
-    cplx* inz = buf + 2 * N;
-    for (int k = lane; k < N; k += 32) {
-      double sn, cs; sincospi(2.0 * k / N, &sn, &cs);
-      roots[k] = make_double2(cs, sn);
-      // vxp: column ly = H of plane lz = H;  vzp: the (H,H) pencil along lz
-      const size_t ix = (size_t)H * N2 + k * N + H, iz = (size_t)k * N2 + H * N + H;
-      inx[k] = pack(FA[ix], hxA[k], syA * szA, FB[ix], hxB[k], syB * szB);
-      inz[k] = pack(FA[iz], hzA[k], sxA * syA, FB[iz], hzB[k], sxB * syB);
-      // vyh: row lx = H of plane lz = H in lane format (side, m), without the y factor
-      const int side = k / H, m = k % H;
-      const cplx* F = side ? FB : FA;
-      const double sc = side ? sxB * szB : sxA * szA;
-      const size_t iy = (size_t)H * N2 + H * N;
-      cplx v = F[iy + m];
-      if (m == 0) v = make_double2(v.x, F[iy + H].x);
-      out[NL::VYH + k] = make_double2(sc * v.x, sc * v.y);
+  cplx* roots = sm1[warp];         // e^{2 pi i k / N}
+  cplx* inx = roots + N;
+  cplx* inz = roots + 2 * N;
+  const size_t iy = (size_t)H * N2 + H * N;
+  for (int k = lane; k < N; k += 32) {
+    double sn, cs; sincospi(2.0 * k / N, &sn, &cs);
+    roots[k] = make_double2(cs, sn);
+    const size_t ix = (size_t)H * N2 + k * N + H, iz = (size_t)k * N2 + H * N + H;
+    inx[k] = pack(FA[ix], hxA[k], syA * szA, FB[ix], hxB[k], syB * szB);
+    inz[k] = pack(FA[iz], hzA[k], sxA * syA, FB[iz], hzB[k], sxB * syB);
+    const int side = k / H, m = k % H;
+    const cplx* F = side ? FB : FA;
+    const double sc = side ? sxB * szB : sxA * szA;
+    cplx v = F[iy + m];
+    if (m == 0) v = make_double2(v.x, F[iy + H].x);
+    out[NL::VYH + k] = make_double2(sc * v.x, sc * v.y);
+  }
+  if (lane == 0) out[NL::VT] = make_double2(sxA * syA * szA * FA[iy + H].x, sxB * syB * szB * FB[iy + H].x);
+  __syncwarp();
+  for (int c = lane; c < N; c += 32) {
+    cplx ax = make_double2(0, 0), az = make_double2(0, 0);
+    for (int l = 0; l < N; ++l) {
+      const cplx w = roots[(l * c) % N];
+      ax = cfma(inx[l], w, ax);
+      az = cfma(inz[l], w, az);
     }
+    out[NL::VXP + c] = ax;
+    out[NL::VZP + c] = az;
+  }
+}
+
+// Pass 1 of a plane job (lane = (side, m), column m of the Hermitian half): multiply by the factor along
+// the pass-1 index, inverse transform in registers, factor of the lane's own column, back into the tile.
+template <int N, bool CORR>
+__device__ __forceinline__ void job_pass1(cplx* buf, int ln, int side, int m, double szs, double scale) {
+  typedef JobSmem<N> JS;
+  constexpr int H = N / 2, P = JS::P;
+  cplx v[N];
+#pragma unroll
+  for (int i = 0; i < N; ++i) v[i] = cmul(buf[i * P + ln], buf[JS::HI + side * N + i]);
+  if (CORR) {
+    const cplx c1 = buf[JS::VYH + ln];
+    v[H].x = fma(-szs, c1.x, v[H].x);
+    v[H].y = fma(-szs, c1.y, v[H].y);
+  }
+  fft_reg<N, +1>(v);
+  // complex h[m] for m >= 1; for the packed lane m = 0 the real h[0], h[H] scale Re (column 0) and
+  // Im (column H) separately
+  const cplx hy0 = buf[JS::HM + side * N + m];
+  const double hyH = buf[JS::HM + side * N + H].x;
+  const double ya = scale * hy0.x, yb = (m == 0) ? 0.0 : -scale * hy0.y, yc = (m == 0) ? 0.0 : scale * hy0.y,
+               yd = (m == 0) ? scale * hyH : scale * hy0.x;
+#pragma unroll
+  for (int i = 0; i < N; ++i)
+    buf[i * P + ln] = make_double2(fma(v[i].x, ya, v[i].y * yb), fma(v[i].x, yc, v[i].y * yd));
+}
+
+// Input of pass 2 (lane = pass-1 output index): the N packed columns X = Y_A + i Y_B, the mirror half by
+// conjugation (Y_A, Y_B are Hermitian along the pass-2 index).
+template <int N, bool CORR>
+__device__ __forceinline__ void job_pass2_in(const cplx* buf, int ln, double szs, double sxb, cplx (&X)[N]) {
+  typedef JobSmem<N> JS;
+  constexpr int H = N / 2, P = JS::P;
+  const cplx* row = buf + ln * P;
+  const cplx a0 = row[0], b0 = row[H];
+  X[0] = make_double2(a0.x, b0.x);
+  X[H] = make_double2(a0.y, b0.y);
+  if (CORR) {
+    const cplx vx = buf[JS::VXP + ln], vz = buf[JS::VZP];
+    X[H].x -= szs * vx.x + sxb * vz.x;
+    X[H].y -= szs * vx.y + sxb * vz.y;
+  }
+#pragma unroll
+  for (int mm = 1; mm < H; ++mm) {
+    const cplx ya = row[mm], yb = row[H + mm];
+    X[mm] = make_double2(ya.x - yb.y, ya.y + yb.x);
+    X[N - mm] = make_double2(ya.x + yb.y, yb.x - ya.y);
+  }
+}
+
+// The three Nyquist-plane fields of every (item, s): block (which, item), warp w runs s = w, w + 4, ...
+//   which 0: uz[cy][cx]  = ifft_xy[ h_x h_y s_z f^(., ., H) ]     pass 1 over lx, pass 2 over ly
+//   which 1: uxp[cz][cy] = ifft_yz[ s_x h_y h_z f^(H, ., .) ] - (-1)^{cy+cz} vt     pass 1 over lz, pass 2 over ly
+//   which 2: uy[cz][cx]  = ifft_xz[ h_x s_y h_z f^(., H, .) ]     pass 1 over lz, pass 2 over lx
+// each a plane job on the Hermitian half (from fhh / nyqy), packed (side A) + i (side B).
+template <int N>
+__global__ void __launch_bounds__(128) k_nyq2(V1Tables t, DevTables tab, const cplx* __restrict__ fhh,
+                                              const cplx* __restrict__ nyqy, cplx* __restrict__ nyq, int r) {
+  constexpr int H = N / 2, NH = N * H;
+  typedef NyqLayout<N> NL;
+  typedef JobSmem<N> JS;
+  constexpr int P = JS::P;
+  extern __shared__ cplx sm[];
+  const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+  const int which = blockIdx.x, item = blockIdx.y;
+  const int pair = item % tab.npairs, xl = item / tab.npairs;
+  const int sp[2] = {pair / tab.ns, pair % tab.ns};
+  cplx* buf = sm + (size_t)warp * JS::WORDS;
+  const bool act = lane < N;
+  const int ln = act ? lane : 0;
+  const int side = ln / H, m = ln % H;
+  // half plane of this lane's side: element (i, m) at src[i * istride + m]
+  const cplx* src;
+  int istride;
+  if (which == 0) { src = fhh + ((size_t)xl * tab.ns + sp[side]) * (size_t)(N * NH) + (size_t)H * NH; istride = H; }
+  else if (which == 1) { src = fhh + ((size_t)xl * tab.ns + sp[side]) * (size_t)(N * NH) + (size_t)H * H; istride = NH; }
+  else { src = nyqy + ((size_t)xl * tab.ns + sp[side]) * (size_t)NH; istride = H; }
+  src += m;
+  const int* zm = t.zmap + (size_t)pair * tab.M * 2;
+  const cplx* hbase = t.hxy + (((size_t)pair * tab.N_rho + r) * tab.M) * 4 * N;
+  const double* sbase = t.sxy + (((size_t)pair * tab.N_rho + r) * tab.M) * 4;
+  auto issue = [&](int s) {
+    if (act) {
+#pragma unroll
+      for (int i = 0; i < N; ++i) cp_async16(&buf[i * P + ln], src + (size_t)i * istride);
+      const cplx* hx = hbase + (size_t)s * 4 * N;            // [side][x|y][N]
+      const cplx* hzA = t.hz + ((size_t)r * t.nz + zm[2 * s]) * N;
+      const cplx* hzB = t.hz + ((size_t)r * t.nz + zm[2 * s + 1]) * N;
+      const cplx *hiA, *hiB, *hmA, *hmB;
+      if (which == 0) { hiA = hx; hiB = hx + 2 * N; hmA = hx + N; hmB = hx + 3 * N; }
+      else if (which == 1) { hiA = hzA; hiB = hzB; hmA = hx + N; hmB = hx + 3 * N; }
+      else { hiA = hzA; hiB = hzB; hmA = hx; hmB = hx + 2 * N; }
+      cp_async16(&buf[JS::HI + ln], hiA + ln);
+      cp_async16(&buf[JS::HI + N + ln], hiB + ln);
+      cp_async16(&buf[JS::HM + ln], hmA + ln);
+      cp_async16(&buf[JS::HM + N + ln], hmB + ln);
+      if (ln == 0) cp_async16(&buf[JS::VZP], nyq + ((size_t)item * tab.M + s) * NL::STRIDE + NL::VT);
+    }
+    cp_async_commit();
+  };
+  auto scale_of = [&](int s) {
+    if (which == 0) return t.szv[(size_t)r * t.nz + zm[2 * s + side]];
+    return sbase[s * 4 + side * 2 + (which == 1 ? 0 : 1)];
+  };
+  if (warp >= tab.M) return;
+  issue(warp);
+  double scale = scale_of(warp);
+  for (int s = warp; s < tab.M; s += 4) {
+    cp_async_wait_all();
     __syncwarp();
-    for (int c = lane; c < N; c += 32) {
-      cplx ax = make_double2(0, 0), az = make_double2(0, 0);
-      for (int l = 0; l < N; ++l) {
-        const cplx w = roots[(l * c) % N];
-        ax = cfma(inx[l], w, ax);
-        az = cfma(inz[l], w, az);
+    cplx X[N];
+    if (act) job_pass1<N, false>(buf, ln, side, m, 0.0, scale);
+    __syncwarp();
+    cplx vt = make_double2(0.0, 0.0);
+    if (act) { job_pass2_in<N, false>(buf, ln, 0.0, 0.0, X); vt = buf[JS::VZP]; }
+    __syncwarp();
+    if (s + 4 < tab.M) { issue(s + 4); scale = scale_of(s + 4); }
+    if (act) {
+      fft_reg<N, +1>(X);
+      cplx* out = nyq + ((size_t)item * tab.M + s) * NL::STRIDE;
+      if (which == 0) {
+#pragma unroll
+        for (int j = 0; j < N; ++j) out[NL::UZ + j * N + ln] = X[j];
+      } else if (which == 1) {
+        const double sb = (ln & 1) ? -1.0 : 1.0;
+#pragma unroll
+        for (int j = 0; j < N; ++j) {
+          const double sg = (j & 1) ? -sb : sb;
+          out[NL::UXP + ln * N + j] = make_double2(X[j].x - sg * vt.x, X[j].y - sg * vt.y);
+        }
+      } else {
+#pragma unroll
+        for (int j = 0; j < N; ++j) out[NL::UY + ln * N + j] = X[j];
       }
-      out[NL::VXP + c] = ax;
-      out[NL::VZP + c] = az;
     }
   }
 }
 
-// The r-loop's main kernel: block (cz, item), W warps; warp w handles s = w, w + W, ...
-//   pass 1 (lane = (side, m), m = Hermitian-half column): v[lx] = Gz_side(lx, m, cz) h_x,side[lx]; inverse x
-//           pass in registers; y factor of the lane's column; transposition through shared memory
-//   pass 2 (lane = cx): rebuild the 32 packed columns X[ly] = Y_A + i Y_B (mirror half by conjugation),
-//           inverse y pass, Z = a_r + i b_r; W from the Nyquist fields; acc[cy] += Re Z Im Z - Re W Im W
-// out: S[item][cz][cy][cx] (real).
+// The r-loop's main kernel: block (cz group, item), warp w owns the plane cz = blockIdx.x * W + w and runs
+// the plane jobs of all s for it, so the sum over s stays in that warp's registers.  Per job:
+//   prefetch (cp.async, issued during the previous job): the two half planes Gz_A(., ., cz), Gz_B(., ., cz)
+//           into the tile, lane = (side, m) owning column m; the x, y factor tables; the Nyquist corrections
+//   pass 1: v[lx] = tile[lx][lane] h_x,side[lx]; inverse x pass in registers; y factor of the lane's column;
+//           back into the tile (transposition)
+//   pass 2: lane = cx rebuilds the N packed columns X[ly] = Y_A + i Y_B (mirror half by conjugation), inverse
+//           y pass: Z = a_r + i b_r;  acc[cy] += Re Z Im Z
+// out: S[item][cz][cy][cx] = sum_s Re Z Im Z (the Nyquist-field product is subtracted by k_zfwd_planes).
 template <int N, int W>
 __global__ void __launch_bounds__(32 * W) k_xy(V1Tables t, DevTables tab, const cplx* __restrict__ Gz,
                                                const cplx* __restrict__ nyq, double* __restrict__ S, int r) {
-  constexpr int H = N / 2, P = N + 1, NH = N * H, N2 = N * N;
+  constexpr int H = N / 2, NH = N * H, N2 = N * N;
   typedef NyqLayout<N> NL;
+  typedef JobSmem<N> JS;
+  constexpr int P = JS::P;
   static_assert(N <= 32, "one lane per pencil");
   extern __shared__ cplx sm[];
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
-  const int cz = blockIdx.x, item = blockIdx.y;
+  const int cz = blockIdx.x * W + warp, item = blockIdx.y;
+  if (cz >= N) return;
   const int pair = item % tab.npairs, xl = item / tab.npairs;
-  cplx* buf = sm + (size_t)warp * (N * P);
+  cplx* buf = sm + (size_t)warp * JS::WORDS;
   const bool act = lane < N;
   const int ln = act ? lane : 0;
   const int side = ln / H, m = ln % H;
   const double szs = (cz & 1) ? -1.0 : 1.0;
   const double sxb = (ln & 1) ? -1.0 : 1.0;
+  const int* zm = t.zmap + (size_t)pair * tab.M * 2;
+  const cplx* gbase = Gz + (size_t)xl * t.nz * (size_t)(N * NH) + (size_t)cz * NH + m;
+  const cplx* hbase = t.hxy + (((size_t)pair * tab.N_rho + r) * tab.M) * 4 * N;
+  const cplx* nbase = nyq + (size_t)item * tab.M * NL::STRIDE;
+  auto issue = [&](int s) {
+    if (act) {
+      const cplx* g = gbase + (size_t)zm[2 * s + side] * (size_t)(N * NH);
+#pragma unroll
+      for (int i = 0; i < N; ++i) cp_async16(&buf[i * P + ln], g + i * H);
+      const cplx* hx = hbase + (size_t)s * 4 * N;          // [side][x|y][N]
+      cp_async16(&buf[JS::HI + ln], hx + ln);               // h_x side A
+      cp_async16(&buf[JS::HI + N + ln], hx + 2 * N + ln);   // h_x side B
+      cp_async16(&buf[JS::HM + ln], hx + N + ln);           // h_y side A
+      cp_async16(&buf[JS::HM + N + ln], hx + 3 * N + ln);   // h_y side B
+      const cplx* nq = nbase + (size_t)s * NL::STRIDE;
+      cp_async16(&buf[JS::VYH + ln], nq + NL::VYH + ln);
+      cp_async16(&buf[JS::VXP + ln], nq + NL::VXP + ln);
+      if (ln == 0) cp_async16(&buf[JS::VZP], nq + NL::VZP + cz);
+    }
+    cp_async_commit();
+  };
   double acc[N];
 #pragma unroll
   for (int j = 0; j < N; ++j) acc[j] = 0.0;
-  for (int s = warp; s < tab.M; s += W) {
-    const int k = t.zmap[((size_t)pair * tab.M + s) * 2 + side];
-    const cplx* g = Gz + ((size_t)xl * t.nz + k) * (size_t)(N * NH) + (size_t)cz * NH + m;
-    const cplx* hx = t.hxy + ((((size_t)pair * tab.N_rho + r) * tab.M + s) * 2 + side) * 2 * N;
-    const cplx* nq = nyq + ((size_t)item * tab.M + s) * NL::STRIDE;
-    if (act) {
-      cplx v[N];
-#pragma unroll
-      for (int i = 0; i < N; ++i) v[i] = cmul(g[i * H], __ldg(&hx[i]));
-      {
-        const cplx c1 = nq[NL::VYH + ln];
-        v[H].x = fma(-szs, c1.x, v[H].x);
-        v[H].y = fma(-szs, c1.y, v[H].y);
-      }
-      fft_reg<N, +1>(v);
-      // y factor: complex h_y[m] for m >= 1; for the packed lane m = 0 the real parts of h_y[0], h_y[H]
-      // scale Re (column 0) and Im (column H) separately
-      const cplx hy0 = __ldg(&hx[N + m]);
-      const double hyH = __ldg(&hx[N + H]).x;
-      const double ya = hy0.x, yb = (m == 0) ? 0.0 : -hy0.y, yc = (m == 0) ? 0.0 : hy0.y, yd = (m == 0) ? hyH : hy0.x;
-#pragma unroll
-      for (int i = 0; i < N; ++i)
-        buf[i * P + ln] = make_double2(fma(v[i].x, ya, v[i].y * yb), fma(v[i].x, yc, v[i].y * yd));
-    }
+  issue(0);
+  for (int s = 0; s < tab.M; ++s) {
+    cp_async_wait_all();
     __syncwarp();
+    cplx X[N];
+    if (act) job_pass1<N, true>(buf, ln, side, m, szs, 1.0);
+    __syncwarp();
+    if (act) job_pass2_in<N, true>(buf, ln, szs, sxb, X);
+    __syncwarp();
+    if (s + 1 < tab.M) issue(s + 1);         // the tile is free: the next job's data arrives during pass 2
     if (act) {
-      const cplx* row = buf + ln * P;
-      cplx X[N];
-      {
-        const cplx a0 = row[0], b0 = row[H];
-        const cplx vx = nq[NL::VXP + ln], vz = nq[NL::VZP + cz];
-        X[0] = make_double2(a0.x, b0.x);
-        X[H] = make_double2(a0.y - szs * vx.x - sxb * vz.x, b0.y - szs * vx.y - sxb * vz.y);
-      }
-#pragma unroll
-      for (int mm = 1; mm < H; ++mm) {
-        const cplx ya = row[mm], yb = row[H + mm];
-        X[mm] = make_double2(ya.x - yb.y, ya.y + yb.x);
-        X[N - mm] = make_double2(ya.x + yb.y, yb.x - ya.y);
-      }
       fft_reg<N, +1>(X);
-      const cplx uyv = nq[NL::UY + cz * N + ln];
-      const cplx* uxp = nq + NL::UXP + cz * N;
-      const cplx* uz = nq + NL::UZ + ln;
 #pragma unroll
-      for (int j = 0; j < N; ++j) {
-        const cplx ux = __ldg(&uxp[j]);
-        const cplx uzv = uz[j * N];
-        const double syj = (j & 1) ? -1.0 : 1.0;
-        const double wx = fma(sxb, ux.x, fma(szs, uzv.x, syj * uyv.x));
-        const double wy = fma(sxb, ux.y, fma(szs, uzv.y, syj * uyv.y));
-        acc[j] = fma(X[j].x, X[j].y, fma(-wx, wy, acc[j]));
+      for (int j = 0; j < N; ++j) acc[j] = fma(X[j].x, X[j].y, acc[j]);
+    }
+  }
+  if (act) {
+    double* o = S + ((size_t)item * N + cz) * N2 + ln;
+#pragma unroll
+    for (int j = 0; j < N; ++j) o[j * N] = acc[j];
+  }
+}
+
+// S_r(c) -= sum_s Re W_s(c) Im W_s(c),  W_s(c) = (-1)^cx ux'_s(cy,cz) + (-1)^cy uy_s(cx,cz) + (-1)^cz uz_s(cx,cy)
+// (W = a_i + i b_i, file header).  Block (cz group of 8 planes, item), thread = 2 x 2 tile of (cx, cy), so
+// every table element serves several nodes and all signs are compile-time constants.  The tables of one s
+// (uz plane, 8 rows of ux' and uy) are staged in shared memory by cp.async, double buffered over s; uz and
+// uy are stored de-interleaved by the parity of cx so that the pair loads are conflict-free.
+template <int N>
+struct WtermSmem {
+  static constexpr int CZG = 8;
+  static constexpr int Z = 0;                       // [cy][parity][H]
+  static constexpr int V = N * N;                   // [i][parity][H]
+  static constexpr int U = N * N + CZG * N;         // [i][cy]
+  static constexpr int WORDS = N * N + 2 * CZG * N;
+};
+template <int N>
+__global__ void __launch_bounds__(256, 2) k_wterm(const cplx* __restrict__ nyq, int M, double* __restrict__ S) {
+  constexpr int H = N / 2, N2 = N * N, N3 = N2 * N;
+  typedef NyqLayout<N> NL;
+  typedef WtermSmem<N> WS;
+  constexpr int CZG = WS::CZG;
+  extern __shared__ cplx sm[];
+  const int tx = threadIdx.x % 16, ty = threadIdx.x / 16;
+  const bool act = tx < H && ty < H;
+  const int cz0 = blockIdx.x * CZG;
+  const cplx* nbase = nyq + (size_t)blockIdx.y * M * NL::STRIDE;
+  auto issue = [&](int s) {
+    cplx* dst = sm + (size_t)(s & 1) * WS::WORDS;
+    const cplx* nq = nbase + (size_t)s * NL::STRIDE;
+    for (int e = threadIdx.x; e < WS::WORDS; e += 256) {
+      if (e < N2) {
+        const int cy = e / N, cx = e % N;
+        cp_async16(&dst[WS::Z + (cy * 2 + (cx & 1)) * H + (cx >> 1)], nq + NL::UZ + e);
+      } else if (e < N2 + CZG * N) {
+        const int i = (e - N2) / N, cx = (e - N2) % N;
+        cp_async16(&dst[WS::V + (i * 2 + (cx & 1)) * H + (cx >> 1)], nq + NL::UY + (cz0 + i) * N + cx);
+      } else {
+        const int i = (e - N2 - CZG * N) / N, cy = (e - N2 - CZG * N) % N;
+        cp_async16(&dst[WS::U + i * N + cy], nq + NL::UXP + (cz0 + i) * N + cy);
       }
     }
-    __syncwarp();
-  }
-  // sum the W partial planes through shared memory and write S(., ., cz)
-  __syncthreads();
-  double* red = reinterpret_cast<double*>(sm);            // [W][N][N] doubles <= W * N * P cplx
-  if (act) {
+    cp_async_commit();
+  };
+  double acc[CZG][2][2];                      // [cz][cy][cx]
 #pragma unroll
-    for (int j = 0; j < N; ++j) red[(warp * N + j) * N + ln] = acc[j];
-  }
-  __syncthreads();
-  double* o = S + ((size_t)item * N + cz) * N2;
-  for (int e2 = threadIdx.x; e2 < N2; e2 += 32 * W) {
-    double sum = 0.0;
+  for (int i = 0; i < CZG; ++i) acc[i][0][0] = acc[i][0][1] = acc[i][1][0] = acc[i][1][1] = 0.0;
+  issue(0);
+  for (int s = 0; s < M; ++s) {
+    cp_async_wait_all();
+    __syncthreads();
+    if (s + 1 < M) issue(s + 1);
+    if (!act) continue;
+    const cplx* b_ = sm + (size_t)(s & 1) * WS::WORDS;
+    cplx z[2][2];
 #pragma unroll
-    for (int w = 0; w < W; ++w) sum += red[w * N2 + e2];
-    o[e2] = sum;
+    for (int b = 0; b < 2; ++b)
+#pragma unroll
+      for (int a = 0; a < 2; ++a) z[b][a] = b_[WS::Z + ((2 * ty + b) * 2 + a) * H + tx];
+#pragma unroll
+    for (int i = 0; i < CZG; ++i) {
+      const cplx u[2] = {b_[WS::U + i * N + 2 * ty], b_[WS::U + i * N + 2 * ty + 1]};
+      const cplx v[2] = {b_[WS::V + (i * 2) * H + tx], b_[WS::V + (i * 2 + 1) * H + tx]};
+#pragma unroll
+      for (int b = 0; b < 2; ++b)
+#pragma unroll
+        for (int a = 0; a < 2; ++a) {
+          // signs: the tile starts at even cx, cy, cz
+          const double ux_ = a ? -u[b].x : u[b].x, uy_ = a ? -u[b].y : u[b].y;
+          const double vx_ = b ? -v[a].x : v[a].x, vy_ = b ? -v[a].y : v[a].y;
+          const double zx_ = (i & 1) ? -z[b][a].x : z[b][a].x, zy_ = (i & 1) ? -z[b][a].y : z[b][a].y;
+          acc[i][b][a] = fma(ux_ + vx_ + zx_, uy_ + vy_ + zy_, acc[i][b][a]);
+        }
+    }
   }
+  if (!act) return;
+  double* o = S + (size_t)blockIdx.y * N3 + (size_t)cz0 * N2 + (2 * ty) * N + 2 * tx;
+#pragma unroll
+  for (int i = 0; i < CZG; ++i)
+#pragma unroll
+    for (int b = 0; b < 2; ++b) {
+      double2* q = reinterpret_cast<double2*>(o + (size_t)i * N2 + b * N);
+      double2 t = *q;
+      t.x -= acc[i][b][0]; t.y -= acc[i][b][1];
+      *q = t;
+    }
 }
 
 // forward z pass of the real field S[item][cz][cy][cx] (thread per (cy,cx) pencil) -> T[item][kz][cy][cx]
@@ -356,7 +555,7 @@ __global__ void __launch_bounds__(128) k_zfwd_planes(const double* __restrict__ 
 namespace {
 struct PlanV1 {
   int nbx;
-  size_t off_fhat, off_fhh, off_qg, off_gz, off_nyq, off_s, off_t, total;
+  size_t off_fhat, off_fhh, off_nyqy, off_qg, off_gz, off_nyq, off_s, off_t, total;
 };
 PlanV1 plan_v1(const dgfs_ctx* c, int nx) {
   PlanV1 pl{};
@@ -373,6 +572,7 @@ PlanV1 plan_v1(const dgfs_ctx* c, int nx) {
   auto take = [&](size_t bytes) { size_t o = off; off += (bytes + 255) & ~(size_t)255; return o; };
   pl.off_fhat = take((size_t)nbx * c->ns * arr);
   pl.off_fhh = take((size_t)nbx * c->ns * (arr / 2));
+  pl.off_nyqy = take((size_t)nbx * c->ns * (N * N / 2) * sizeof(cplx));
   pl.off_qg = take(items * arr);
   pl.off_gz = take(gz > g2 ? gz : g2);
   pl.off_nyq = take(items * c->M * nyq_stride * sizeof(cplx));
@@ -388,17 +588,18 @@ size_t workspace_bytes_v1(const dgfs_ctx* c, int nx) { return plan_v1(c, nx).tot
 // algorithmic FLOPs of the executed algorithm: a 1-D transform of length N counts
 // 5 N log2 N, pointwise work counts the real operations of the formulas in this file's header.
 namespace {
-struct FlopsV1 { double zshift, nyq, xy, zfwd, acc, per_r, tail; };
+struct FlopsV1 { double zshift, nyq, xy, wterm, zfwd, acc, per_r, tail; };
 FlopsV1 flops_v1(const dgfs_ctx* c) {
   const double N = c->N, N2 = N * N, N3 = N2 * N, H = N / 2, M = c->M;
   const double fft1 = 5.0 * N * log2(N), fft3 = 3.0 * N2 * fft1;
   FlopsV1 f{};
   f.zshift = (double)c->v1_nz / c->npairs * N * H * (fft1 + 6.0 * N);   // per item
-  f.nyq = M * (3.0 * (2.0 * N * fft1 + 28.0 * N2) + 16.0 * N2);
-  f.xy = M * N * (2.0 * N * fft1 + 28.0 * N2);
+  f.nyq = M * (3.0 * (2.0 * N * fft1 + 14.0 * N2) + 16.0 * N2);   // three plane jobs + the 1-D sums
+  f.xy = M * N * (2.0 * N * fft1 + 18.0 * N2);    // x, y factors 6 + 6, packing 2, corrections ~2, product 2
+  f.wterm = M * N3 * 6.0 + N3;                      // 4 adds + 1 fma per (node, s)
   f.zfwd = N2 * fft1;
   f.acc = 2.0 * N2 * fft1 + 4.0 * N3;
-  f.per_r = f.zshift + f.nyq + f.xy + f.zfwd + f.acc;
+  f.per_r = f.zshift + f.nyq + f.xy + f.wterm + f.zfwd + f.acc;
   f.tail = 2.0 * fft3 + 11.0 * N3 + fft3 / c->ns;
   return f;
 }
@@ -419,6 +620,7 @@ static int collide_v1_impl(dgfs_ctx* c, const double* f, double* out, int nx, bo
   char* ws = (char*)c->ws;
   cplx* fhat = (cplx*)(ws + pl.off_fhat);
   cplx* fhh = (cplx*)(ws + pl.off_fhh);
+  cplx* nyqy = (cplx*)(ws + pl.off_nyqy);
   cplx* QG = (cplx*)(ws + pl.off_qg);
   cplx* Gz = (cplx*)(ws + pl.off_gz);
   cplx* nyq = (cplx*)(ws + pl.off_nyq);
@@ -427,15 +629,17 @@ static int collide_v1_impl(dgfs_ctx* c, const double* f, double* out, int nx, bo
   const int ns = c->ns, np = c->npairs, nz = c->v1_nz;
   const size_t smem_plane = plane_smem_per_warp<N>() * W;
   const size_t smem_final = plane_smem_per_warp<N>() * 2;
-  const size_t smem_xy = sizeof(cplx) * (size_t)W * N * (N + 1);
-  const size_t smem_nyq = sizeof(cplx) * (size_t)4 * N * (N + 1);
+  const size_t smem_xy = sizeof(cplx) * (size_t)W * JobSmem<N>::WORDS;
+  const size_t smem_wt = sizeof(cplx) * (size_t)2 * WtermSmem<N>::WORDS;
+  const size_t smem_nyq = sizeof(cplx) * (size_t)4 * JobSmem<N>::WORDS;
   static bool attr_done = false;
   if (!attr_done) {
     cudaFuncSetAttribute(k_plane_fwd<N, W, 0>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_plane);
     cudaFuncSetAttribute(k_plane_fwd<N, W, 1>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_plane);
     cudaFuncSetAttribute(k_final_xy<N>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_final);
     cudaFuncSetAttribute(k_xy<N, W>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_xy);
-    cudaFuncSetAttribute(k_nyq<N>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_nyq);
+    cudaFuncSetAttribute(k_wterm<N>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_wt);
+    cudaFuncSetAttribute(k_nyq2<N>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_nyq);
     attr_done = true;
   }
   const int pen_blocks = (N2 + 127) / 128;
@@ -453,15 +657,19 @@ static int collide_v1_impl(dgfs_ctx* c, const double* f, double* out, int nx, bo
     { ProfScope ps(c->prof, st, "k_plane_fwd<store>", nb * ns * fft3 * 2.0 / 3.0);
       k_plane_fwd<N, W, 0><<<dim3(plane_blocks, nb * ns), 32 * W, smem_plane, st>>>(c->tab, T, 1, fhat, 0); }
     { ProfScope ps(c->prof, st, "k_pack_half", 0.0);
-      k_pack_half<N><<<(nb * ns * N2 * H + 255) / 256, 256, 0, st>>>(fhat, fhh, nb * ns); }
+      k_pack_half<N><<<(nb * ns * N2 * H + 255) / 256, 256, 0, st>>>(fhat, fhh, nyqy, nb * ns); }
     cudaMemsetAsync(QG, 0, (size_t)items * N3 * sizeof(cplx), st);
     for (int r = 0; r < c->N_rho; ++r) {
       { ProfScope ps(c->prof, st, "k_zshift", items * fl.zshift);
         k_zshift<N><<<dim3(hpen_blocks, nz, nb), 128, 0, st>>>(c->v1, ns, fhh, Gz, r); }
-      { ProfScope ps(c->prof, st, "k_nyq", items * fl.nyq);
-        k_nyq<N><<<dim3(c->M, items), 128, smem_nyq, st>>>(c->v1, c->tab, fhat, nyq, r); }
+      { ProfScope ps(c->prof, st, "k_nyq1d", items * c->M * 16.0 * N2);
+        k_nyq1d<N><<<(items * c->M + 3) / 4, 128, 0, st>>>(c->v1, c->tab, fhat, nyq, r, items * c->M); }
+      { ProfScope ps(c->prof, st, "k_nyq2", items * (fl.nyq - c->M * 16.0 * N2));
+        k_nyq2<N><<<dim3(3, items), 128, smem_nyq, st>>>(c->v1, c->tab, fhh, nyqy, nyq, r); }
       { ProfScope ps(c->prof, st, "k_xy", items * fl.xy);
-        k_xy<N, W><<<dim3(N, items), 32 * W, smem_xy, st>>>(c->v1, c->tab, Gz, nyq, S, r); }
+        k_xy<N, W><<<dim3((N + W - 1) / W, items), 32 * W, smem_xy, st>>>(c->v1, c->tab, Gz, nyq, S, r); }
+      { ProfScope ps(c->prof, st, "k_wterm", items * fl.wterm);
+        k_wterm<N><<<dim3(N / 8, items), 256, smem_wt, st>>>(nyq, c->M, S); }
       { ProfScope ps(c->prof, st, "k_zfwd_planes", items * fl.zfwd);
         k_zfwd_planes<N><<<dim3(pen_blocks, items), 128, 0, st>>>(S, T); }
       { ProfScope ps(c->prof, st, "k_plane_fwd<accumulate>", items * fl.acc);
