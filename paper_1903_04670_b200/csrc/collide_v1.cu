@@ -19,11 +19,11 @@
 //   k_zshift  inverse z pass of h_z f^ for every DISTINCT z shift (the sphere rules share sigma_z values:
 //             18 arrays instead of 96 at c2), on the Hermitian half of the (lx,ly) plane (R-7)
 //   k_nyq1d / k_nyq2   the Nyquist-plane fields: three 1-D sums and three 2-D transforms per (pair, s)
+//   k_wterm   -sum_s Re W Im W
 //   k_xy      per (pair, cz plane): for every s the inverse x,y passes of the packed field in one warp
 //             (lane = pencil, FFTs in registers, one transposition through shared memory), the product
-//             and the sum over s in registers; writes the real plane sum_s Re Z Im Z (., ., cz)
-//   k_wterm   subtracts sum_s Re W Im W
-//   k_zfwd_real / k_plane_fwd<accumulate> (kernels_v0.cuh): fft3(S_r), QG += w_r b_r .
+//             and the sum over s in registers, then the forward x,y passes of the real plane S_r(., ., cz)
+//   k_zfwd_acc  forward z pass, QG += w_r b_r .
 // Steps 1 and 10 reuse the v0 kernels.
 #include <cmath>
 #include <cstdio>
@@ -163,6 +163,7 @@ __device__ __forceinline__ void cp_async16(void* smem, const void* gmem) {
 }
 __device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;\n" ::); }
 __device__ __forceinline__ void cp_async_wait_all() { asm volatile("cp.async.wait_group 0;\n" ::: "memory"); }
+__device__ __forceinline__ void cp_async_wait_one() { asm volatile("cp.async.wait_group 1;\n" ::: "memory"); }
 
 // Per-warp shared memory of a plane job: the N x (N+1) tile (input columns, then the transposition) and
 // the job's small tables.
@@ -287,13 +288,13 @@ __device__ __forceinline__ void job_pass2_in(const cplx* buf, int ln, double szs
   }
 }
 
-// The three Nyquist-plane fields of every (item, s): block (which, item), warp w runs s = w, w + 4, ...
+// The three Nyquist-plane fields of every (item, s): block (which, item), warp w of NW runs s = w, w + NW, ...
 //   which 0: uz[cy][cx]  = ifft_xy[ h_x h_y s_z f^(., ., H) ]     pass 1 over lx, pass 2 over ly
-//   which 1: uxp[cz][cy] = ifft_yz[ s_x h_y h_z f^(H, ., .) ] - (-1)^{cy+cz} vt     pass 1 over lz, pass 2 over ly
-//   which 2: uy[cz][cx]  = ifft_xz[ h_x s_y h_z f^(., H, .) ]     pass 1 over lz, pass 2 over lx
+//   which 1: uxp[cy][cz] = ifft_yz[ s_x h_y h_z f^(H, ., .) ] - (-1)^{cy+cz} vt     pass 1 over lz, pass 2 over ly
+//   which 2: uy[cx][cz]  = ifft_xz[ h_x s_y h_z f^(., H, .) ]     pass 1 over lz, pass 2 over lx
 // each a plane job on the Hermitian half (from fhh / nyqy), packed (side A) + i (side B).
-template <int N>
-__global__ void __launch_bounds__(128) k_nyq2(V1Tables t, DevTables tab, const cplx* __restrict__ fhh,
+template <int N, int NW>
+__global__ void __launch_bounds__(32 * NW) k_nyq2(V1Tables t, DevTables tab, const cplx* __restrict__ fhh,
                                               const cplx* __restrict__ nyqy, cplx* __restrict__ nyq, int r) {
   constexpr int H = N / 2, NH = N * H;
   typedef NyqLayout<N> NL;
@@ -344,7 +345,7 @@ __global__ void __launch_bounds__(128) k_nyq2(V1Tables t, DevTables tab, const c
   if (warp >= tab.M) return;
   issue(warp);
   double scale = scale_of(warp);
-  for (int s = warp; s < tab.M; s += 4) {
+  for (int s = warp; s < tab.M; s += NW) {
     cp_async_wait_all();
     __syncwarp();
     cplx X[N];
@@ -353,7 +354,7 @@ __global__ void __launch_bounds__(128) k_nyq2(V1Tables t, DevTables tab, const c
     cplx vt = make_double2(0.0, 0.0);
     if (act) { job_pass2_in<N, false>(buf, ln, 0.0, 0.0, X); vt = buf[JS::VZP]; }
     __syncwarp();
-    if (s + 4 < tab.M) { issue(s + 4); scale = scale_of(s + 4); }
+    if (s + NW < tab.M) { issue(s + NW); scale = scale_of(s + NW); }
     if (act) {
       fft_reg<N, +1>(X);
       cplx* out = nyq + ((size_t)item * tab.M + s) * NL::STRIDE;
@@ -365,11 +366,11 @@ __global__ void __launch_bounds__(128) k_nyq2(V1Tables t, DevTables tab, const c
 #pragma unroll
         for (int j = 0; j < N; ++j) {
           const double sg = (j & 1) ? -sb : sb;
-          out[NL::UXP + ln * N + j] = make_double2(X[j].x - sg * vt.x, X[j].y - sg * vt.y);
+          out[NL::UXP + j * N + ln] = make_double2(X[j].x - sg * vt.x, X[j].y - sg * vt.y);
         }
       } else {
 #pragma unroll
-        for (int j = 0; j < N; ++j) out[NL::UY + ln * N + j] = X[j];
+        for (int j = 0; j < N; ++j) out[NL::UY + j * N + ln] = X[j];
       }
     }
   }
@@ -383,10 +384,11 @@ __global__ void __launch_bounds__(128) k_nyq2(V1Tables t, DevTables tab, const c
 //           back into the tile (transposition)
 //   pass 2: lane = cx rebuilds the N packed columns X[ly] = Y_A + i Y_B (mirror half by conjugation), inverse
 //           y pass: Z = a_r + i b_r;  acc[cy] += Re Z Im Z
-// out: S[item][cz][cy][cx] = sum_s Re Z Im Z (the Nyquist-field product is subtracted by k_zfwd_planes).
+// in: S[item][cz][cy][cx] = -sum_s Re W Im W (k_wterm);  out: T[item][cz][kx][ky] = fft_xy of S_r(., ., cz).
 template <int N, int W>
 __global__ void __launch_bounds__(32 * W) k_xy(V1Tables t, DevTables tab, const cplx* __restrict__ Gz,
-                                               const cplx* __restrict__ nyq, double* __restrict__ S, int r) {
+                                               const cplx* __restrict__ nyq, const double* __restrict__ S,
+                                               cplx* __restrict__ T, int r) {
   constexpr int H = N / 2, NH = N * H, N2 = N * N;
   typedef NyqLayout<N> NL;
   typedef JobSmem<N> JS;
@@ -424,10 +426,14 @@ __global__ void __launch_bounds__(32 * W) k_xy(V1Tables t, DevTables tab, const 
     }
     cp_async_commit();
   };
-  double acc[N];
-#pragma unroll
-  for (int j = 0; j < N; ++j) acc[j] = 0.0;
   issue(0);
+  // start from the Nyquist-field product written by k_wterm
+  double acc[N];
+  {
+    const double* w0 = S + ((size_t)item * N + cz) * N2 + ln;
+#pragma unroll
+    for (int j = 0; j < N; ++j) acc[j] = w0[j * N];
+  }
   for (int s = 0; s < tab.M; ++s) {
     cp_async_wait_all();
     __syncwarp();
@@ -443,17 +449,31 @@ __global__ void __launch_bounds__(32 * W) k_xy(V1Tables t, DevTables tab, const 
       for (int j = 0; j < N; ++j) acc[j] = fma(X[j].x, X[j].y, acc[j]);
     }
   }
+  // forward y and x passes of the real plane S_r(., ., cz) (steps 6-7, after R-1)
   if (act) {
-    double* o = S + ((size_t)item * N + cz) * N2 + ln;
+    cplx v[N];
 #pragma unroll
-    for (int j = 0; j < N; ++j) o[j * N] = acc[j];
+    for (int j = 0; j < N; ++j) v[j] = make_double2(acc[j], 0.0);
+    fft_reg<N, -1>(v);
+#pragma unroll
+    for (int j = 0; j < N; ++j) buf[j * P + ln] = v[j];          // [ky][cx]
+  }
+  __syncwarp();
+  if (act) {
+    cplx v[N];
+#pragma unroll
+    for (int i = 0; i < N; ++i) v[i] = buf[ln * P + i];          // lane = ky
+    fft_reg<N, -1>(v);
+    cplx* o = T + ((size_t)item * N + cz) * N2 + ln;
+#pragma unroll
+    for (int k = 0; k < N; ++k) o[k * N] = v[k];                 // [cz][kx][ky]
   }
 }
 
-// S_r(c) -= sum_s Re W_s(c) Im W_s(c),  W_s(c) = (-1)^cx ux'_s(cy,cz) + (-1)^cy uy_s(cx,cz) + (-1)^cz uz_s(cx,cy)
+// S(c) = -sum_s Re W_s(c) Im W_s(c),  W_s(c) = (-1)^cx ux'_s(cy,cz) + (-1)^cy uy_s(cx,cz) + (-1)^cz uz_s(cx,cy)
 // (W = a_i + i b_i, file header).  Block (cz group of 8 planes, item), thread = 2 x 2 tile of (cx, cy), so
 // every table element serves several nodes and all signs are compile-time constants.  The tables of one s
-// (uz plane, 8 rows of ux' and uy) are staged in shared memory by cp.async, double buffered over s; uz and
+// (uz plane, 8 rows of ux' and uy) are staged in shared memory by cp.async, three stages over s; uz and
 // uy are stored de-interleaved by the parity of cx so that the pair loads are conflict-free.
 template <int N>
 struct WtermSmem {
@@ -475,18 +495,18 @@ __global__ void __launch_bounds__(256, 2) k_wterm(const cplx* __restrict__ nyq, 
   const int cz0 = blockIdx.x * CZG;
   const cplx* nbase = nyq + (size_t)blockIdx.y * M * NL::STRIDE;
   auto issue = [&](int s) {
-    cplx* dst = sm + (size_t)(s & 1) * WS::WORDS;
+    cplx* dst = sm + (size_t)(s % 3) * WS::WORDS;
     const cplx* nq = nbase + (size_t)s * NL::STRIDE;
     for (int e = threadIdx.x; e < WS::WORDS; e += 256) {
       if (e < N2) {
         const int cy = e / N, cx = e % N;
         cp_async16(&dst[WS::Z + (cy * 2 + (cx & 1)) * H + (cx >> 1)], nq + NL::UZ + e);
       } else if (e < N2 + CZG * N) {
-        const int i = (e - N2) / N, cx = (e - N2) % N;
-        cp_async16(&dst[WS::V + (i * 2 + (cx & 1)) * H + (cx >> 1)], nq + NL::UY + (cz0 + i) * N + cx);
+        const int cx = (e - N2) / CZG, i = (e - N2) % CZG;
+        cp_async16(&dst[WS::V + (i * 2 + (cx & 1)) * H + (cx >> 1)], nq + NL::UY + cx * N + cz0 + i);
       } else {
-        const int i = (e - N2 - CZG * N) / N, cy = (e - N2 - CZG * N) % N;
-        cp_async16(&dst[WS::U + i * N + cy], nq + NL::UXP + (cz0 + i) * N + cy);
+        const int cy = (e - N2 - CZG * N) / CZG, i = (e - N2 - CZG * N) % CZG;
+        cp_async16(&dst[WS::U + i * N + cy], nq + NL::UXP + cy * N + cz0 + i);
       }
     }
     cp_async_commit();
@@ -495,12 +515,13 @@ __global__ void __launch_bounds__(256, 2) k_wterm(const cplx* __restrict__ nyq, 
 #pragma unroll
   for (int i = 0; i < CZG; ++i) acc[i][0][0] = acc[i][0][1] = acc[i][1][0] = acc[i][1][1] = 0.0;
   issue(0);
+  if (M > 1) issue(1);
   for (int s = 0; s < M; ++s) {
-    cp_async_wait_all();
+    if (s + 1 < M) cp_async_wait_one(); else cp_async_wait_all();
     __syncthreads();
-    if (s + 1 < M) issue(s + 1);
+    if (s + 2 < M) issue(s + 2);
     if (!act) continue;
-    const cplx* b_ = sm + (size_t)(s & 1) * WS::WORDS;
+    const cplx* b_ = sm + (size_t)(s % 3) * WS::WORDS;
     cplx z[2][2];
 #pragma unroll
     for (int b = 0; b < 2; ++b)
@@ -528,27 +549,37 @@ __global__ void __launch_bounds__(256, 2) k_wterm(const cplx* __restrict__ nyq, 
   for (int i = 0; i < CZG; ++i)
 #pragma unroll
     for (int b = 0; b < 2; ++b) {
-      double2* q = reinterpret_cast<double2*>(o + (size_t)i * N2 + b * N);
-      double2 t = *q;
-      t.x -= acc[i][b][0]; t.y -= acc[i][b][1];
-      *q = t;
+      *reinterpret_cast<double2*>(o + (size_t)i * N2 + b * N) = make_double2(-acc[i][b][0], -acc[i][b][1]);
     }
 }
 
-// forward z pass of the real field S[item][cz][cy][cx] (thread per (cy,cx) pencil) -> T[item][kz][cy][cx]
-template <int N>
-__global__ void __launch_bounds__(128) k_zfwd_planes(const double* __restrict__ S, cplx* __restrict__ T) {
+// Forward z pass and steps 7-8: thread per (kx,ky) pencil of T[item][cz][kx][ky];
+// QG[item][kz][kx][ky] (+)= w_r b_r(|k|^2) t3.  FIRST: the first radial node stores instead of accumulating.
+template <int N, bool FIRST>
+__global__ void __launch_bounds__(128) k_zfwd_acc(DevTables tab, const cplx* __restrict__ T, cplx* __restrict__ QG, int r) {
   constexpr int N2 = N * N, N3 = N2 * N;
   const int pid = blockIdx.x * 128 + threadIdx.x;
   if (pid >= N2) return;
-  const double* src = S + (size_t)blockIdx.y * N3 + pid;
+  const int item = blockIdx.y, pair = item % tab.npairs;
+  const cplx* src = T + (size_t)item * N3 + pid;
   cplx v[N];
 #pragma unroll
-  for (int i = 0; i < N; ++i) v[i] = make_double2(src[(size_t)i * N2], 0.0);
+  for (int i = 0; i < N; ++i) v[i] = src[(size_t)i * N2];
   fft_reg<N, -1>(v);
-  cplx* dst = T + (size_t)blockIdx.y * N3 + pid;
+  const int kxs = sfreq(pid / N, N), kys = sfreq(pid % N, N);
+  const int k2xy = kxs * kxs + kys * kys;
+  const double* bv = tab.bvhs + ((size_t)pair * tab.N_rho + r) * tab.K2n;
+  const double scale = tab.w_rho[r];
+  cplx* dst = QG + (size_t)item * N3 + pid;
 #pragma unroll
-  for (int k = 0; k < N; ++k) dst[(size_t)k * N2] = v[k];
+  for (int k = 0; k < N; ++k) {
+    const int kzs = k - (k >= N / 2 ? N : 0);
+    const double b = scale * __ldg(&bv[k2xy + kzs * kzs]);
+    cplx acc = FIRST ? make_double2(0.0, 0.0) : dst[(size_t)k * N2];
+    acc.x = fma(b, v[k].x, acc.x);
+    acc.y = fma(b, v[k].y, acc.y);
+    dst[(size_t)k * N2] = acc;
+  }
 }
 
 // ---------------------------------------------------------------- host orchestration ------------
@@ -588,18 +619,17 @@ size_t workspace_bytes_v1(const dgfs_ctx* c, int nx) { return plan_v1(c, nx).tot
 // algorithmic FLOPs of the executed algorithm: a 1-D transform of length N counts
 // 5 N log2 N, pointwise work counts the real operations of the formulas in this file's header.
 namespace {
-struct FlopsV1 { double zshift, nyq, xy, wterm, zfwd, acc, per_r, tail; };
+struct FlopsV1 { double zshift, nyq, xy, wterm, acc, per_r, tail; };
 FlopsV1 flops_v1(const dgfs_ctx* c) {
   const double N = c->N, N2 = N * N, N3 = N2 * N, H = N / 2, M = c->M;
   const double fft1 = 5.0 * N * log2(N), fft3 = 3.0 * N2 * fft1;
   FlopsV1 f{};
   f.zshift = (double)c->v1_nz / c->npairs * N * H * (fft1 + 6.0 * N);   // per item
   f.nyq = M * (3.0 * (2.0 * N * fft1 + 14.0 * N2) + 16.0 * N2);   // three plane jobs + the 1-D sums
-  f.xy = M * N * (2.0 * N * fft1 + 18.0 * N2);    // x, y factors 6 + 6, packing 2, corrections ~2, product 2
+  f.xy = M * N * (2.0 * N * fft1 + 18.0 * N2) + 2.0 * N2 * fft1;   // + forward x, y passes of S_r;    // x, y factors 6 + 6, packing 2, corrections ~2, product 2
   f.wterm = M * N3 * 6.0 + N3;                      // 4 adds + 1 fma per (node, s)
-  f.zfwd = N2 * fft1;
-  f.acc = 2.0 * N2 * fft1 + 4.0 * N3;
-  f.per_r = f.zshift + f.nyq + f.xy + f.wterm + f.zfwd + f.acc;
+  f.acc = N2 * fft1 + 4.0 * N3;                     // forward z pass, QG += w_r b_r .
+  f.per_r = f.zshift + f.nyq + f.xy + f.wterm + f.acc;
   f.tail = 2.0 * fft3 + 11.0 * N3 + fft3 / c->ns;
   return f;
 }
@@ -630,8 +660,8 @@ static int collide_v1_impl(dgfs_ctx* c, const double* f, double* out, int nx, bo
   const size_t smem_plane = plane_smem_per_warp<N>() * W;
   const size_t smem_final = plane_smem_per_warp<N>() * 2;
   const size_t smem_xy = sizeof(cplx) * (size_t)W * JobSmem<N>::WORDS;
-  const size_t smem_wt = sizeof(cplx) * (size_t)2 * WtermSmem<N>::WORDS;
-  const size_t smem_nyq = sizeof(cplx) * (size_t)4 * JobSmem<N>::WORDS;
+  const size_t smem_wt = sizeof(cplx) * (size_t)3 * WtermSmem<N>::WORDS;
+  const size_t smem_nyq = sizeof(cplx) * (size_t)2 * JobSmem<N>::WORDS;
   static bool attr_done = false;
   if (!attr_done) {
     cudaFuncSetAttribute(k_plane_fwd<N, W, 0>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_plane);
@@ -639,7 +669,7 @@ static int collide_v1_impl(dgfs_ctx* c, const double* f, double* out, int nx, bo
     cudaFuncSetAttribute(k_final_xy<N>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_final);
     cudaFuncSetAttribute(k_xy<N, W>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_xy);
     cudaFuncSetAttribute(k_wterm<N>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_wt);
-    cudaFuncSetAttribute(k_nyq2<N>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_nyq);
+    cudaFuncSetAttribute(k_nyq2<N, 2>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_nyq);
     attr_done = true;
   }
   const int pen_blocks = (N2 + 127) / 128;
@@ -658,22 +688,20 @@ static int collide_v1_impl(dgfs_ctx* c, const double* f, double* out, int nx, bo
       k_plane_fwd<N, W, 0><<<dim3(plane_blocks, nb * ns), 32 * W, smem_plane, st>>>(c->tab, T, 1, fhat, 0); }
     { ProfScope ps(c->prof, st, "k_pack_half", 0.0);
       k_pack_half<N><<<(nb * ns * N2 * H + 255) / 256, 256, 0, st>>>(fhat, fhh, nyqy, nb * ns); }
-    cudaMemsetAsync(QG, 0, (size_t)items * N3 * sizeof(cplx), st);
     for (int r = 0; r < c->N_rho; ++r) {
       { ProfScope ps(c->prof, st, "k_zshift", items * fl.zshift);
         k_zshift<N><<<dim3(hpen_blocks, nz, nb), 128, 0, st>>>(c->v1, ns, fhh, Gz, r); }
       { ProfScope ps(c->prof, st, "k_nyq1d", items * c->M * 16.0 * N2);
         k_nyq1d<N><<<(items * c->M + 3) / 4, 128, 0, st>>>(c->v1, c->tab, fhat, nyq, r, items * c->M); }
       { ProfScope ps(c->prof, st, "k_nyq2", items * (fl.nyq - c->M * 16.0 * N2));
-        k_nyq2<N><<<dim3(3, items), 128, smem_nyq, st>>>(c->v1, c->tab, fhh, nyqy, nyq, r); }
-      { ProfScope ps(c->prof, st, "k_xy", items * fl.xy);
-        k_xy<N, W><<<dim3((N + W - 1) / W, items), 32 * W, smem_xy, st>>>(c->v1, c->tab, Gz, nyq, S, r); }
+        k_nyq2<N, 2><<<dim3(3, items), 64, smem_nyq, st>>>(c->v1, c->tab, fhh, nyqy, nyq, r); }
       { ProfScope ps(c->prof, st, "k_wterm", items * fl.wterm);
         k_wterm<N><<<dim3(N / 8, items), 256, smem_wt, st>>>(nyq, c->M, S); }
-      { ProfScope ps(c->prof, st, "k_zfwd_planes", items * fl.zfwd);
-        k_zfwd_planes<N><<<dim3(pen_blocks, items), 128, 0, st>>>(S, T); }
-      { ProfScope ps(c->prof, st, "k_plane_fwd<accumulate>", items * fl.acc);
-        k_plane_fwd<N, W, 1><<<dim3(plane_blocks, items), 32 * W, smem_plane, st>>>(c->tab, T, 1, QG, r); }
+      { ProfScope ps(c->prof, st, "k_xy", items * fl.xy);
+        k_xy<N, W><<<dim3((N + W - 1) / W, items), 32 * W, smem_xy, st>>>(c->v1, c->tab, Gz, nyq, S, T, r); }
+      { ProfScope ps(c->prof, st, "k_zfwd_acc", items * fl.acc);
+        if (r == 0) k_zfwd_acc<N, true><<<dim3(pen_blocks, items), 128, 0, st>>>(c->tab, T, QG, r);
+        else k_zfwd_acc<N, false><<<dim3(pen_blocks, items), 128, 0, st>>>(c->tab, T, QG, r); }
     }
     // step 10
     { ProfScope ps(c->prof, st, "k_final_xy", items * (2.0 * fft3 * 2.0 / 3.0 + 6.0 * N3));

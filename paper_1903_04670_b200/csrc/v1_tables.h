@@ -28,8 +28,8 @@ struct NyqLayout {
   static constexpr int VXP = N;            // [N]     packed (A + iB), y-Nyquist column correction
   static constexpr int VZP = 2 * N;        // [N]     packed, (H,H) element correction per cz
   static constexpr int VT = 3 * N;         // [1]     packed, s_x s_y s_z f^(H,H,H)
-  static constexpr int UXP = 4 * N;        // [cz][cy]
-  static constexpr int UY = 4 * N + N * N; // [cz][cx]
+  static constexpr int UXP = 4 * N;        // [cy][cz]
+  static constexpr int UY = 4 * N + N * N; // [cx][cz]
   static constexpr int UZ = 4 * N + 2 * N * N;   // [cy][cx]
   static constexpr int STRIDE = 4 * N + 3 * N * N;
 };
