@@ -384,7 +384,7 @@ __global__ void __launch_bounds__(32 * NW) k_nyq2(V1Tables t, DevTables tab, con
 //           back into the tile (transposition)
 //   pass 2: lane = cx rebuilds the N packed columns X[ly] = Y_A + i Y_B (mirror half by conjugation), inverse
 //           y pass: Z = a_r + i b_r;  acc[cy] += Re Z Im Z
-// in: S[item][cz][cy][cx] = -sum_s Re W Im W (k_wterm);  out: T[item][cz][kx][ky] = fft_xy of S_r(., ., cz).
+// in: S[item][cz][cy][cx] = -sum_s Re W Im W (k_wterm);  out: T[item][cz][kx][ky <= H] = fft_xy of S_r(., ., cz).
 template <int N, int W>
 __global__ void __launch_bounds__(32 * W) k_xy(V1Tables t, DevTables tab, const cplx* __restrict__ Gz,
                                                const cplx* __restrict__ nyq, const double* __restrict__ S,
@@ -464,9 +464,12 @@ __global__ void __launch_bounds__(32 * W) k_xy(V1Tables t, DevTables tab, const 
 #pragma unroll
     for (int i = 0; i < N; ++i) v[i] = buf[ln * P + i];          // lane = ky
     fft_reg<N, -1>(v);
-    cplx* o = T + ((size_t)item * N + cz) * N2 + ln;
+    // S_r is real: columns ky = 0 .. H determine the rest (Hermitian symmetry), only they are kept
+    if (ln <= H) {
+      cplx* o = T + ((size_t)item * N + cz) * (size_t)(N * (H + 1)) + ln;
 #pragma unroll
-    for (int k = 0; k < N; ++k) o[k * N] = v[k];                 // [cz][kx][ky]
+      for (int k = 0; k < N; ++k) o[k * (H + 1)] = v[k];         // [cz][kx][ky <= H]
+    }
   }
 }
 
@@ -553,33 +556,83 @@ __global__ void __launch_bounds__(256, 2) k_wterm(const cplx* __restrict__ nyq, 
     }
 }
 
-// Forward z pass and steps 7-8: thread per (kx,ky) pencil of T[item][cz][kx][ky];
-// QG[item][kz][kx][ky] (+)= w_r b_r(|k|^2) t3.  FIRST: the first radial node stores instead of accumulating.
+// Forward z pass and steps 7-8 for a group of nr radial nodes r0 .. r0+nr-1:
+//   QGh[item][kz][kx][ky <= H] (+)= sum_r w_r b_r(|k|^2) fft_z( T_r[item][.][kx][ky] ).
+// Thread pair per (kx,ky) pencil: parity 0 computes the even kz, parity 1 the odd kz (one radix-2
+// decimation-in-frequency step, then a length-N/2 transform in registers), so that the accumulators of
+// the whole group stay in registers and QG is touched once per group.  FIRST: store, do not accumulate.
 template <int N, bool FIRST>
-__global__ void __launch_bounds__(128) k_zfwd_acc(DevTables tab, const cplx* __restrict__ T, cplx* __restrict__ QG, int r) {
-  constexpr int N2 = N * N, N3 = N2 * N;
-  const int pid = blockIdx.x * 128 + threadIdx.x;
-  if (pid >= N2) return;
+__global__ void __launch_bounds__(256) k_zfwd_acc(DevTables tab, const cplx* __restrict__ T, size_t slot_stride,
+                                                  cplx* __restrict__ QGh, int r0, int nr) {
+  constexpr int H = N / 2, NPH = N * (H + 1);
+  const int par = threadIdx.x >> 7;
+  const int pid = blockIdx.x * 128 + (threadIdx.x & 127);
+  if (pid >= NPH) return;
   const int item = blockIdx.y, pair = item % tab.npairs;
-  const cplx* src = T + (size_t)item * N3 + pid;
-  cplx v[N];
-#pragma unroll
-  for (int i = 0; i < N; ++i) v[i] = src[(size_t)i * N2];
-  fft_reg<N, -1>(v);
-  const int kxs = sfreq(pid / N, N), kys = sfreq(pid % N, N);
+  const int kxs = sfreq(pid / (H + 1), N), kys = sfreq(pid % (H + 1), N);
   const int k2xy = kxs * kxs + kys * kys;
-  const double* bv = tab.bvhs + ((size_t)pair * tab.N_rho + r) * tab.K2n;
-  const double scale = tab.w_rho[r];
-  cplx* dst = QG + (size_t)item * N3 + pid;
+  cplx acc[H];
 #pragma unroll
-  for (int k = 0; k < N; ++k) {
-    const int kzs = k - (k >= N / 2 ? N : 0);
-    const double b = scale * __ldg(&bv[k2xy + kzs * kzs]);
-    cplx acc = FIRST ? make_double2(0.0, 0.0) : dst[(size_t)k * N2];
-    acc.x = fma(b, v[k].x, acc.x);
-    acc.y = fma(b, v[k].y, acc.y);
-    dst[(size_t)k * N2] = acc;
+  for (int k = 0; k < H; ++k) acc[k] = make_double2(0.0, 0.0);
+  for (int sl = 0; sl < nr; ++sl) {
+    const cplx* src = T + (size_t)sl * slot_stride + (size_t)item * (N * NPH) + pid;
+    cplx u[H];
+    if (par == 0) {
+#pragma unroll
+      for (int j = 0; j < H; ++j) u[j] = cadd(src[(size_t)j * NPH], src[(size_t)(j + H) * NPH]);
+    } else {
+#pragma unroll
+      for (int j = 0; j < H; ++j) u[j] = twiddle_mul<N, -1>(csub(src[(size_t)j * NPH], src[(size_t)(j + H) * NPH]), j);
+    }
+    fft_reg<H, -1>(u);
+    const double* bv = tab.bvhs + ((size_t)pair * tab.N_rho + r0 + sl) * tab.K2n + k2xy;
+    const double scale = tab.w_rho[r0 + sl];
+#pragma unroll
+    for (int k = 0; k < H; ++k) {
+      const int kz = 2 * k + par, kzs = kz - (kz >= H ? N : 0);
+      const double b = scale * __ldg(&bv[kzs * kzs]);
+      acc[k].x = fma(b, u[k].x, acc[k].x);
+      acc[k].y = fma(b, u[k].y, acc[k].y);
+    }
   }
+  cplx* dst = QGh + (size_t)item * (N * NPH) + pid;
+#pragma unroll
+  for (int k = 0; k < H; ++k) {
+    cplx* d = dst + (size_t)(2 * k + par) * NPH;
+    if (FIRST) *d = acc[k];
+    else { cplx o = *d; *d = make_double2(o.x + acc[k].x, o.y + acc[k].y); }
+  }
+}
+
+// Step 10, spectral part, from the Hermitian half of QG: inverse x,y passes of QG (job 0) and of
+// c^(pq) f^_q (job 1), scaled by 1/N^3.  QG(lx, ly, lz) for ly > H is conj QGh(-lx, -ly, -lz).
+// out: G2[item][job][lz][cy][cx] (the layout k_z_final reads).
+template <int N>
+__global__ void __launch_bounds__(64) k_final_xy_h(DevTables tab, const cplx* __restrict__ fhat, const cplx* __restrict__ QGh,
+                                                   cplx* __restrict__ G2) {
+  constexpr int N2 = N * N, N3 = N2 * N, H = N / 2, NPH = N * (H + 1);
+  extern __shared__ cplx sm[];
+  const int job = threadIdx.x >> 5, lane = threadIdx.x & 31;
+  cplx* buf = sm + (size_t)job * (N * (N + 1) + N);
+  const int lz = blockIdx.x, item = blockIdx.y;
+  const int pair = item % tab.npairs, xl = item / tab.npairs;
+  const int q = pair % tab.ns;
+  const double inv = 1.0 / ((double)N3);
+  const cplx* qa = QGh + (size_t)item * (N * NPH) + (size_t)lz * NPH;
+  const cplx* qb = QGh + (size_t)item * (N * NPH) + (size_t)((N - lz) % N) * NPH;
+  const cplx* in = fhat + ((size_t)xl * tab.ns + q) * N3 + (size_t)lz * N2;
+  const cplx* cl = tab.closs + (size_t)pair * N3 + (size_t)lz * N2;
+  cplx* o = G2 + ((size_t)item * 2 + job) * N3 + (size_t)lz * N2;
+  warp_plane_fft<N, +1>(
+      buf, lane,
+      [&](int lx, int ly) {
+        cplx v;
+        if (job == 1) v = cmul(in[lx * N + ly], cl[lx * N + ly]);
+        else if (ly <= H) v = qa[lx * (H + 1) + ly];
+        else { v = qb[((N - lx) % N) * (H + 1) + (N - ly)]; v.y = -v.y; }
+        return make_double2(v.x * inv, v.y * inv);
+      },
+      [](cplx x, int) { return x; }, [&](int cy, int cx, cplx val) { o[cy * N + cx] = val; });
 }
 
 // ---------------------------------------------------------------- host orchestration ------------
@@ -604,11 +657,14 @@ PlanV1 plan_v1(const dgfs_ctx* c, int nx) {
   pl.off_fhat = take((size_t)nbx * c->ns * arr);
   pl.off_fhh = take((size_t)nbx * c->ns * (arr / 2));
   pl.off_nyqy = take((size_t)nbx * c->ns * (N * N / 2) * sizeof(cplx));
-  pl.off_qg = take(items * arr);
+  const size_t half_arr = N * N * (N / 2 + 1) * sizeof(cplx);
+  pl.off_qg = take(items * half_arr);
   pl.off_gz = take(gz > g2 ? gz : g2);
   pl.off_nyq = take(items * c->M * nyq_stride * sizeof(cplx));
   pl.off_s = take(items * N3 * sizeof(double));
-  pl.off_t = take(items * arr);
+  // T: forward-transformed planes of a group of radial nodes; also the z-pass scratch of step 1
+  const size_t tg = (size_t)c->v1_rgroup * items * half_arr, t1 = (size_t)nbx * c->ns * arr;
+  pl.off_t = take(tg > t1 ? tg : t1);
   pl.total = off;
   return pl;
 }
@@ -626,9 +682,9 @@ FlopsV1 flops_v1(const dgfs_ctx* c) {
   FlopsV1 f{};
   f.zshift = (double)c->v1_nz / c->npairs * N * H * (fft1 + 6.0 * N);   // per item
   f.nyq = M * (3.0 * (2.0 * N * fft1 + 14.0 * N2) + 16.0 * N2);   // three plane jobs + the 1-D sums
-  f.xy = M * N * (2.0 * N * fft1 + 18.0 * N2) + 2.0 * N2 * fft1;   // + forward x, y passes of S_r;    // x, y factors 6 + 6, packing 2, corrections ~2, product 2
+  f.xy = M * N * (2.0 * N * fft1 + 18.0 * N2) + N * (N + 1.0) * fft1;   // + forward y (real rows) and x (H+1 columns) passes of S_r;    // x, y factors 6 + 6, packing 2, corrections ~2, product 2
   f.wterm = M * N3 * 6.0 + N3;                      // 4 adds + 1 fma per (node, s)
-  f.acc = N2 * fft1 + 4.0 * N3;                     // forward z pass, QG += w_r b_r .
+  f.acc = N * (H + 1.0) * (fft1 + 4.0 * N);         // forward z pass and QG += w_r b_r . on the Hermitian half
   f.per_r = f.zshift + f.nyq + f.xy + f.wterm + f.acc;
   f.tail = 2.0 * fft3 + 11.0 * N3 + fft3 / c->ns;
   return f;
@@ -666,7 +722,7 @@ static int collide_v1_impl(dgfs_ctx* c, const double* f, double* out, int nx, bo
   if (!attr_done) {
     cudaFuncSetAttribute(k_plane_fwd<N, W, 0>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_plane);
     cudaFuncSetAttribute(k_plane_fwd<N, W, 1>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_plane);
-    cudaFuncSetAttribute(k_final_xy<N>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_final);
+    cudaFuncSetAttribute(k_final_xy_h<N>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_final);
     cudaFuncSetAttribute(k_xy<N, W>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_xy);
     cudaFuncSetAttribute(k_wterm<N>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_wt);
     cudaFuncSetAttribute(k_nyq2<N, 2>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_nyq);
@@ -675,12 +731,15 @@ static int collide_v1_impl(dgfs_ctx* c, const double* f, double* out, int nx, bo
   const int pen_blocks = (N2 + 127) / 128;
   const int hpen_blocks = (N * H + 127) / 128;
   const int plane_blocks = (N + W - 1) / W;
+  const int hp_blocks = (N * (H + 1) + 127) / 128;
+  const int RG = c->v1_rgroup;
   const double fft3 = 15.0 * N3 * log2((double)N);
   const FlopsV1 fl = flops_v1(c);
   for (int x0 = 0; x0 < nx; x0 += pl.nbx) {
     const int nb = (nx - x0 < pl.nbx) ? nx - x0 : pl.nbx;
     const int items = nb * np;
     const double* fc = f + (size_t)x0 * ns * N3;
+    const size_t slot_stride = (size_t)items * N2 * (H + 1);
     // step 1, once per species (R-2), plus the half-packed copy
     { ProfScope ps(c->prof, st, "k_zfwd_real", nb * ns * fft3 / 3.0);
       k_zfwd_real<N><<<dim3(pen_blocks, nb * ns), 128, 0, st>>>(fc, T); }
@@ -698,14 +757,17 @@ static int collide_v1_impl(dgfs_ctx* c, const double* f, double* out, int nx, bo
       { ProfScope ps(c->prof, st, "k_wterm", items * fl.wterm);
         k_wterm<N><<<dim3(N / 8, items), 256, smem_wt, st>>>(nyq, c->M, S); }
       { ProfScope ps(c->prof, st, "k_xy", items * fl.xy);
-        k_xy<N, W><<<dim3((N + W - 1) / W, items), 32 * W, smem_xy, st>>>(c->v1, c->tab, Gz, nyq, S, T, r); }
-      { ProfScope ps(c->prof, st, "k_zfwd_acc", items * fl.acc);
-        if (r == 0) k_zfwd_acc<N, true><<<dim3(pen_blocks, items), 128, 0, st>>>(c->tab, T, QG, r);
-        else k_zfwd_acc<N, false><<<dim3(pen_blocks, items), 128, 0, st>>>(c->tab, T, QG, r); }
+        k_xy<N, W><<<dim3((N + W - 1) / W, items), 32 * W, smem_xy, st>>>(c->v1, c->tab, Gz, nyq, S, T + (size_t)(r % RG) * slot_stride, r); }
+      if ((r + 1) % RG == 0 || r + 1 == c->N_rho) {
+        const int r0 = (r / RG) * RG, nr = r + 1 - r0;
+        ProfScope ps(c->prof, st, "k_zfwd_acc", items * fl.acc * nr);
+        if (r0 == 0) k_zfwd_acc<N, true><<<dim3(hp_blocks, items), 256, 0, st>>>(c->tab, T, slot_stride, QG, r0, nr);
+        else k_zfwd_acc<N, false><<<dim3(hp_blocks, items), 256, 0, st>>>(c->tab, T, slot_stride, QG, r0, nr);
+      }
     }
     // step 10
     { ProfScope ps(c->prof, st, "k_final_xy", items * (2.0 * fft3 * 2.0 / 3.0 + 6.0 * N3));
-      k_final_xy<N><<<dim3(N, items), 64, smem_final, st>>>(c->tab, fhat, QG, Gz); }
+      k_final_xy_h<N><<<dim3(N, items), 64, smem_final, st>>>(c->tab, fhat, QG, Gz); }
     { ProfScope ps(c->prof, st, "k_z_final", items * (2.0 * fft3 / 3.0 + 5.0 * N3));
       if (pairs_out)
         k_z_final<N, false><<<dim3(pen_blocks, items), 128, 0, st>>>(c->tab, Gz, fc, out + (size_t)x0 * np * N3);

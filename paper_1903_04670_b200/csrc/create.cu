@@ -477,6 +477,9 @@ extern "C" int dgfs_create(const dgfs_params* P, dgfs_ctx** out) {
   if (c->use_v1) {
     const char* ch = getenv("DGFS_V1_CHUNK");
     if (ch && atoi(ch) > 0) c->v1_chunk = atoi(ch);
+    const char* rg = getenv("DGFS_V1_RGROUP");
+    if (rg && atoi(rg) > 0) c->v1_rgroup = atoi(rg);
+    if (c->v1_rgroup > c->N_rho) c->v1_rgroup = c->N_rho;
     rc = build_tables_v1(c);
     if (rc != DGFS_OK) { g_create_error = c->err; dgfs_destroy(c); return rc; }
   }

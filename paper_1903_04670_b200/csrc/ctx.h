@@ -102,6 +102,7 @@ struct dgfs_ctx {
   // v1 pipeline (collide_v1.cu): tables built by build_tables_v1, used when no pair needs the full b table
   bool use_v1 = false;
   int v1_chunk = 128;                    // spatial points per launch group (sized for the L2)
+  int v1_rgroup = 8;                     // radial nodes per forward-z / QG accumulation launch
   int v1_nz = 0;
   std::vector<int> v1_zsp, v1_zmap;
   int *d_v1_zsp = nullptr, *d_v1_zmap = nullptr;
