@@ -139,7 +139,7 @@ __global__ void __launch_bounds__(256) k_pack_half(const cplx* __restrict__ fhat
 // Inverse z pass of h_z f^ for z job k = blockIdx.y of point blockIdx.z; thread per (lx, m) pencil.
 // in: fhh[xl][species][lz][lx][m];  out: Gz[xl][k][cz][lx][m].
 template <int N>
-__global__ void __launch_bounds__(128) k_zshift(V1Tables t, int ns, const cplx* __restrict__ fhh, cplx* __restrict__ Gz, int r) {
+__global__ void __launch_bounds__(128, 3) k_zshift(V1Tables t, int ns, const cplx* __restrict__ fhh, cplx* __restrict__ Gz, int r) {
   constexpr int H = N / 2, NP = N * H;
   const int pid = blockIdx.x * 128 + threadIdx.x;
   if (pid >= NP) return;

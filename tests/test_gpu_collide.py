@@ -90,6 +90,7 @@ def test_v0_pipeline_on_vhs_pairs(torch_cuda, monkeypatch, N, N_rho, M, ns):
     (8, 3, 12, 3, 0.5),        # 9 pairs, strongly rough input: the Nyquist-plane terms are O(1) of the result
     (16, 2, 32, 1, 0.3),       # single species: sides A and B share their z shifts
     (32, 2, 6, 2, 0.3),        # octahedron: sigma with two zero components
+    (32, 1, 32, 1, 0.3),       # more uz planes than k_wterm keeps resident in shared memory
 ])
 def test_v1_nyquist_terms(torch_cuda, N, N_rho, M, ns, noise):
     _small_radial_rule(torch_cuda, N, N_rho, M, ns, (1.0,) * ns, noise=noise)
