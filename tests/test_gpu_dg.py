@@ -1,0 +1,109 @@
+"""Parity of dgfs_advect_rhs / dgfs_step (rows D1-D4, through the C ABI) with oracle/dg.py.
+
+Tolerances: transport alone is a handful of fp64 operations per node: 1e-12 relative to max|rhs|.
+A full step carries the collision term (1e-10 relative to max|Q|, north_star); after n steps the
+state is compared at 1e-10 relative to max|f| (dt |Q| << |f|, so this is the looser of the two bars
+only in appearance: the difference is dominated by dt times the collision-term difference)."""
+import numpy as np
+import pytest
+
+from workloads import get_config, make_dg_state
+
+pytestmark = pytest.mark.gpu
+
+
+@pytest.fixture(scope="module")
+def torch_cuda():
+    import torch
+    if not torch.cuda.is_available():
+        pytest.fail("GPU tests need a CUDA device: there is no CPU fallback")
+    torch.cuda.set_device(0)
+    return torch
+
+
+def _rough_state(ne, K, ns, N, L, mass, seed, wall_T=(1.0, 1.0)):
+    from oracle.dg import wall_maxwellian
+    rng = np.random.default_rng(seed)
+    f = np.empty((ne, K, ns, N ** 3))
+    for p in range(ns):
+        f[:, :, p] = (0.6 + 0.4 * p) * wall_maxwellian(N, L, (0.1, -0.05, 0.0), 1.1, mass[p])
+    return f * (1.0 + 0.2 * rng.uniform(-1, 1, f.shape))
+
+
+@pytest.mark.parametrize("ne,order,ns,N", [(1, 1, 1, 8), (3, 2, 2, 8), (5, 3, 2, 16), (2, 7, 1, 8), (16, 3, 3, 8)])
+def test_advect_rhs_matches_oracle(torch_cuda, ne, order, ns, N):
+    torch = torch_cuda
+    from oracle import dg
+    from paper_1903_04670_b200 import Dgfs, Mesh1D, api
+    L = 5.0
+    mass = (1.0, 1.5, 2.0)[:ns]
+    K = order + 1
+    wall_T, wall_u = (0.8, 1.2), ((0.0, 0.2, 0.0), (0.0, -0.2, 0.1))
+    f = _rough_state(ne, K, ns, N, L, mass, seed=ne * 10 + order)
+    omesh = dg.Mesh1D(ne, order, x0=-0.3, x1=1.4, wall_T=wall_T, wall_u=wall_u)
+    ro = dg.advect_rhs(omesh, f, N, L, mass)
+    om = [[0.5] * ns] * ns
+    al = [[1.0] * ns] * ns
+    with Dgfs(mass, om, al, N, 2, 6, L, device=0) as op:
+        mesh = Mesh1D(ne, order, x0=-0.3, x1=1.4, wall_T=wall_T, wall_u=wall_u)
+        fd = torch.from_numpy(f).cuda()
+        rd = torch.empty_like(fd)
+        api.dgfs_advect_rhs(op.ctx, mesh, fd, rd)
+        rg = rd.cpu().numpy()
+        with pytest.raises(api.DgfsError):
+            api.dgfs_advect_rhs(op.ctx, mesh, fd, fd)                       # aliasing
+        with pytest.raises(api.DgfsError):
+            api.dgfs_advect_rhs(op.ctx, Mesh1D(ne, 9), fd, rd)              # order out of range
+    assert np.max(np.abs(rg - ro)) < 1e-12 * np.max(np.abs(ro))
+
+
+def test_step_matches_oracle_small(torch_cuda):
+    """2 species, VHS (v1 collision pipeline inside), 3 elements of order 2, 2 SSP-RK3 steps."""
+    torch = torch_cuda
+    from oracle import dg
+    from oracle.tables import precompute
+    from oracle.collide import collide
+    from paper_1903_04670_b200 import Dgfs, Mesh1D, api
+    N, L, N_rho, M = 8, 5.0, 3, 6
+    mass = (1.0, 2.0)
+    om = ((0.81, 0.805), (0.805, 0.8))
+    al = ((1.0, 1.0), (1.0, 1.0))
+    ne, order, dt, nsteps = 3, 2, 2e-3, 2
+    f = _rough_state(ne, order + 1, 2, N, L, mass, seed=3)
+    tab = precompute(N, N_rho, M, L, mass, om, al)
+    omesh = dg.Mesh1D(ne, order, wall_T=(0.8, 1.2))
+    fo = dg.step(omesh, f, dt, nsteps, N, L, mass, collide=lambda g: collide(tab, g))
+    with Dgfs(mass, om, al, N, N_rho, M, L, device=0) as op:
+        fd = torch.from_numpy(f).cuda()
+        api.dgfs_step(op.ctx, Mesh1D(ne, order, wall_T=(0.8, 1.2)), fd, dt, nsteps)
+        fg = fd.cpu().numpy()
+        api.dgfs_step(op.ctx, Mesh1D(ne, order, wall_T=(0.8, 1.2)), fd, dt, 0)          # nsteps = 0: no-op
+        assert np.array_equal(fd.cpu().numpy(), fg)
+    assert np.max(np.abs(fg - fo)) < 1e-10 * np.max(np.abs(fo))
+    assert np.max(np.abs(fg - f)) > 1e-4 * np.max(np.abs(f))                  # the state did move
+
+
+def test_step_c3_one_step_sampled_elements(torch_cuda):
+    """Config c3 (3 species, 8 of 9 pairs VSS, 16 elements of order 3, N = 24): one full RK3 step of the
+    whole slab on the GPU.  Upwinding moves information by one element per stage, so element 0 after one
+    step of three stages depends on elements 0..3 and the left wall only; the oracle steps that 4-element
+    sub-slab (its artificial right wall reaches element 1 at the earliest) and element 0 is compared."""
+    torch = torch_cuda
+    from oracle import dg
+    from oracle.tables import precompute
+    from oracle.collide import collide
+    from paper_1903_04670_b200 import Dgfs, Mesh1D, api
+    cfg = get_config("c3")
+    f = make_dg_state(cfg)
+    K = cfg.order + 1
+    tab = precompute(cfg.N, cfg.N_rho, cfg.M, cfg.L, cfg.mass, cfg.omega, cfg.alpha)
+    h = 1.0 / cfg.ne
+    # oracle on elements 0..3 with the true left wall; its element 0 after one step only depends on elements 0..3
+    nsub = 4
+    omesh = dg.Mesh1D(nsub, cfg.order, x0=0.0, x1=nsub * h, wall_T=cfg.wall_T)
+    fo = dg.step(omesh, f[:nsub].copy(), cfg.dt, 1, cfg.N, cfg.L, cfg.mass, collide=lambda g: collide(tab, g))
+    with Dgfs.from_config(cfg, device=0) as op:
+        fd = torch.from_numpy(f).cuda()
+        api.dgfs_step(op.ctx, Mesh1D(cfg.ne, cfg.order, wall_T=cfg.wall_T), fd, cfg.dt, 1)
+        fg = fd[:1].cpu().numpy()
+    assert np.max(np.abs(fg[0] - fo[0])) < 1e-10 * np.max(np.abs(fo[0]))
