@@ -164,10 +164,11 @@ def main():
     if world > 1:
         dist.barrier()
     from paper_1903_04670_b200 import Dgfs
+    from paper_1903_04670_b200.parallel import rank_seed, max_over_ranks, whole_job_rate
 
     nx = args.nx if args.nx > 0 else cfg.nx
     # weak scaling: every rank owns its own nx points (rank r draws them with seed + 1000 r)
-    rcfg = dataclasses.replace(cfg, seed=cfg.seed + 1000 * rank)
+    rcfg = dataclasses.replace(cfg, seed=rank_seed(cfg.seed, rank))
     if nx == cfg.nx:
         f_np = make_points(rcfg, range(nx))
     else:      # reduced batch keeps both halves of the c2 mix
@@ -206,13 +207,10 @@ def main():
     total_ms = ev[0].elapsed_time(ev[-1])
     prof = op.profile(on=False)
     launches = op.launch_count() - launches0
-    t = torch.tensor([total_ms], dtype=torch.float64, device="cuda")
-    if world > 1:
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-    total_ms = float(t.item())
+    total_ms = max_over_ranks(total_ms)
     ms_per_step = total_ms / args.steps
     evals_per_step = nx * cfg.ns * cfg.ns * world
-    value = evals_per_step / (ms_per_step * 1e-3)
+    value = whole_job_rate(nx * cfg.ns * cfg.ns, world, ms_per_step)
 
     # ---------------- end to end: pinned host -> device -> collide -> pinned host ----------------
     # dgfs_collide_host: HOST pointers in and out; the library's own streams carry the copies and the
@@ -230,10 +228,7 @@ def main():
     for _ in range(args.steps):
         e2e_step()
     barrier()
-    t = torch.tensor([(time.perf_counter() - t0) * 1e3], dtype=torch.float64, device="cuda")
-    if world > 1:
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-    e2e_ms = float(t.item()) / args.steps
+    e2e_ms = max_over_ranks((time.perf_counter() - t0) * 1e3) / args.steps
     nbytes = f_host.numel() * 8
 
     if rank == 0:
