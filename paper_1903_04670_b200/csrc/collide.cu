@@ -165,7 +165,7 @@ extern "C" int dgfs_collide_host(dgfs_ctx* c, const double* f_host, double* Q_ho
   cudaError_t e = cudaSetDevice(c->device);
   if (e != cudaSuccess) return check_cuda(c, e, "cudaSetDevice");
   const size_t per_pt = (size_t)c->ns * c->N3;
-  int slab = (int)((size_t)(128u << 20) / (per_pt * sizeof(double)));      // ~128 MiB per slab buffer
+  int slab = (int)((size_t)(256u << 20) / (per_pt * sizeof(double)));      // ~256 MiB per slab buffer
   if (slab < 1) slab = 1;
   if (slab > nx) slab = nx;
   int rc;

@@ -72,6 +72,17 @@ int build_tables_v1(dgfs_ctx* c) {
   }
   const int nz = (int)zk.size();
   c->v1_nz = nz;
+  // jobs with kappa = 0 (sigma_z = 0) do not depend on the radial node: put them last, they run once per chunk
+  {
+    std::vector<int> perm, inv(nz);
+    for (int k = 0; k < nz; ++k) if (zk[k] != 0.0) perm.push_back(k);
+    c->v1_nz0 = nz - (int)perm.size();
+    for (int k = 0; k < nz; ++k) if (zk[k] == 0.0) perm.push_back(k);
+    std::vector<double> zk2(nz); std::vector<int> zsp2(nz);
+    for (int k = 0; k < nz; ++k) { zk2[k] = zk[perm[k]]; zsp2[k] = c->v1_zsp[perm[k]]; inv[perm[k]] = k; }
+    zk = zk2; c->v1_zsp = zsp2;
+    for (auto& m : c->v1_zmap) m = inv[m];
+  }
   std::vector<cplx> hz((size_t)Nr * nz * N), hxy((size_t)np * Nr * M * 2 * 2 * N);
   std::vector<double> szv((size_t)Nr * nz), sxy((size_t)np * Nr * M * 2 * 2);
   for (int r = 0; r < Nr; ++r) {
@@ -136,14 +147,14 @@ __global__ void __launch_bounds__(256) k_pack_half(const cplx* __restrict__ fhat
   }
 }
 
-// Inverse z pass of h_z f^ for z job k = blockIdx.y of point blockIdx.z; thread per (lx, m) pencil.
+// Inverse z pass of h_z f^ for z job k = k0 + blockIdx.y of point blockIdx.z; thread per (lx, m) pencil.
 // in: fhh[xl][species][lz][lx][m];  out: Gz[xl][k][cz][lx][m].
 template <int N>
-__global__ void __launch_bounds__(128, 3) k_zshift(V1Tables t, int ns, const cplx* __restrict__ fhh, cplx* __restrict__ Gz, int r) {
+__global__ void __launch_bounds__(128, 3) k_zshift(V1Tables t, int ns, const cplx* __restrict__ fhh, cplx* __restrict__ Gz, int r, int k0) {
   constexpr int H = N / 2, NP = N * H;
   const int pid = blockIdx.x * 128 + threadIdx.x;
   if (pid >= NP) return;
-  const int k = blockIdx.y, xl = blockIdx.z;
+  const int k = k0 + blockIdx.y, xl = blockIdx.z;
   const cplx* src = fhh + ((size_t)xl * ns + t.zsp[k]) * (size_t)(N * NP) + pid;
   const cplx* hz = t.hz + ((size_t)r * t.nz + k) * N;
   cplx v[N];
@@ -680,7 +691,7 @@ FlopsV1 flops_v1(const dgfs_ctx* c) {
   const double N = c->N, N2 = N * N, N3 = N2 * N, H = N / 2, M = c->M;
   const double fft1 = 5.0 * N * log2(N), fft3 = 3.0 * N2 * fft1;
   FlopsV1 f{};
-  f.zshift = (double)c->v1_nz / c->npairs * N * H * (fft1 + 6.0 * N);   // per item
+  f.zshift = (double)(c->v1_nz - c->v1_nz0) / c->npairs * N * H * (fft1 + 6.0 * N);   // per item and radial node
   f.nyq = M * (3.0 * (2.0 * N * fft1 + 14.0 * N2) + 16.0 * N2);   // three plane jobs + the 1-D sums
   f.xy = M * N * (2.0 * N * fft1 + 18.0 * N2) + N * (N + 1.0) * fft1;   // + forward y (real rows) and x (H+1 columns) passes of S_r;    // x, y factors 6 + 6, packing 2, corrections ~2, product 2
   f.wterm = M * N3 * 6.0 + N3;                      // 4 adds + 1 fma per (node, s)
@@ -712,7 +723,7 @@ static int collide_v1_impl(dgfs_ctx* c, const double* f, double* out, int nx, bo
   cplx* nyq = (cplx*)(ws + pl.off_nyq);
   double* S = (double*)(ws + pl.off_s);
   cplx* T = (cplx*)(ws + pl.off_t);
-  const int ns = c->ns, np = c->npairs, nz = c->v1_nz;
+  const int ns = c->ns, np = c->npairs, nz = c->v1_nz, nz0 = c->v1_nz0;
   const size_t smem_plane = plane_smem_per_warp<N>() * W;
   const size_t smem_final = plane_smem_per_warp<N>() * 2;
   const size_t smem_xy = sizeof(cplx) * (size_t)W * JobSmem<N>::WORDS;
@@ -747,9 +758,14 @@ static int collide_v1_impl(dgfs_ctx* c, const double* f, double* out, int nx, bo
       k_plane_fwd<N, W, 0><<<dim3(plane_blocks, nb * ns), 32 * W, smem_plane, st>>>(c->tab, T, 1, fhat, 0); }
     { ProfScope ps(c->prof, st, "k_pack_half", 0.0);
       k_pack_half<N><<<(nb * ns * N2 * H + 255) / 256, 256, 0, st>>>(fhat, fhh, nyqy, nb * ns); }
+    if (nz0 > 0) {     // the unshifted arrays (sigma_z = 0), the same for every radial node
+      ProfScope ps(c->prof, st, "k_zshift", items * fl.zshift * nz0 / (nz - nz0 > 0 ? nz - nz0 : 1));
+      k_zshift<N><<<dim3(hpen_blocks, nz0, nb), 128, 0, st>>>(c->v1, ns, fhh, Gz, 0, nz - nz0);
+    }
     for (int r = 0; r < c->N_rho; ++r) {
+      if (nz > nz0)
       { ProfScope ps(c->prof, st, "k_zshift", items * fl.zshift);
-        k_zshift<N><<<dim3(hpen_blocks, nz, nb), 128, 0, st>>>(c->v1, ns, fhh, Gz, r); }
+        k_zshift<N><<<dim3(hpen_blocks, nz - nz0, nb), 128, 0, st>>>(c->v1, ns, fhh, Gz, r, 0); }
       { ProfScope ps(c->prof, st, "k_nyq1d", items * c->M * 16.0 * N2);
         k_nyq1d<N><<<(items * c->M + 3) / 4, 128, 0, st>>>(c->v1, c->tab, fhat, nyq, r, items * c->M); }
       { ProfScope ps(c->prof, st, "k_nyq2", items * (fl.nyq - c->M * 16.0 * N2));

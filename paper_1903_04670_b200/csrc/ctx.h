@@ -101,9 +101,9 @@ struct dgfs_ctx {
   dgfs::DevTables tab{};
   // v1 pipeline (collide_v1.cu): tables built by build_tables_v1, used when no pair needs the full b table
   bool use_v1 = false;
-  int v1_chunk = 128;                    // spatial points per launch group (sized for the L2)
-  int v1_rgroup = 8;                     // radial nodes per forward-z / QG accumulation launch
-  int v1_nz = 0;
+  int v1_chunk = 512;                    // spatial points per launch group (large launches amortise the tails)
+  int v1_rgroup = 16;                    // radial nodes per forward-z / QG accumulation launch
+  int v1_nz = 0, v1_nz0 = 0;             // z jobs; the last v1_nz0 of them have sigma_z = 0
   std::vector<int> v1_zsp, v1_zmap;
   int *d_v1_zsp = nullptr, *d_v1_zmap = nullptr;
   dgfs::cplx *d_v1_hz = nullptr, *d_v1_hxy = nullptr;
