@@ -485,41 +485,45 @@ __global__ void __launch_bounds__(32 * W) k_xy(V1Tables t, DevTables tab, const 
 }
 
 // S(c) = -sum_s Re W_s(c) Im W_s(c),  W_s(c) = (-1)^cx ux'_s(cy,cz) + (-1)^cy uy_s(cx,cz) + (-1)^cz uz_s(cx,cy)
-// (W = a_i + i b_i, file header).  Block (cz group of 8 planes, item), thread = 2 x 2 tile of (cx, cy), so
-// every table element serves several nodes and all signs are compile-time constants.  The tables of one s
-// (uz plane, 8 rows of ux' and uy) are staged in shared memory by cp.async, three stages over s; uz and
-// uy are stored de-interleaved by the parity of cx so that the pair loads are conflict-free.
+// (W = a_i + i b_i, file header).  This kernel is bound by the L2 -> SM traffic of its tables (150 KB per
+// (item, s) if every byte is fetched once, for 5 FP64 instructions per node), so a block covers as many cz
+// planes as its registers allow: 16 (two groups of 256 threads with 8 planes each; 8 when 16 does not divide
+// N), and the uz plane is fetched once per block.  Thread = 2 x 2 tile of (cx, cy): every table element
+// serves several nodes and all signs are compile-time constants.  The tables of one s (uz plane, rows of
+// ux' and uy) are staged in shared memory by cp.async, three stages over s; uz and uy are stored
+// de-interleaved by the parity of cx so that the pair loads are conflict-free.
 template <int N>
 struct WtermSmem {
-  static constexpr int CZG = 8;
+  static constexpr int CZG = 8, NH = (N % 16 == 0) ? 2 : 1, CZB = CZG * NH, THREADS = 256 * NH;
   static constexpr int Z = 0;                       // [cy][parity][H]
   static constexpr int V = N * N;                   // [i][parity][H]
-  static constexpr int U = N * N + CZG * N;         // [i][cy]
-  static constexpr int WORDS = N * N + 2 * CZG * N;
+  static constexpr int U = N * N + CZB * N;         // [i][cy]
+  static constexpr int WORDS = N * N + 2 * CZB * N;
 };
 template <int N>
-__global__ void __launch_bounds__(256, 2) k_wterm(const cplx* __restrict__ nyq, int M, double* __restrict__ S) {
+__global__ void __launch_bounds__(WtermSmem<N>::THREADS, 2 / WtermSmem<N>::NH) k_wterm(const cplx* __restrict__ nyq, int M, double* __restrict__ S) {
   constexpr int H = N / 2, N2 = N * N, N3 = N2 * N;
   typedef NyqLayout<N> NL;
   typedef WtermSmem<N> WS;
-  constexpr int CZG = WS::CZG;
+  constexpr int CZG = WS::CZG, CZB = WS::CZB, NT = WS::THREADS;
   extern __shared__ cplx sm[];
-  const int tx = threadIdx.x % 16, ty = threadIdx.x / 16;
+  const int half = threadIdx.x / 256, tt = threadIdx.x % 256;
+  const int tx = tt % 16, ty = tt / 16;
   const bool act = tx < H && ty < H;
-  const int cz0 = blockIdx.x * CZG;
+  const int cz0 = blockIdx.x * CZB;
   const cplx* nbase = nyq + (size_t)blockIdx.y * M * NL::STRIDE;
   auto issue = [&](int s) {
     cplx* dst = sm + (size_t)(s % 3) * WS::WORDS;
     const cplx* nq = nbase + (size_t)s * NL::STRIDE;
-    for (int e = threadIdx.x; e < WS::WORDS; e += 256) {
+    for (int e = threadIdx.x; e < WS::WORDS; e += NT) {
       if (e < N2) {
         const int cy = e / N, cx = e % N;
         cp_async16(&dst[WS::Z + (cy * 2 + (cx & 1)) * H + (cx >> 1)], nq + NL::UZ + e);
-      } else if (e < N2 + CZG * N) {
-        const int cx = (e - N2) / CZG, i = (e - N2) % CZG;
+      } else if (e < N2 + CZB * N) {
+        const int cx = (e - N2) / CZB, i = (e - N2) % CZB;
         cp_async16(&dst[WS::V + (i * 2 + (cx & 1)) * H + (cx >> 1)], nq + NL::UY + cx * N + cz0 + i);
       } else {
-        const int cy = (e - N2 - CZG * N) / CZG, i = (e - N2 - CZG * N) % CZG;
+        const int cy = (e - N2 - CZB * N) / CZB, i = (e - N2 - CZB * N) % CZB;
         cp_async16(&dst[WS::U + i * N + cy], nq + NL::UXP + cy * N + cz0 + i);
       }
     }
@@ -541,15 +545,22 @@ __global__ void __launch_bounds__(256, 2) k_wterm(const cplx* __restrict__ nyq, 
     for (int b = 0; b < 2; ++b)
 #pragma unroll
       for (int a = 0; a < 2; ++a) z[b][a] = b_[WS::Z + ((2 * ty + b) * 2 + a) * H + tx];
+    // software pipeline over the planes: the loads of plane i + 1 are in flight during the arithmetic of plane i
+    const cplx* ub = b_ + WS::U + (half * CZG) * N + 2 * ty;
+    const cplx* vb = b_ + WS::V + (half * CZG * 2) * H + tx;
+    cplx un[2] = {ub[0], ub[1]}, vn[2] = {vb[0], vb[H]};
 #pragma unroll
     for (int i = 0; i < CZG; ++i) {
-      const cplx u[2] = {b_[WS::U + i * N + 2 * ty], b_[WS::U + i * N + 2 * ty + 1]};
-      const cplx v[2] = {b_[WS::V + (i * 2) * H + tx], b_[WS::V + (i * 2 + 1) * H + tx]};
+      const cplx u[2] = {un[0], un[1]}, v[2] = {vn[0], vn[1]};
+      if (i + 1 < CZG) {
+        un[0] = ub[(i + 1) * N]; un[1] = ub[(i + 1) * N + 1];
+        vn[0] = vb[(i + 1) * 2 * H]; vn[1] = vb[(i + 1) * 2 * H + H];
+      }
 #pragma unroll
       for (int b = 0; b < 2; ++b)
 #pragma unroll
         for (int a = 0; a < 2; ++a) {
-          // signs: the tile starts at even cx, cy, cz
+          // signs: the tile starts at even cx, cy; plane groups start at even cz
           const double ux_ = a ? -u[b].x : u[b].x, uy_ = a ? -u[b].y : u[b].y;
           const double vx_ = b ? -v[a].x : v[a].x, vy_ = b ? -v[a].y : v[a].y;
           const double zx_ = (i & 1) ? -z[b][a].x : z[b][a].x, zy_ = (i & 1) ? -z[b][a].y : z[b][a].y;
@@ -558,7 +569,7 @@ __global__ void __launch_bounds__(256, 2) k_wterm(const cplx* __restrict__ nyq, 
     }
   }
   if (!act) return;
-  double* o = S + (size_t)blockIdx.y * N3 + (size_t)cz0 * N2 + (2 * ty) * N + 2 * tx;
+  double* o = S + (size_t)blockIdx.y * N3 + (size_t)(cz0 + half * CZG) * N2 + (2 * ty) * N + 2 * tx;
 #pragma unroll
   for (int i = 0; i < CZG; ++i)
 #pragma unroll
@@ -771,7 +782,7 @@ static int collide_v1_impl(dgfs_ctx* c, const double* f, double* out, int nx, bo
       { ProfScope ps(c->prof, st, "k_nyq2", items * (fl.nyq - c->M * 16.0 * N2));
         k_nyq2<N, 2><<<dim3(3, items), 64, smem_nyq, st>>>(c->v1, c->tab, fhh, nyqy, nyq, r); }
       { ProfScope ps(c->prof, st, "k_wterm", items * fl.wterm);
-        k_wterm<N><<<dim3(N / 8, items), 256, smem_wt, st>>>(nyq, c->M, S); }
+        k_wterm<N><<<dim3(N / WtermSmem<N>::CZB, items), WtermSmem<N>::THREADS, smem_wt, st>>>(nyq, c->M, S); }
       { ProfScope ps(c->prof, st, "k_xy", items * fl.xy);
         k_xy<N, W><<<dim3((N + W - 1) / W, items), 32 * W, smem_xy, st>>>(c->v1, c->tab, Gz, nyq, S, T + (size_t)(r % RG) * slot_stride, r); }
       if ((r + 1) % RG == 0 || r + 1 == c->N_rho) {
