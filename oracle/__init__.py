@@ -13,6 +13,7 @@ Pins (tests/test_oracle_*.py, `-m "not gpu"`): brute-force wrapped Galerkin sum 
 exact-kernel Galerkin sum (Eq. 12), closed-form Krook-Wu solution and printed Table 1 errors
 (P:263-327), Table 2 Knudsen numbers, table closed forms, shift/permutation/
 bilinearity invariants, shift identity of Eq. 8, conservation and Maxwellian-null trends.
-Parity-unpinned functions: none for the collision path.  dg.py (reading DG-1..4, the paper
-gives no formulas) is pinned only by textbook properties -- see its header.
+Parity-unpinned functions: none for the collision path.  dg.py (readings DG-1..3, the paper
+gives no formulas) is PARITY-UNPINNED against the paper and pinned only by textbook properties
+(tests/test_oracle_dg.py) -- see its header.
 """
