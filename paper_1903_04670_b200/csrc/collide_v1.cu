@@ -495,10 +495,12 @@ __global__ void __launch_bounds__(32 * W) k_xy(V1Tables t, DevTables tab, const 
 template <int N>
 struct WtermSmem {
   static constexpr int CZG = 8, NH = (N % 16 == 0) ? 2 : 1, CZB = CZG * NH, THREADS = 256 * NH;
+  static constexpr int RS = N + 1;                  // row stride of V and U: consecutive planes land in different banks
   static constexpr int Z = 0;                       // [cy][parity][H]
-  static constexpr int V = N * N;                   // [i][parity][H]
-  static constexpr int U = N * N + CZB * N;         // [i][cy]
-  static constexpr int WORDS = N * N + 2 * CZB * N;
+  static constexpr int V = N * N;                   // [i][parity][H], rows padded to RS
+  static constexpr int U = N * N + CZB * RS;        // [i][cy], rows padded to RS
+  static constexpr int WORDS = N * N + 2 * CZB * RS;
+  static constexpr int COPIES = N * N + 2 * CZB * N;   // elements staged per s
 };
 template <int N>
 __global__ void __launch_bounds__(WtermSmem<N>::THREADS, 2 / WtermSmem<N>::NH) k_wterm(const cplx* __restrict__ nyq, int M, double* __restrict__ S) {
@@ -515,16 +517,16 @@ __global__ void __launch_bounds__(WtermSmem<N>::THREADS, 2 / WtermSmem<N>::NH) k
   auto issue = [&](int s) {
     cplx* dst = sm + (size_t)(s % 3) * WS::WORDS;
     const cplx* nq = nbase + (size_t)s * NL::STRIDE;
-    for (int e = threadIdx.x; e < WS::WORDS; e += NT) {
+    for (int e = threadIdx.x; e < WS::COPIES; e += NT) {
       if (e < N2) {
         const int cy = e / N, cx = e % N;
         cp_async16(&dst[WS::Z + (cy * 2 + (cx & 1)) * H + (cx >> 1)], nq + NL::UZ + e);
       } else if (e < N2 + CZB * N) {
         const int cx = (e - N2) / CZB, i = (e - N2) % CZB;
-        cp_async16(&dst[WS::V + (i * 2 + (cx & 1)) * H + (cx >> 1)], nq + NL::UY + cx * N + cz0 + i);
+        cp_async16(&dst[WS::V + i * WS::RS + (cx & 1) * H + (cx >> 1)], nq + NL::UY + cx * N + cz0 + i);
       } else {
         const int cy = (e - N2 - CZB * N) / CZB, i = (e - N2 - CZB * N) % CZB;
-        cp_async16(&dst[WS::U + i * N + cy], nq + NL::UXP + cy * N + cz0 + i);
+        cp_async16(&dst[WS::U + i * WS::RS + cy], nq + NL::UXP + cy * N + cz0 + i);
       }
     }
     cp_async_commit();
@@ -546,15 +548,15 @@ __global__ void __launch_bounds__(WtermSmem<N>::THREADS, 2 / WtermSmem<N>::NH) k
 #pragma unroll
       for (int a = 0; a < 2; ++a) z[b][a] = b_[WS::Z + ((2 * ty + b) * 2 + a) * H + tx];
     // software pipeline over the planes: the loads of plane i + 1 are in flight during the arithmetic of plane i
-    const cplx* ub = b_ + WS::U + (half * CZG) * N + 2 * ty;
-    const cplx* vb = b_ + WS::V + (half * CZG * 2) * H + tx;
+    const cplx* ub = b_ + WS::U + (half * CZG) * WS::RS + 2 * ty;
+    const cplx* vb = b_ + WS::V + (half * CZG) * WS::RS + tx;
     cplx un[2] = {ub[0], ub[1]}, vn[2] = {vb[0], vb[H]};
 #pragma unroll
     for (int i = 0; i < CZG; ++i) {
       const cplx u[2] = {un[0], un[1]}, v[2] = {vn[0], vn[1]};
       if (i + 1 < CZG) {
-        un[0] = ub[(i + 1) * N]; un[1] = ub[(i + 1) * N + 1];
-        vn[0] = vb[(i + 1) * 2 * H]; vn[1] = vb[(i + 1) * 2 * H + H];
+        un[0] = ub[(i + 1) * WS::RS]; un[1] = ub[(i + 1) * WS::RS + 1];
+        vn[0] = vb[(i + 1) * WS::RS]; vn[1] = vb[(i + 1) * WS::RS + H];
       }
 #pragma unroll
       for (int b = 0; b < 2; ++b)
