@@ -175,6 +175,8 @@ __device__ __forceinline__ void cp_async16(void* smem, const void* gmem) {
 __device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;\n" ::); }
 __device__ __forceinline__ void cp_async_wait_all() { asm volatile("cp.async.wait_group 0;\n" ::: "memory"); }
 __device__ __forceinline__ void cp_async_wait_one() { asm volatile("cp.async.wait_group 1;\n" ::: "memory"); }
+template <int PENDING>
+__device__ __forceinline__ void cp_async_wait_pending() { asm volatile("cp.async.wait_group %0;\n" ::"n"(PENDING) : "memory"); }
 
 // Per-warp shared memory of a plane job: the N x (N+1) tile (input columns, then the transposition) and
 // the job's small tables.
@@ -490,7 +492,7 @@ __global__ void __launch_bounds__(32 * W) k_xy(V1Tables t, DevTables tab, const 
 // planes as its registers allow: 16 (two groups of 256 threads with 8 planes each; 8 when 16 does not divide
 // N), and the uz plane is fetched once per block.  Thread = 2 x 2 tile of (cx, cy): every table element
 // serves several nodes and all signs are compile-time constants.  The tables of one s (uz plane, rows of
-// ux' and uy) are staged in shared memory by cp.async, three stages over s; uz and uy are stored
+// ux' and uy) are staged in shared memory by cp.async, a ring of five stages over s; uz and uy are stored
 // de-interleaved by the parity of cx so that the pair loads are conflict-free.
 template <int N>
 struct WtermSmem {
@@ -501,13 +503,14 @@ struct WtermSmem {
   static constexpr int U = N * N + CZB * RS;        // [i][cy], rows padded to RS
   static constexpr int WORDS = N * N + 2 * CZB * RS;
   static constexpr int COPIES = N * N + 2 * CZB * N;   // elements staged per s
+  static constexpr int STAGES = 5;                     // ring depth: enough bytes in flight to cover the HBM latency
 };
 template <int N>
 __global__ void __launch_bounds__(WtermSmem<N>::THREADS, 2 / WtermSmem<N>::NH) k_wterm(const cplx* __restrict__ nyq, int M, double* __restrict__ S) {
   constexpr int H = N / 2, N2 = N * N, N3 = N2 * N;
   typedef NyqLayout<N> NL;
   typedef WtermSmem<N> WS;
-  constexpr int CZG = WS::CZG, CZB = WS::CZB, NT = WS::THREADS;
+  constexpr int CZG = WS::CZG, CZB = WS::CZB, NT = WS::THREADS, NS = WS::STAGES;
   extern __shared__ cplx sm[];
   const int half = threadIdx.x / 256, tt = threadIdx.x % 256;
   const int tx = tt % 16, ty = tt / 16;
@@ -515,7 +518,7 @@ __global__ void __launch_bounds__(WtermSmem<N>::THREADS, 2 / WtermSmem<N>::NH) k
   const int cz0 = blockIdx.x * CZB;
   const cplx* nbase = nyq + (size_t)blockIdx.y * M * NL::STRIDE;
   auto issue = [&](int s) {
-    cplx* dst = sm + (size_t)(s % 3) * WS::WORDS;
+    cplx* dst = sm + (size_t)(s % NS) * WS::WORDS;
     const cplx* nq = nbase + (size_t)s * NL::STRIDE;
     for (int e = threadIdx.x; e < WS::COPIES; e += NT) {
       if (e < N2) {
@@ -534,14 +537,16 @@ __global__ void __launch_bounds__(WtermSmem<N>::THREADS, 2 / WtermSmem<N>::NH) k
   double acc[CZG][2][2];                      // [cz][cy][cx]
 #pragma unroll
   for (int i = 0; i < CZG; ++i) acc[i][0][0] = acc[i][0][1] = acc[i][1][0] = acc[i][1][1] = 0.0;
-  issue(0);
-  if (M > 1) issue(1);
+  // ring of NS stages: groups 0 .. s + NS - 2 are committed when iteration s waits for group s (empty groups
+  // keep the count uniform at the end)
+#pragma unroll
+  for (int k = 0; k < NS - 1; ++k) { if (k < M) issue(k); else cp_async_commit(); }
   for (int s = 0; s < M; ++s) {
-    if (s + 1 < M) cp_async_wait_one(); else cp_async_wait_all();
+    cp_async_wait_pending<NS - 2>();
     __syncthreads();
-    if (s + 2 < M) issue(s + 2);
+    if (s + NS - 1 < M) issue(s + NS - 1); else cp_async_commit();
     if (!act) continue;
-    const cplx* b_ = sm + (size_t)(s % 3) * WS::WORDS;
+    const cplx* b_ = sm + (size_t)(s % NS) * WS::WORDS;
     cplx z[2][2];
 #pragma unroll
     for (int b = 0; b < 2; ++b)
@@ -740,7 +745,7 @@ static int collide_v1_impl(dgfs_ctx* c, const double* f, double* out, int nx, bo
   const size_t smem_plane = plane_smem_per_warp<N>() * W;
   const size_t smem_final = plane_smem_per_warp<N>() * 2;
   const size_t smem_xy = sizeof(cplx) * (size_t)W * JobSmem<N>::WORDS;
-  const size_t smem_wt = sizeof(cplx) * (size_t)3 * WtermSmem<N>::WORDS;
+  const size_t smem_wt = sizeof(cplx) * (size_t)WtermSmem<N>::STAGES * WtermSmem<N>::WORDS;
   const size_t smem_nyq = sizeof(cplx) * (size_t)2 * JobSmem<N>::WORDS;
   static bool attr_done = false;
   if (!attr_done) {
