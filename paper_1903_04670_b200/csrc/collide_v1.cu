@@ -711,7 +711,9 @@ FlopsV1 flops_v1(const dgfs_ctx* c) {
   FlopsV1 f{};
   f.zshift = (double)(c->v1_nz - c->v1_nz0) / c->npairs * N * H * (fft1 + 6.0 * N);   // per item and radial node
   f.nyq = M * (3.0 * (2.0 * N * fft1 + 14.0 * N2) + 16.0 * N2);   // three plane jobs + the 1-D sums
-  f.xy = M * N * (2.0 * N * fft1 + 18.0 * N2) + N * (N + 1.0) * fft1;   // + forward y (real rows) and x (H+1 columns) passes of S_r;    // x, y factors 6 + 6, packing 2, corrections ~2, product 2
+  // per plane job: two passes of N transforms, x and y factors (6 + 6 per element), packing adds (2), product
+  // fma (2), Nyquist row / column fixes (12 N); per plane: forward y pass on real rows (half) and x pass on H+1 columns
+  f.xy = M * N * (2.0 * N * fft1 + 16.0 * N2 + 12.0 * N) + N * (N + 1.0) * fft1;
   f.wterm = M * N3 * 6.0 + N3;                      // 4 adds + 1 fma per (node, s)
   f.acc = N * (H + 1.0) * (fft1 + 4.0 * N);         // forward z pass and QG += w_r b_r . on the Hermitian half
   f.per_r = f.zshift + f.nyq + f.xy + f.wterm + f.acc;
