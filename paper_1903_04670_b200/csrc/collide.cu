@@ -251,7 +251,7 @@ extern "C" int dgfs_profile_reset(dgfs_ctx* c) {
 }
 extern "C" double dgfs_flops_per_pair_eval(const dgfs_ctx* c, int p, int q) {
   if (!c || p < 0 || q < 0 || p >= c->ns || q >= c->ns) return 0.0;
-  if (c->use_v1) return flops_per_pair_eval_v1(c);
+  if (c->use_v1) return flops_per_pair_eval_v1(c, p * c->ns + q);
   const double N3 = c->N3, fft3 = 15.0 * N3 * log2((double)c->N);
   const double tail = 2.0 * fft3 + 11.0 * N3 + fft3 / c->ns;
   const double rs = (double)c->N_rho * c->M;

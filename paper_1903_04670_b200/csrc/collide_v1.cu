@@ -410,8 +410,8 @@ __global__ void __launch_bounds__(32 * W) k_xy(V1Tables t, DevTables tab, const 
   extern __shared__ cplx sm[];
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
   const int cz = blockIdx.x * W + warp, item = blockIdx.y;
-  if (cz >= N) return;
   const int pair = item % tab.npairs, xl = item / tab.npairs;
+  if (cz >= N || tab.full[pair]) return;
   cplx* buf = sm + (size_t)warp * JS::WORDS;
   const bool act = lane < N;
   const int ln = act ? lane : 0;
@@ -486,6 +486,146 @@ __global__ void __launch_bounds__(32 * W) k_xy(V1Tables t, DevTables tab, const 
   }
 }
 
+// Pairs with a full table b_rs(k) (VSS, table_mode 1): the plane job of every s ends in its own forward
+// transform (no sum over s before it, b depends on s), and the complex product A B is needed:
+//   P = (a_r b_r - a_i b_i) + i (a_r b_i + a_i b_r),   W = a_i + i b_i from the Nyquist fields (file header).
+// Same block / warp mapping and prefetch as k_xy; the warp's shared memory also holds the uz plane and the
+// ux', uy columns of the job.  out: Tf[item][s][cz][kx][ky] = fft_xy of P_s(., ., cz).
+template <int N>
+struct FullSmem {
+  typedef JobSmem<N> JS;
+  static constexpr int UZ = JS::WORDS;          // [cy][cx]
+  static constexpr int UX = JS::WORDS + N * N;  // [cy]   ux'(cy, cz)
+  static constexpr int UY = UX + N;             // [cx]   uy(cx, cz)
+  static constexpr int WORDS = UY + N;
+};
+template <int N, int W>
+__global__ void __launch_bounds__(32 * W) k_xy_full(V1Tables t, DevTables tab, const cplx* __restrict__ Gz,
+                                                    const cplx* __restrict__ nyq, cplx* __restrict__ Tf, int r) {
+  constexpr int H = N / 2, NH = N * H, N2 = N * N, N3 = N2 * N;
+  typedef NyqLayout<N> NL;
+  typedef JobSmem<N> JS;
+  typedef FullSmem<N> FS;
+  constexpr int P = JS::P;
+  static_assert(N <= 32, "one lane per pencil");
+  extern __shared__ cplx sm[];
+  const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+  const int cz = blockIdx.x * W + warp, item = blockIdx.y;
+  const int pair = item % tab.npairs, xl = item / tab.npairs;
+  if (cz >= N || !tab.full[pair]) return;
+  cplx* buf = sm + (size_t)warp * FS::WORDS;
+  const bool act = lane < N;
+  const int ln = act ? lane : 0;
+  const int side = ln / H, m = ln % H;
+  const double szs = (cz & 1) ? -1.0 : 1.0;
+  const double sxb = (ln & 1) ? -1.0 : 1.0;
+  const int* zm = t.zmap + (size_t)pair * tab.M * 2;
+  const cplx* gbase = Gz + (size_t)xl * t.nz * (size_t)(N * NH) + (size_t)cz * NH + m;
+  const cplx* hbase = t.hxy + (((size_t)pair * tab.N_rho + r) * tab.M) * 4 * N;
+  const cplx* nbase = nyq + (size_t)item * tab.M * NL::STRIDE;
+  auto issue = [&](int s) {
+    if (act) {
+      const cplx* g = gbase + (size_t)zm[2 * s + side] * (size_t)(N * NH);
+#pragma unroll
+      for (int i = 0; i < N; ++i) cp_async16(&buf[i * P + ln], g + i * H);
+      const cplx* hx = hbase + (size_t)s * 4 * N;          // [side][x|y][N]
+      cp_async16(&buf[JS::HI + ln], hx + ln);
+      cp_async16(&buf[JS::HI + N + ln], hx + 2 * N + ln);
+      cp_async16(&buf[JS::HM + ln], hx + N + ln);
+      cp_async16(&buf[JS::HM + N + ln], hx + 3 * N + ln);
+      const cplx* nq = nbase + (size_t)s * NL::STRIDE;
+      cp_async16(&buf[JS::VYH + ln], nq + NL::VYH + ln);
+      cp_async16(&buf[JS::VXP + ln], nq + NL::VXP + ln);
+      if (ln == 0) cp_async16(&buf[JS::VZP], nq + NL::VZP + cz);
+#pragma unroll
+      for (int j = 0; j < N; ++j) cp_async16(&buf[FS::UZ + j * N + ln], nq + NL::UZ + j * N + ln);
+      cp_async16(&buf[FS::UX + ln], nq + NL::UXP + ln * N + cz);
+      cp_async16(&buf[FS::UY + ln], nq + NL::UY + ln * N + cz);
+    }
+    cp_async_commit();
+  };
+  issue(0);
+  for (int s = 0; s < tab.M; ++s) {
+    cp_async_wait_all();
+    __syncwarp();
+    cplx X[N];
+    if (act) job_pass1<N, true>(buf, ln, side, m, szs, 1.0);
+    __syncwarp();
+    if (act) {
+      job_pass2_in<N, true>(buf, ln, szs, sxb, X);
+      fft_reg<N, +1>(X);                                   // Z = a_r + i b_r, lane = cx, index = cy
+      const cplx uyv = buf[FS::UY + ln];
+#pragma unroll
+      for (int j = 0; j < N; ++j) {
+        const cplx ux = buf[FS::UX + j], uz = buf[FS::UZ + j * N + ln];
+        const double syj = (j & 1) ? -1.0 : 1.0;
+        const double ai = fma(sxb, ux.x, fma(szs, uz.x, syj * uyv.x));
+        const double bi = fma(sxb, ux.y, fma(szs, uz.y, syj * uyv.y));
+        const double ar = X[j].x, br = X[j].y;
+        X[j] = make_double2(fma(ar, br, -ai * bi), fma(ar, bi, ai * br));
+      }
+      fft_reg<N, -1>(X);                                   // forward y pass: index = ky
+    }
+    __syncwarp();                                          // every lane has read its row of the tile
+    if (act) {
+#pragma unroll
+      for (int j = 0; j < N; ++j) buf[j * P + ln] = X[j];          // [ky][cx]
+    }
+    __syncwarp();
+    if (act) {
+#pragma unroll
+      for (int i = 0; i < N; ++i) X[i] = buf[ln * P + i];          // lane = ky
+    }
+    __syncwarp();
+    if (s + 1 < tab.M) issue(s + 1);                       // tile and tables are free again
+    if (act) {
+      fft_reg<N, -1>(X);                                   // forward x pass
+      cplx* o = Tf + ((size_t)item * tab.M + s) * N3 + (size_t)cz * N2 + ln;
+#pragma unroll
+      for (int k = 0; k < N; ++k) o[k * N] = X[k];         // [cz][kx][ky]
+    }
+  }
+}
+
+// Forward z pass and steps 7-8 of a full-table pair for one radial node:
+//   QG[item][kz][kx][ky] (+)= w_r sum_s b_rs(k) fft_z( Tf[item][s][.][kx][ky] );  thread pair per pencil as in
+// k_zfwd_acc, the sum over s stays in registers.  b is read in SPEC layout [r][s][kz][kx][ky].
+template <int N, bool FIRST>
+__global__ void __launch_bounds__(256) k_zfwd_full(DevTables tab, const cplx* __restrict__ Tf, cplx* __restrict__ QG,
+                                                   size_t qstride, int r) {
+  constexpr int H = N / 2, N2 = N * N, N3 = N2 * N;
+  const int par = threadIdx.x >> 7;
+  const int pid = blockIdx.x * 128 + (threadIdx.x & 127);
+  const int item = blockIdx.y, pair = item % tab.npairs;
+  if (pid >= N2 || !tab.full[pair]) return;
+  const double scale = tab.w_rho[r];
+  cplx acc[H];
+#pragma unroll
+  for (int k = 0; k < H; ++k) acc[k] = make_double2(0.0, 0.0);
+  for (int s = 0; s < tab.M; ++s) {
+    const cplx* src = Tf + ((size_t)item * tab.M + s) * N3 + pid;
+    cplx u[H];
+    if (par == 0) {
+#pragma unroll
+      for (int j = 0; j < H; ++j) u[j] = cadd(src[(size_t)j * N2], src[(size_t)(j + H) * N2]);
+    } else {
+#pragma unroll
+      for (int j = 0; j < H; ++j) u[j] = twiddle_mul<N, -1>(csub(src[(size_t)j * N2], src[(size_t)(j + H) * N2]), j);
+    }
+    fft_reg<H, -1>(u);
+    const cplx* bf = tab.bfull[pair] + ((size_t)r * tab.M + s) * N3 + pid;
+#pragma unroll
+    for (int k = 0; k < H; ++k) acc[k] = cfma(bf[(size_t)(2 * k + par) * N2], u[k], acc[k]);
+  }
+  cplx* dst = QG + (size_t)item * qstride + pid;
+#pragma unroll
+  for (int k = 0; k < H; ++k) {
+    cplx* d = dst + (size_t)(2 * k + par) * N2;
+    const cplx o = FIRST ? make_double2(0.0, 0.0) : *d;
+    *d = make_double2(fma(scale, acc[k].x, o.x), fma(scale, acc[k].y, o.y));
+  }
+}
+
 // S(c) = -sum_s Re W_s(c) Im W_s(c),  W_s(c) = (-1)^cx ux'_s(cy,cz) + (-1)^cy uy_s(cx,cz) + (-1)^cz uz_s(cx,cy)
 // (W = a_i + i b_i, file header).  This kernel is bound by the L2 -> SM traffic of its tables (150 KB per
 // (item, s) if every byte is fetched once, for 5 FP64 instructions per node), so a block covers as many cz
@@ -506,12 +646,13 @@ struct WtermSmem {
   static constexpr int STAGES = 5;                     // ring depth: enough bytes in flight to cover the HBM latency
 };
 template <int N>
-__global__ void __launch_bounds__(WtermSmem<N>::THREADS, 2 / WtermSmem<N>::NH) k_wterm(const cplx* __restrict__ nyq, int M, double* __restrict__ S) {
+__global__ void __launch_bounds__(WtermSmem<N>::THREADS, 2 / WtermSmem<N>::NH) k_wterm(const cplx* __restrict__ nyq, int M, double* __restrict__ S, const unsigned char* __restrict__ full, int npairs) {
   constexpr int H = N / 2, N2 = N * N, N3 = N2 * N;
   typedef NyqLayout<N> NL;
   typedef WtermSmem<N> WS;
   constexpr int CZG = WS::CZG, CZB = WS::CZB, NT = WS::THREADS, NS = WS::STAGES;
   extern __shared__ cplx sm[];
+  if (full[blockIdx.y % npairs]) return;            // pairs with a full b table take k_xy_full (uniform per block)
   const int half = threadIdx.x / 256, tt = threadIdx.x % 256;
   const int tx = tt % 16, ty = tt / 16;
   const bool act = tx < H && ty < H;
@@ -592,12 +733,12 @@ __global__ void __launch_bounds__(WtermSmem<N>::THREADS, 2 / WtermSmem<N>::NH) k
 // the whole group stay in registers and QG is touched once per group.  FIRST: store, do not accumulate.
 template <int N, bool FIRST>
 __global__ void __launch_bounds__(256) k_zfwd_acc(DevTables tab, const cplx* __restrict__ T, size_t slot_stride,
-                                                  cplx* __restrict__ QGh, int r0, int nr) {
+                                                  cplx* __restrict__ QGh, size_t qstride, int r0, int nr) {
   constexpr int H = N / 2, NPH = N * (H + 1);
   const int par = threadIdx.x >> 7;
   const int pid = blockIdx.x * 128 + (threadIdx.x & 127);
-  if (pid >= NPH) return;
   const int item = blockIdx.y, pair = item % tab.npairs;
+  if (pid >= NPH || tab.full[pair]) return;
   const int kxs = sfreq(pid / (H + 1), N), kys = sfreq(pid % (H + 1), N);
   const int k2xy = kxs * kxs + kys * kys;
   cplx acc[H];
@@ -624,7 +765,7 @@ __global__ void __launch_bounds__(256) k_zfwd_acc(DevTables tab, const cplx* __r
       acc[k].y = fma(b, u[k].y, acc[k].y);
     }
   }
-  cplx* dst = QGh + (size_t)item * (N * NPH) + pid;
+  cplx* dst = QGh + (size_t)item * qstride + pid;
 #pragma unroll
   for (int k = 0; k < H; ++k) {
     cplx* d = dst + (size_t)(2 * k + par) * NPH;
@@ -638,7 +779,7 @@ __global__ void __launch_bounds__(256) k_zfwd_acc(DevTables tab, const cplx* __r
 // out: G2[item][job][lz][cy][cx] (the layout k_z_final reads).
 template <int N>
 __global__ void __launch_bounds__(64) k_final_xy_h(DevTables tab, const cplx* __restrict__ fhat, const cplx* __restrict__ QGh,
-                                                   cplx* __restrict__ G2) {
+                                                   size_t qstride, cplx* __restrict__ G2) {
   constexpr int N2 = N * N, N3 = N2 * N, H = N / 2, NPH = N * (H + 1);
   extern __shared__ cplx sm[];
   const int job = threadIdx.x >> 5, lane = threadIdx.x & 31;
@@ -647,8 +788,9 @@ __global__ void __launch_bounds__(64) k_final_xy_h(DevTables tab, const cplx* __
   const int pair = item % tab.npairs, xl = item / tab.npairs;
   const int q = pair % tab.ns;
   const double inv = 1.0 / ((double)N3);
-  const cplx* qa = QGh + (size_t)item * (N * NPH) + (size_t)lz * NPH;
-  const cplx* qb = QGh + (size_t)item * (N * NPH) + (size_t)((N - lz) % N) * NPH;
+  const bool full = tab.full[pair];              // full-table pairs keep the whole spectrum, [lz][lx][ly]
+  const cplx* qa = QGh + (size_t)item * qstride + (size_t)lz * (full ? N2 : NPH);
+  const cplx* qb = QGh + (size_t)item * qstride + (size_t)((N - lz) % N) * NPH;
   const cplx* in = fhat + ((size_t)xl * tab.ns + q) * N3 + (size_t)lz * N2;
   const cplx* cl = tab.closs + (size_t)pair * N3 + (size_t)lz * N2;
   cplx* o = G2 + ((size_t)item * 2 + job) * N3 + (size_t)lz * N2;
@@ -657,6 +799,7 @@ __global__ void __launch_bounds__(64) k_final_xy_h(DevTables tab, const cplx* __
       [&](int lx, int ly) {
         cplx v;
         if (job == 1) v = cmul(in[lx * N + ly], cl[lx * N + ly]);
+        else if (full) v = qa[lx * N + ly];
         else if (ly <= H) v = qa[lx * (H + 1) + ly];
         else { v = qb[((N - lx) % N) * (H + 1) + (N - ly)]; v.y = -v.y; }
         return make_double2(v.x * inv, v.y * inv);
@@ -668,7 +811,7 @@ __global__ void __launch_bounds__(64) k_final_xy_h(DevTables tab, const cplx* __
 namespace {
 struct PlanV1 {
   int nbx;
-  size_t off_fhat, off_fhh, off_nyqy, off_qg, off_gz, off_nyq, off_s, off_t, total;
+  size_t off_fhat, off_fhh, off_nyqy, off_qg, off_gz, off_nyq, off_s, off_t, off_tf, qstride, total;
 };
 PlanV1 plan_v1(const dgfs_ctx* c, int nx) {
   PlanV1 pl{};
@@ -687,13 +830,17 @@ PlanV1 plan_v1(const dgfs_ctx* c, int nx) {
   pl.off_fhh = take((size_t)nbx * c->ns * (arr / 2));
   pl.off_nyqy = take((size_t)nbx * c->ns * (N * N / 2) * sizeof(cplx));
   const size_t half_arr = N * N * (N / 2 + 1) * sizeof(cplx);
-  pl.off_qg = take(items * half_arr);
+  // QG per item: Hermitian half for VHS pairs, the whole spectrum for pairs with a full b table
+  pl.qstride = (c->any_full ? arr : half_arr) / sizeof(cplx);
+  pl.off_qg = take(items * pl.qstride * sizeof(cplx));
   pl.off_gz = take(gz > g2 ? gz : g2);
   pl.off_nyq = take(items * c->M * nyq_stride * sizeof(cplx));
   pl.off_s = take(items * N3 * sizeof(double));
   // T: forward-transformed planes of a group of radial nodes; also the z-pass scratch of step 1
   const size_t tg = (size_t)c->v1_rgroup * items * half_arr, t1 = (size_t)nbx * c->ns * arr;
   pl.off_t = take(tg > t1 ? tg : t1);
+  // Tf: per-s forward-transformed planes of the full-table pairs
+  pl.off_tf = take(c->any_full ? items * c->M * arr : 0);
   pl.total = off;
   return pl;
 }
@@ -704,7 +851,7 @@ size_t workspace_bytes_v1(const dgfs_ctx* c, int nx) { return plan_v1(c, nx).tot
 // algorithmic FLOPs of the executed algorithm: a 1-D transform of length N counts
 // 5 N log2 N, pointwise work counts the real operations of the formulas in this file's header.
 namespace {
-struct FlopsV1 { double zshift, nyq, xy, wterm, acc, per_r, tail; };
+struct FlopsV1 { double zshift, nyq, xy, wterm, acc, xy_full, acc_full, per_r, per_r_full, tail; };
 FlopsV1 flops_v1(const dgfs_ctx* c) {
   const double N = c->N, N2 = N * N, N3 = N2 * N, H = N / 2, M = c->M;
   const double fft1 = 5.0 * N * log2(N), fft3 = 3.0 * N2 * fft1;
@@ -717,14 +864,19 @@ FlopsV1 flops_v1(const dgfs_ctx* c) {
   f.wterm = M * N3 * 6.0 + N3;                      // 4 adds + 1 fma per (node, s)
   f.acc = N * (H + 1.0) * (fft1 + 4.0 * N);         // forward z pass and QG += w_r b_r . on the Hermitian half
   f.per_r = f.zshift + f.nyq + f.xy + f.wterm + f.acc;
+  // full-table pairs: four passes per plane job, W (10 per element) and the complex product (8), then per s
+  // a forward z pass and the complex multiply-accumulate with b_rs (8 per mode)
+  f.xy_full = M * N * (4.0 * N * fft1 + 32.0 * N2 + 12.0 * N);
+  f.acc_full = M * (N2 * fft1 + 8.0 * N3);
+  f.per_r_full = f.zshift + f.nyq + f.xy_full + f.acc_full;
   f.tail = 2.0 * fft3 + 11.0 * N3 + fft3 / c->ns;
   return f;
 }
 }  // namespace
 
-double flops_per_pair_eval_v1(const dgfs_ctx* c) {
+double flops_per_pair_eval_v1(const dgfs_ctx* c, int pair) {
   const FlopsV1 f = flops_v1(c);
-  return c->N_rho * f.per_r + f.tail;
+  return c->N_rho * (c->full[pair] ? f.per_r_full : f.per_r) + f.tail;
 }
 
 template <int N>
@@ -743,10 +895,16 @@ static int collide_v1_impl(dgfs_ctx* c, const double* f, double* out, int nx, bo
   cplx* nyq = (cplx*)(ws + pl.off_nyq);
   double* S = (double*)(ws + pl.off_s);
   cplx* T = (cplx*)(ws + pl.off_t);
+  cplx* Tf = (cplx*)(ws + pl.off_tf);
+  const size_t qstride = pl.qstride;
+  int nfull = 0;
+  for (int pr = 0; pr < c->npairs; ++pr) nfull += c->full[pr];
+  const int nvhs = c->npairs - nfull;
   const int ns = c->ns, np = c->npairs, nz = c->v1_nz, nz0 = c->v1_nz0;
   const size_t smem_plane = plane_smem_per_warp<N>() * W;
   const size_t smem_final = plane_smem_per_warp<N>() * 2;
   const size_t smem_xy = sizeof(cplx) * (size_t)W * JobSmem<N>::WORDS;
+  const size_t smem_xyf = sizeof(cplx) * (size_t)W * FullSmem<N>::WORDS;
   const size_t smem_wt = sizeof(cplx) * (size_t)WtermSmem<N>::STAGES * WtermSmem<N>::WORDS;
   const size_t smem_nyq = sizeof(cplx) * (size_t)2 * JobSmem<N>::WORDS;
   static bool attr_done = false;
@@ -755,6 +913,7 @@ static int collide_v1_impl(dgfs_ctx* c, const double* f, double* out, int nx, bo
     cudaFuncSetAttribute(k_plane_fwd<N, W, 1>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_plane);
     cudaFuncSetAttribute(k_final_xy_h<N>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_final);
     cudaFuncSetAttribute(k_xy<N, W>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_xy);
+    cudaFuncSetAttribute(k_xy_full<N, W>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_xyf);
     cudaFuncSetAttribute(k_wterm<N>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_wt);
     cudaFuncSetAttribute(k_nyq2<N, 2>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_nyq);
     attr_done = true;
@@ -790,20 +949,29 @@ static int collide_v1_impl(dgfs_ctx* c, const double* f, double* out, int nx, bo
         k_nyq1d<N><<<(items * c->M + 3) / 4, 128, 0, st>>>(c->v1, c->tab, fhat, nyq, r, items * c->M); }
       { ProfScope ps(c->prof, st, "k_nyq2", items * (fl.nyq - c->M * 16.0 * N2));
         k_nyq2<N, 2><<<dim3(3, items), 64, smem_nyq, st>>>(c->v1, c->tab, fhh, nyqy, nyq, r); }
-      { ProfScope ps(c->prof, st, "k_wterm", items * fl.wterm);
-        k_wterm<N><<<dim3(N / WtermSmem<N>::CZB, items), WtermSmem<N>::THREADS, smem_wt, st>>>(nyq, c->M, S); }
-      { ProfScope ps(c->prof, st, "k_xy", items * fl.xy);
-        k_xy<N, W><<<dim3((N + W - 1) / W, items), 32 * W, smem_xy, st>>>(c->v1, c->tab, Gz, nyq, S, T + (size_t)(r % RG) * slot_stride, r); }
-      if ((r + 1) % RG == 0 || r + 1 == c->N_rho) {
-        const int r0 = (r / RG) * RG, nr = r + 1 - r0;
-        ProfScope ps(c->prof, st, "k_zfwd_acc", items * fl.acc * nr);
-        if (r0 == 0) k_zfwd_acc<N, true><<<dim3(hp_blocks, items), 256, 0, st>>>(c->tab, T, slot_stride, QG, r0, nr);
-        else k_zfwd_acc<N, false><<<dim3(hp_blocks, items), 256, 0, st>>>(c->tab, T, slot_stride, QG, r0, nr);
+      if (nvhs > 0) {
+        { ProfScope ps(c->prof, st, "k_wterm", nb * nvhs * fl.wterm);
+          k_wterm<N><<<dim3(N / WtermSmem<N>::CZB, items), WtermSmem<N>::THREADS, smem_wt, st>>>(nyq, c->M, S, c->tab.full, np); }
+        { ProfScope ps(c->prof, st, "k_xy", nb * nvhs * fl.xy);
+          k_xy<N, W><<<dim3((N + W - 1) / W, items), 32 * W, smem_xy, st>>>(c->v1, c->tab, Gz, nyq, S, T + (size_t)(r % RG) * slot_stride, r); }
+        if ((r + 1) % RG == 0 || r + 1 == c->N_rho) {
+          const int r0 = (r / RG) * RG, nr = r + 1 - r0;
+          ProfScope ps(c->prof, st, "k_zfwd_acc", nb * nvhs * fl.acc * nr);
+          if (r0 == 0) k_zfwd_acc<N, true><<<dim3(hp_blocks, items), 256, 0, st>>>(c->tab, T, slot_stride, QG, qstride, r0, nr);
+          else k_zfwd_acc<N, false><<<dim3(hp_blocks, items), 256, 0, st>>>(c->tab, T, slot_stride, QG, qstride, r0, nr);
+        }
+      }
+      if (nfull > 0) {
+        { ProfScope ps(c->prof, st, "k_xy_full", nb * nfull * fl.xy_full);
+          k_xy_full<N, W><<<dim3((N + W - 1) / W, items), 32 * W, smem_xyf, st>>>(c->v1, c->tab, Gz, nyq, Tf, r); }
+        { ProfScope ps(c->prof, st, "k_zfwd_full", nb * nfull * fl.acc_full);
+          if (r == 0) k_zfwd_full<N, true><<<dim3(pen_blocks, items), 256, 0, st>>>(c->tab, Tf, QG, qstride, r);
+          else k_zfwd_full<N, false><<<dim3(pen_blocks, items), 256, 0, st>>>(c->tab, Tf, QG, qstride, r); }
       }
     }
     // step 10
     { ProfScope ps(c->prof, st, "k_final_xy", items * (2.0 * fft3 * 2.0 / 3.0 + 6.0 * N3));
-      k_final_xy_h<N><<<dim3(N, items), 64, smem_final, st>>>(c->tab, fhat, QG, Gz); }
+      k_final_xy_h<N><<<dim3(N, items), 64, smem_final, st>>>(c->tab, fhat, QG, qstride, Gz); }
     { ProfScope ps(c->prof, st, "k_z_final", items * (2.0 * fft3 / 3.0 + 5.0 * N3));
       if (pairs_out)
         k_z_final<N, false><<<dim3(pen_blocks, items), 128, 0, st>>>(c->tab, Gz, fc, out + (size_t)x0 * np * N3);

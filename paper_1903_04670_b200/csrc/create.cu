@@ -470,10 +470,10 @@ extern "C" int dgfs_create(const dgfs_params* P, dgfs_ctx** out) {
   c->scratch_budget = (size_t)(env ? atol(env) : 3072) << 20;
   int rc = build_tables(c);
   if (rc != DGFS_OK) { g_create_error = c->err; dgfs_destroy(c); return rc; }
-  // pipeline choice: v1 (collide_v1.cu) needs b independent of s for every pair and one lane per pencil;
-  // DGFS_PIPELINE=v0 forces the stage-per-kernel pipeline (used by the parity tests to cover both)
+  // pipeline choice: v1 (collide_v1.cu) needs one lane per pencil (N <= 32); DGFS_PIPELINE=v0 forces the
+  // stage-per-kernel pipeline (N = 48 always runs it; the parity tests cover both)
   const char* pipe = getenv("DGFS_PIPELINE");
-  c->use_v1 = !c->any_full && N <= 32 && !(pipe && std::string(pipe) == "v0");
+  c->use_v1 = N <= 32 && !(pipe && std::string(pipe) == "v0");
   if (c->use_v1) {
     const char* ch = getenv("DGFS_V1_CHUNK");
     if (ch && atoi(ch) > 0) c->v1_chunk = atoi(ch);

@@ -99,7 +99,7 @@ struct dgfs_ctx {
   double* d_sigma = nullptr;
   unsigned char* d_full = nullptr;
   dgfs::DevTables tab{};
-  // v1 pipeline (collide_v1.cu): tables built by build_tables_v1, used when no pair needs the full b table
+  // v1 pipeline (collide_v1.cu): tables built by build_tables_v1, used for N <= 32
   bool use_v1 = false;
   int v1_chunk = 512;                    // spatial points per launch group (large launches amortise the tails)
   int v1_rgroup = 16;                    // radial nodes per forward-z / QG accumulation launch
@@ -145,6 +145,6 @@ int build_tables_v1(dgfs_ctx* c);
 void free_tables_v1(dgfs_ctx* c);
 size_t workspace_bytes_v1(const dgfs_ctx* c, int nx);
 int run_collide_v1(dgfs_ctx* c, const double* f, double* out, int nx, bool pairs_out, cudaStream_t st);
-double flops_per_pair_eval_v1(const dgfs_ctx* c);
+double flops_per_pair_eval_v1(const dgfs_ctx* c, int pair);
 
 }  // namespace dgfs

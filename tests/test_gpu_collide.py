@@ -96,6 +96,31 @@ def test_v1_nyquist_terms(torch_cuda, N, N_rho, M, ns, noise):
     _small_radial_rule(torch_cuda, N, N_rho, M, ns, (1.0,) * ns, noise=noise)
 
 
+def test_table_mode_1_collide(torch_cuda):
+    """Algorithm 1 taken literally (pre-computation sphere): every pair then has a full b table, also
+    the VHS ones, and runs the per-s forward transforms of the v1 pipeline."""
+    torch = torch_cuda
+    from oracle.collide import collide_pairs
+    from oracle.quadrature import sphere_rule
+    sp, wp = sphere_rule(12)
+    cfg = _rand_cfg("t", 2, 16, 3, 6, (1.0, 1.3), (0.6, 0.8), (1.0, 2.0), seed=31)
+    rng = np.random.default_rng(31)
+    f = make_points(cfg, range(cfg.nx)) * (1.0 + 0.2 * rng.uniform(-1, 1, (cfg.nx, 2, 16 ** 3)))
+    kw = dict(table_mode=1, sigma_pre=sp, w_pre=wp)
+    Qo = collide_pairs(_oracle_tables(cfg, **kw), f)
+    with _gpu_op(cfg, **kw) as op:
+        Qg = op.collide_pairs(torch.from_numpy(f).cuda()).cpu().numpy()
+    assert _pair_errs(Qg, Qo).max() < TOL
+
+
+@pytest.mark.parametrize("N,alpha", [(8, (1.0, 1.2, 1.4)), (16, (1.3, 1.0))])
+def test_v0_pipeline_on_vss_pairs(torch_cuda, monkeypatch, N, alpha):
+    """VSS pairs default to the v1 pipeline for N <= 32; DGFS_PIPELINE=v0 keeps the stage-per-kernel one
+    (which N = 48 always uses) covered on the same inputs."""
+    monkeypatch.setenv("DGFS_PIPELINE", "v0")
+    _small_radial_rule(torch_cuda, N, 3, 12, len(alpha), alpha)
+
+
 def test_v1_user_sphere_rule_without_symmetry(torch_cuda):
     """A caller-supplied sigma set with no shared sigma_z values (every z shift is its own job)."""
     torch = torch_cuda
