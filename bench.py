@@ -87,12 +87,13 @@ class ClockSampler(threading.Thread):
 
 
 def oracle_sample(cfg, n_points):
-    """Time the oracle, as it stands, on the first n_points points of the workload (all pairs).
-    Returns (pair_evals, seconds, cores)."""
+    """Time the oracle, as it stands, on n_points points of the workload (all pairs), taken alternately from
+    the start and from the middle of the batch (both halves of the c2 mix).  Returns (pair_evals, seconds, cores)."""
     from workloads import make_points
     from oracle.tables import precompute
     from oracle.collide import collide_pairs
-    f = make_points(cfg, range(n_points))
+    xs = [(i // 2) + (cfg.nx // 2 if i % 2 else 0) for i in range(n_points)]
+    f = make_points(cfg, xs)
     tab = precompute(cfg.N, cfg.N_rho, cfg.M, cfg.L, cfg.mass, cfg.omega, cfg.alpha)   # create: untimed
     t0 = time.perf_counter()
     collide_pairs(tab, f)
@@ -104,7 +105,7 @@ def run_reference(args, cfg, rank):
     """--impl reference: the CPU oracle on the host cores (kind = oracle)."""
     if rank != 0:
         return
-    sample_pts = 1
+    sample_pts = 2
     times = []
     evals = 0
     for i in range(args.warmup + args.steps):
@@ -263,10 +264,11 @@ def main():
         }
         cpu = None
         if world == 1 and not args.no_cpu_baseline:
-            ev_n, dt, cores = oracle_sample(cfg, 1)
+            npts = 4
+            ev_n, dt, cores = oracle_sample(cfg, npts)
             cpu = {"value": ev_n / dt, "unit": UNIT, "cores": cores, "kind": "oracle",
-                   "sample": "first point of %s, all %d pairs, %.1f s (oracle collide_pairs, numpy, tables untimed)" % (
-                       cfg.name, cfg.ns * cfg.ns, dt)}
+                   "sample": "%d points of %s (two from each half of the batch), all %d pairs, %.1f s (oracle "
+                             "collide_pairs, numpy, one thread, tables untimed)" % (npts, cfg.name, cfg.ns * cfg.ns, dt)}
         out = {
             "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
             "warmup": args.warmup, "ms_per_step": ms_per_step, "higher_is_better": True, "scaling": "weak",

@@ -261,6 +261,23 @@ def test_v1_batch_consistency_and_chunking(torch_cuda, monkeypatch):
         assert torch.equal(op.collide(f), Qs)
 
 
+def test_v1_mixed_pairs_batch_consistency_and_chunking(torch_cuda, monkeypatch):
+    """3 species, pair (0,0) VHS and the other eight VSS in one context: the two kinds share the z shifts and
+    the Nyquist fields and take different kernels afterwards; chunking must not change a bit."""
+    torch = torch_cuda
+    cfg = _rand_cfg("t", 3, 8, 3, 12, (1.0, 1.2, 1.4), (0.5, 0.7, 0.8), (1.0, 1.5, 2.0), seed=12)
+    f = torch.from_numpy(make_points(cfg, range(7))).cuda()
+    with _gpu_op(cfg) as op:
+        Qb = op.collide_pairs(f).clone()
+        Qs = op.collide(f).clone()
+        Q1 = op.collide_pairs(f[5:6].contiguous())
+        assert torch.equal(Q1[0], Qb[5])
+    monkeypatch.setenv("DGFS_V1_CHUNK", "3")
+    with _gpu_op(cfg) as op:
+        assert torch.equal(op.collide_pairs(f), Qb)
+        assert torch.equal(op.collide(f), Qs)
+
+
 def test_output_on_side_stream_and_repeatability(torch_cuda):
     torch = torch_cuda
     cfg = get_config("c0")
