@@ -101,7 +101,14 @@ int build_tables_v1(dgfs_ctx* c) {
       }
     }
   }
+  // sphere points with a vanishing component (every point of the octahedron and of the icosahedron has one):
+  // sin(0) = 0, so that axis contributes no anti-Hermitian part at all
+  c->v1_smask.assign(M, 0);
+  for (int s2 = 0; s2 < M; ++s2)
+    for (int d = 0; d < 3; ++d)
+      if (c->sigma[3 * s2 + d] == 0.0) c->v1_smask[s2] |= (unsigned char)(1 << d);
   int rc;
+  if ((rc = upload(c, &c->d_v1_smask, c->v1_smask, "upload sphere masks"))) return rc;
   if ((rc = upload(c, &c->d_v1_zsp, c->v1_zsp, "upload z-job species"))) return rc;
   if ((rc = upload(c, &c->d_v1_zmap, c->v1_zmap, "upload z-job map"))) return rc;
   if ((rc = upload(c, &c->d_v1_hz, hz, "upload z factors"))) return rc;
@@ -110,13 +117,13 @@ int build_tables_v1(dgfs_ctx* c) {
   if ((rc = upload(c, &c->d_v1_sxy, sxy, "upload x,y scalars"))) return rc;
   V1Tables& t = c->v1;
   t.nz = nz; t.zsp = c->d_v1_zsp; t.zmap = c->d_v1_zmap; t.hz = c->d_v1_hz; t.szv = c->d_v1_szv;
-  t.hxy = c->d_v1_hxy; t.sxy = c->d_v1_sxy;
+  t.hxy = c->d_v1_hxy; t.sxy = c->d_v1_sxy; t.smask = c->d_v1_smask;
   return DGFS_OK;
 }
 
 void free_tables_v1(dgfs_ctx* c) {
   cudaFree(c->d_v1_zsp); cudaFree(c->d_v1_zmap); cudaFree(c->d_v1_hz); cudaFree(c->d_v1_szv);
-  cudaFree(c->d_v1_hxy); cudaFree(c->d_v1_sxy);
+  cudaFree(c->d_v1_hxy); cudaFree(c->d_v1_sxy); cudaFree(c->d_v1_smask);
 }
 
 // ---------------------------------------------------------------- device code -------------------
@@ -355,10 +362,26 @@ __global__ void __launch_bounds__(32 * NW) k_nyq2(V1Tables t, DevTables tab, con
     if (which == 0) return t.szv[(size_t)r * t.nz + zm[2 * s + side]];
     return sbase[s * 4 + side * 2 + (which == 1 ? 0 : 1)];
   };
-  if (warp >= tab.M) return;
-  issue(warp);
-  double scale = scale_of(warp);
-  for (int s = warp; s < tab.M; s += NW) {
+  // fields of an axis with sigma_{s,d} = 0 vanish identically (v1_tables.h): write zeros, run no job
+  const int zbit = (which == 0) ? 4 : (which == 1 ? 1 : 2);
+  const int ooff = (which == 0) ? NL::UZ : (which == 1 ? NL::UXP : NL::UY);
+  auto next_job = [&](int s) {                   // first s' >= s in this warp's sequence with a job to run
+    while (s < tab.M && (t.smask[s] & zbit)) {
+      if (act) {
+        cplx* out = nyq + ((size_t)item * tab.M + s) * NL::STRIDE + ooff;
+#pragma unroll
+        for (int j = 0; j < N; ++j) out[j * N + ln] = make_double2(0.0, 0.0);
+      }
+      s += NW;
+    }
+    return s;
+  };
+  int s = next_job(warp);
+  if (s >= tab.M) return;
+  issue(s);
+  double scale = scale_of(s);
+  while (s < tab.M) {
+    const int sn = next_job(s + NW);
     cp_async_wait_all();
     __syncwarp();
     cplx X[N];
@@ -367,7 +390,8 @@ __global__ void __launch_bounds__(32 * NW) k_nyq2(V1Tables t, DevTables tab, con
     cplx vt = make_double2(0.0, 0.0);
     if (act) { job_pass2_in<N, false>(buf, ln, 0.0, 0.0, X); vt = buf[JS::VZP]; }
     __syncwarp();
-    if (s + NW < tab.M) { issue(s + NW); scale = scale_of(s + NW); }
+    const double scale_next = (sn < tab.M) ? scale_of(sn) : 0.0;
+    if (sn < tab.M) issue(sn);
     if (act) {
       fft_reg<N, +1>(X);
       cplx* out = nyq + ((size_t)item * tab.M + s) * NL::STRIDE;
@@ -386,6 +410,7 @@ __global__ void __launch_bounds__(32 * NW) k_nyq2(V1Tables t, DevTables tab, con
         for (int j = 0; j < N; ++j) out[NL::UY + j * N + ln] = X[j];
       }
     }
+    s = sn; scale = scale_next;
   }
 }
 
@@ -645,8 +670,47 @@ struct WtermSmem {
   static constexpr int COPIES = N * N + 2 * CZB * N;   // elements staged per s
   static constexpr int STAGES = 5;                     // ring depth: enough bytes in flight to cover the HBM latency
 };
+// Arithmetic of one s for the thread's 2 x 2 x 8 nodes.  MASK bit d set: the field of axis d (ux', uy, uz) is
+// identically zero for this sphere point (V1Tables::smask) and is neither staged nor read.
+template <int N, int MASK>
+__device__ __forceinline__ void wterm_planes(const cplx* __restrict__ b_, int half, int tx, int ty, double (&acc)[8][2][2]) {
+  typedef WtermSmem<N> WS;
+  constexpr int H = N / 2, CZG = WS::CZG;
+  constexpr bool HU = !(MASK & 1), HV = !(MASK & 2), HZ = !(MASK & 4);
+  const cplx zero = make_double2(0.0, 0.0);
+  cplx z[2][2];
+#pragma unroll
+  for (int b = 0; b < 2; ++b)
+#pragma unroll
+    for (int a = 0; a < 2; ++a) z[b][a] = HZ ? b_[WS::Z + ((2 * ty + b) * 2 + a) * H + tx] : zero;
+  // software pipeline over the planes: the loads of plane i + 1 are in flight during the arithmetic of plane i
+  const cplx* ub = b_ + WS::U + (half * CZG) * WS::RS + 2 * ty;
+  const cplx* vb = b_ + WS::V + (half * CZG) * WS::RS + tx;
+  cplx un[2] = {HU ? ub[0] : zero, HU ? ub[1] : zero}, vn[2] = {HV ? vb[0] : zero, HV ? vb[H] : zero};
+#pragma unroll
+  for (int i = 0; i < CZG; ++i) {
+    const cplx u[2] = {un[0], un[1]}, v[2] = {vn[0], vn[1]};
+    if (i + 1 < CZG) {
+      if (HU) { un[0] = ub[(i + 1) * WS::RS]; un[1] = ub[(i + 1) * WS::RS + 1]; }
+      if (HV) { vn[0] = vb[(i + 1) * WS::RS]; vn[1] = vb[(i + 1) * WS::RS + H]; }
+    }
+#pragma unroll
+    for (int b = 0; b < 2; ++b)
+#pragma unroll
+      for (int a = 0; a < 2; ++a) {
+        // signs: the tile starts at even cx, cy; plane groups start at even cz
+        double wx = 0.0, wy = 0.0;
+        if (HU) { wx = a ? -u[b].x : u[b].x; wy = a ? -u[b].y : u[b].y; }
+        if (HV) { wx += b ? -v[a].x : v[a].x; wy += b ? -v[a].y : v[a].y; }
+        if (HZ) { wx += (i & 1) ? -z[b][a].x : z[b][a].x; wy += (i & 1) ? -z[b][a].y : z[b][a].y; }
+        acc[i][b][a] = fma(wx, wy, acc[i][b][a]);
+      }
+  }
+}
+
 template <int N>
-__global__ void __launch_bounds__(WtermSmem<N>::THREADS, 2 / WtermSmem<N>::NH) k_wterm(const cplx* __restrict__ nyq, int M, double* __restrict__ S, const unsigned char* __restrict__ full, int npairs) {
+__global__ void __launch_bounds__(WtermSmem<N>::THREADS, 2 / WtermSmem<N>::NH) k_wterm(const cplx* __restrict__ nyq, int M, double* __restrict__ S, const unsigned char* __restrict__ full, int npairs,
+        const unsigned char* __restrict__ smask) {
   constexpr int H = N / 2, N2 = N * N, N3 = N2 * N;
   typedef NyqLayout<N> NL;
   typedef WtermSmem<N> WS;
@@ -661,16 +725,17 @@ __global__ void __launch_bounds__(WtermSmem<N>::THREADS, 2 / WtermSmem<N>::NH) k
   auto issue = [&](int s) {
     cplx* dst = sm + (size_t)(s % NS) * WS::WORDS;
     const cplx* nq = nbase + (size_t)s * NL::STRIDE;
+    const int mask = smask[s];                       // vanishing fields are not staged
     for (int e = threadIdx.x; e < WS::COPIES; e += NT) {
       if (e < N2) {
         const int cy = e / N, cx = e % N;
-        cp_async16(&dst[WS::Z + (cy * 2 + (cx & 1)) * H + (cx >> 1)], nq + NL::UZ + e);
+        if (!(mask & 4)) cp_async16(&dst[WS::Z + (cy * 2 + (cx & 1)) * H + (cx >> 1)], nq + NL::UZ + e);
       } else if (e < N2 + CZB * N) {
         const int cx = (e - N2) / CZB, i = (e - N2) % CZB;
-        cp_async16(&dst[WS::V + i * WS::RS + (cx & 1) * H + (cx >> 1)], nq + NL::UY + cx * N + cz0 + i);
+        if (!(mask & 2)) cp_async16(&dst[WS::V + i * WS::RS + (cx & 1) * H + (cx >> 1)], nq + NL::UY + cx * N + cz0 + i);
       } else {
         const int cy = (e - N2 - CZB * N) / CZB, i = (e - N2 - CZB * N) % CZB;
-        cp_async16(&dst[WS::U + i * WS::RS + cy], nq + NL::UXP + cy * N + cz0 + i);
+        if (!(mask & 1)) cp_async16(&dst[WS::U + i * WS::RS + cy], nq + NL::UXP + cy * N + cz0 + i);
       }
     }
     cp_async_commit();
@@ -688,32 +753,15 @@ __global__ void __launch_bounds__(WtermSmem<N>::THREADS, 2 / WtermSmem<N>::NH) k
     if (s + NS - 1 < M) issue(s + NS - 1); else cp_async_commit();
     if (!act) continue;
     const cplx* b_ = sm + (size_t)(s % NS) * WS::WORDS;
-    cplx z[2][2];
-#pragma unroll
-    for (int b = 0; b < 2; ++b)
-#pragma unroll
-      for (int a = 0; a < 2; ++a) z[b][a] = b_[WS::Z + ((2 * ty + b) * 2 + a) * H + tx];
-    // software pipeline over the planes: the loads of plane i + 1 are in flight during the arithmetic of plane i
-    const cplx* ub = b_ + WS::U + (half * CZG) * WS::RS + 2 * ty;
-    const cplx* vb = b_ + WS::V + (half * CZG) * WS::RS + tx;
-    cplx un[2] = {ub[0], ub[1]}, vn[2] = {vb[0], vb[H]};
-#pragma unroll
-    for (int i = 0; i < CZG; ++i) {
-      const cplx u[2] = {un[0], un[1]}, v[2] = {vn[0], vn[1]};
-      if (i + 1 < CZG) {
-        un[0] = ub[(i + 1) * WS::RS]; un[1] = ub[(i + 1) * WS::RS + 1];
-        vn[0] = vb[(i + 1) * WS::RS]; vn[1] = vb[(i + 1) * WS::RS + H];
-      }
-#pragma unroll
-      for (int b = 0; b < 2; ++b)
-#pragma unroll
-        for (int a = 0; a < 2; ++a) {
-          // signs: the tile starts at even cx, cy; plane groups start at even cz
-          const double ux_ = a ? -u[b].x : u[b].x, uy_ = a ? -u[b].y : u[b].y;
-          const double vx_ = b ? -v[a].x : v[a].x, vy_ = b ? -v[a].y : v[a].y;
-          const double zx_ = (i & 1) ? -z[b][a].x : z[b][a].x, zy_ = (i & 1) ? -z[b][a].y : z[b][a].y;
-          acc[i][b][a] = fma(ux_ + vx_ + zx_, uy_ + vy_ + zy_, acc[i][b][a]);
-        }
+    switch (smask[s]) {                              // uniform over the block
+      case 0: wterm_planes<N, 0>(b_, half, tx, ty, acc); break;
+      case 1: wterm_planes<N, 1>(b_, half, tx, ty, acc); break;
+      case 2: wterm_planes<N, 2>(b_, half, tx, ty, acc); break;
+      case 3: wterm_planes<N, 3>(b_, half, tx, ty, acc); break;
+      case 4: wterm_planes<N, 4>(b_, half, tx, ty, acc); break;
+      case 5: wterm_planes<N, 5>(b_, half, tx, ty, acc); break;
+      case 6: wterm_planes<N, 6>(b_, half, tx, ty, acc); break;
+      default: break;                                // all three fields vanish
     }
   }
   if (!act) return;
@@ -857,11 +905,18 @@ FlopsV1 flops_v1(const dgfs_ctx* c) {
   const double fft1 = 5.0 * N * log2(N), fft3 = 3.0 * N2 * fft1;
   FlopsV1 f{};
   f.zshift = (double)(c->v1_nz - c->v1_nz0) / c->npairs * N * H * (fft1 + 6.0 * N);   // per item and radial node
-  f.nyq = M * (3.0 * (2.0 * N * fft1 + 14.0 * N2) + 16.0 * N2);   // three plane jobs + the 1-D sums
+  // plane jobs and product terms actually run: fields of an axis with sigma_{s,d} = 0 vanish and are skipped
+  double njobs = 0.0, wops = 0.0;
+  for (int s2 = 0; s2 < c->M; ++s2) {
+    const int nt = 3 - ((c->v1_smask[s2] & 1) + ((c->v1_smask[s2] >> 1) & 1) + ((c->v1_smask[s2] >> 2) & 1));
+    njobs += nt;
+    wops += nt > 0 ? 2.0 * (nt - 1) + 2.0 : 0.0;     // adds forming Re W, Im W, one fma
+  }
+  f.nyq = njobs * (2.0 * N * fft1 + 14.0 * N2) + M * 16.0 * N2;   // the plane jobs + the 1-D sums
   // per plane job: two passes of N transforms, x and y factors (6 + 6 per element), packing adds (2), product
   // fma (2), Nyquist row / column fixes (12 N); per plane: forward y pass on real rows (half) and x pass on H+1 columns
   f.xy = M * N * (2.0 * N * fft1 + 16.0 * N2 + 12.0 * N) + N * (N + 1.0) * fft1;
-  f.wterm = M * N3 * 6.0 + N3;                      // 4 adds + 1 fma per (node, s)
+  f.wterm = wops * N3 + N3;
   f.acc = N * (H + 1.0) * (fft1 + 4.0 * N);         // forward z pass and QG += w_r b_r . on the Hermitian half
   f.per_r = f.zshift + f.nyq + f.xy + f.wterm + f.acc;
   // full-table pairs: four passes per plane job, W (10 per element) and the complex product (8), then per s
@@ -951,7 +1006,7 @@ static int collide_v1_impl(dgfs_ctx* c, const double* f, double* out, int nx, bo
         k_nyq2<N, 2><<<dim3(3, items), 64, smem_nyq, st>>>(c->v1, c->tab, fhh, nyqy, nyq, r); }
       if (nvhs > 0) {
         { ProfScope ps(c->prof, st, "k_wterm", nb * nvhs * fl.wterm);
-          k_wterm<N><<<dim3(N / WtermSmem<N>::CZB, items), WtermSmem<N>::THREADS, smem_wt, st>>>(nyq, c->M, S, c->tab.full, np); }
+          k_wterm<N><<<dim3(N / WtermSmem<N>::CZB, items), WtermSmem<N>::THREADS, smem_wt, st>>>(nyq, c->M, S, c->tab.full, np, c->v1.smask); }
         { ProfScope ps(c->prof, st, "k_xy", nb * nvhs * fl.xy);
           k_xy<N, W><<<dim3((N + W - 1) / W, items), 32 * W, smem_xy, st>>>(c->v1, c->tab, Gz, nyq, S, T + (size_t)(r % RG) * slot_stride, r); }
         if ((r + 1) % RG == 0 || r + 1 == c->N_rho) {
