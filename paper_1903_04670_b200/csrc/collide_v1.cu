@@ -262,12 +262,20 @@ __global__ void __launch_bounds__(128) k_nyq1d(V1Tables t, DevTables tab, const 
 // Pass 1 of a plane job (lane = (side, m), column m of the Hermitian half): multiply by the factor along
 // the pass-1 index, inverse transform in registers, factor of the lane's own column, back into the tile.
 template <int N, bool CORR>
-__device__ __forceinline__ void job_pass1(cplx* buf, int ln, int side, int m, double szs, double scale) {
+__device__ __forceinline__ void job_pass1(cplx* buf, int ln, int side, int m, double szs, double scale,
+                                          bool unit_i = false, bool real_m = false) {
   typedef JobSmem<N> JS;
   constexpr int H = N / 2, P = JS::P;
   cplx v[N];
+  if (unit_i) {
+    // theta = 0 along the pass-1 axis: the factor is the same real number for every index; the caller has
+    // folded it into `scale` (warp-uniform branch)
 #pragma unroll
-  for (int i = 0; i < N; ++i) v[i] = cmul(buf[i * P + ln], buf[JS::HI + side * N + i]);
+    for (int i = 0; i < N; ++i) v[i] = buf[i * P + ln];
+  } else {
+#pragma unroll
+    for (int i = 0; i < N; ++i) v[i] = cmul(buf[i * P + ln], buf[JS::HI + side * N + i]);
+  }
   if (CORR) {
     const cplx c1 = buf[JS::VYH + ln];
     v[H].x = fma(-szs, c1.x, v[H].x);
@@ -280,9 +288,15 @@ __device__ __forceinline__ void job_pass1(cplx* buf, int ln, int side, int m, do
   const double hyH = buf[JS::HM + side * N + H].x;
   const double ya = scale * hy0.x, yb = (m == 0) ? 0.0 : -scale * hy0.y, yc = (m == 0) ? 0.0 : scale * hy0.y,
                yd = (m == 0) ? scale * hyH : scale * hy0.x;
+  if (real_m) {
+    // theta = 0 along the pass-2 axis: every h[m] is the same real number (yb = yc = 0)
 #pragma unroll
-  for (int i = 0; i < N; ++i)
-    buf[i * P + ln] = make_double2(fma(v[i].x, ya, v[i].y * yb), fma(v[i].x, yc, v[i].y * yd));
+    for (int i = 0; i < N; ++i) buf[i * P + ln] = make_double2(v[i].x * ya, v[i].y * yd);
+  } else {
+#pragma unroll
+    for (int i = 0; i < N; ++i)
+      buf[i * P + ln] = make_double2(fma(v[i].x, ya, v[i].y * yb), fma(v[i].x, yc, v[i].y * yd));
+  }
 }
 
 // Input of pass 2 (lane = pass-1 output index): the N packed columns X = Y_A + i Y_B, the mirror half by
@@ -476,7 +490,12 @@ __global__ void __launch_bounds__(32 * W) k_xy(V1Tables t, DevTables tab, const 
     cp_async_wait_all();
     __syncwarp();
     cplx X[N];
-    if (act) job_pass1<N, true>(buf, ln, side, m, szs, 1.0);
+    if (act) {
+      // sigma_x = 0: h_x is the constant w_s / N (side A) or 1 / N; sigma_y = 0: h_y is the constant 1 / N
+      const int mk = t.smask[s];
+      const bool ux_ = (mk & 1) != 0, ry_ = (mk & 2) != 0;
+      job_pass1<N, true>(buf, ln, side, m, szs, ux_ ? buf[JS::HI + side * N].x : 1.0, ux_, ry_);
+    }
     __syncwarp();
     if (act) job_pass2_in<N, true>(buf, ln, szs, sxb, X);
     __syncwarp();
@@ -574,7 +593,12 @@ __global__ void __launch_bounds__(32 * W) k_xy_full(V1Tables t, DevTables tab, c
     cp_async_wait_all();
     __syncwarp();
     cplx X[N];
-    if (act) job_pass1<N, true>(buf, ln, side, m, szs, 1.0);
+    if (act) {
+      // sigma_x = 0: h_x is the constant w_s / N (side A) or 1 / N; sigma_y = 0: h_y is the constant 1 / N
+      const int mk = t.smask[s];
+      const bool ux_ = (mk & 1) != 0, ry_ = (mk & 2) != 0;
+      job_pass1<N, true>(buf, ln, side, m, szs, ux_ ? buf[JS::HI + side * N].x : 1.0, ux_, ry_);
+    }
     __syncwarp();
     if (act) {
       job_pass2_in<N, true>(buf, ln, szs, sxb, X);
@@ -913,15 +937,19 @@ FlopsV1 flops_v1(const dgfs_ctx* c) {
     wops += nt > 0 ? 2.0 * (nt - 1) + 2.0 : 0.0;     // adds forming Re W, Im W, one fma
   }
   f.nyq = njobs * (2.0 * N * fft1 + 14.0 * N2) + M * 16.0 * N2;   // the plane jobs + the 1-D sums
-  // per plane job: two passes of N transforms, x and y factors (6 + 6 per element), packing adds (2), product
+  // per plane job: two passes of N transforms, x and y factors (6 + 6 per element; none / 2 where sigma_x / sigma_y
+  // vanishes), packing adds (2), product
   // fma (2), Nyquist row / column fixes (12 N); per plane: forward y pass on real rows (half) and x pass on H+1 columns
-  f.xy = M * N * (2.0 * N * fft1 + 16.0 * N2 + 12.0 * N) + N * (N + 1.0) * fft1;
+  double fac = 0.0;                                    // x and y factor work per element, summed over s
+  for (int s2 = 0; s2 < c->M; ++s2)
+    fac += ((c->v1_smask[s2] & 1) ? 0.0 : 6.0) + ((c->v1_smask[s2] & 2) ? 2.0 : 6.0);
+  f.xy = N * (M * (2.0 * N * fft1 + 4.0 * N2 + 12.0 * N) + fac * N2) + N * (N + 1.0) * fft1;
   f.wterm = wops * N3 + N3;
   f.acc = N * (H + 1.0) * (fft1 + 4.0 * N);         // forward z pass and QG += w_r b_r . on the Hermitian half
   f.per_r = f.zshift + f.nyq + f.xy + f.wterm + f.acc;
   // full-table pairs: four passes per plane job, W (10 per element) and the complex product (8), then per s
   // a forward z pass and the complex multiply-accumulate with b_rs (8 per mode)
-  f.xy_full = M * N * (4.0 * N * fft1 + 32.0 * N2 + 12.0 * N);
+  f.xy_full = N * (M * (4.0 * N * fft1 + 20.0 * N2 + 12.0 * N) + fac * N2);
   f.acc_full = M * (N2 * fft1 + 8.0 * N3);
   f.per_r_full = f.zshift + f.nyq + f.xy_full + f.acc_full;
   f.tail = 2.0 * fft3 + 11.0 * N3 + fft3 / c->ns;
