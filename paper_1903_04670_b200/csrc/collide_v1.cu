@@ -101,6 +101,36 @@ int build_tables_v1(dgfs_ctx* c) {
       }
     }
   }
+  // R-10, same-species VHS pairs: mu_q = mu_p = 1/2 and f_p = f_q, so the antipode s' of a sphere point s swaps
+  // the two shifted fields, A_s' = B_s and B_s' = A_s, and A_s' B_s' = A_s B_s exactly.  Only one point of every
+  // antipodal couple is run, with weight w_s + w_s' (the weight sits in the side-A x factors).  The paper's
+  // "M points on the half sphere" is this symmetry; it does not hold for p != q (reading S-1).
+  c->v1_sskip.assign((size_t)np * M, 0);
+  {
+    const char* ap = getenv("DGFS_V1_ANTIPODAL");
+    const bool on = !(ap && atoi(ap) == 0);
+    for (int p = 0; on && p < ns; ++p) {
+      const int pair = p * ns + p;
+      if (c->full[pair]) continue;
+      for (int s2 = 0; s2 < M; ++s2) {
+        if (c->v1_sskip[(size_t)pair * M + s2]) continue;
+        for (int s3 = s2 + 1; s3 < M; ++s3) {
+          if (c->v1_sskip[(size_t)pair * M + s3]) continue;
+          if (c->sigma[3 * s3] == -c->sigma[3 * s2] && c->sigma[3 * s3 + 1] == -c->sigma[3 * s2 + 1] &&
+              c->sigma[3 * s3 + 2] == -c->sigma[3 * s2 + 2]) {
+            c->v1_sskip[(size_t)pair * M + s3] = 1;
+            const double fac = (c->w_sigma[s2] + c->w_sigma[s3]) / c->w_sigma[s2];
+            for (int r = 0; r < Nr; ++r) {
+              const size_t e = (((size_t)pair * Nr + r) * M + s2) * 2;        // side A
+              for (int j = 0; j < N; ++j) { hxy[e * 2 * N + j].x *= fac; hxy[e * 2 * N + j].y *= fac; }
+              sxy[e * 2] *= fac;
+            }
+            break;
+          }
+        }
+      }
+    }
+  }
   // sphere points with a vanishing component (every point of the octahedron and of the icosahedron has one):
   // sin(0) = 0, so that axis contributes no anti-Hermitian part at all
   c->v1_smask.assign(M, 0);
@@ -109,6 +139,7 @@ int build_tables_v1(dgfs_ctx* c) {
       if (c->sigma[3 * s2 + d] == 0.0) c->v1_smask[s2] |= (unsigned char)(1 << d);
   int rc;
   if ((rc = upload(c, &c->d_v1_smask, c->v1_smask, "upload sphere masks"))) return rc;
+  if ((rc = upload(c, &c->d_v1_sskip, c->v1_sskip, "upload antipode masks"))) return rc;
   if ((rc = upload(c, &c->d_v1_zsp, c->v1_zsp, "upload z-job species"))) return rc;
   if ((rc = upload(c, &c->d_v1_zmap, c->v1_zmap, "upload z-job map"))) return rc;
   if ((rc = upload(c, &c->d_v1_hz, hz, "upload z factors"))) return rc;
@@ -117,13 +148,13 @@ int build_tables_v1(dgfs_ctx* c) {
   if ((rc = upload(c, &c->d_v1_sxy, sxy, "upload x,y scalars"))) return rc;
   V1Tables& t = c->v1;
   t.nz = nz; t.zsp = c->d_v1_zsp; t.zmap = c->d_v1_zmap; t.hz = c->d_v1_hz; t.szv = c->d_v1_szv;
-  t.hxy = c->d_v1_hxy; t.sxy = c->d_v1_sxy; t.smask = c->d_v1_smask;
+  t.hxy = c->d_v1_hxy; t.sxy = c->d_v1_sxy; t.smask = c->d_v1_smask; t.sskip = c->d_v1_sskip;
   return DGFS_OK;
 }
 
 void free_tables_v1(dgfs_ctx* c) {
   cudaFree(c->d_v1_zsp); cudaFree(c->d_v1_zmap); cudaFree(c->d_v1_hz); cudaFree(c->d_v1_szv);
-  cudaFree(c->d_v1_hxy); cudaFree(c->d_v1_sxy); cudaFree(c->d_v1_smask);
+  cudaFree(c->d_v1_hxy); cudaFree(c->d_v1_sxy); cudaFree(c->d_v1_smask); cudaFree(c->d_v1_sskip);
 }
 
 // ---------------------------------------------------------------- device code -------------------
@@ -214,6 +245,7 @@ __global__ void __launch_bounds__(128) k_nyq1d(V1Tables t, DevTables tab, const 
   if (job >= njobs) return;
   const int s = job % tab.M, item = job / tab.M;
   const int pair = item % tab.npairs, xl = item / tab.npairs;
+  if (t.sskip[(size_t)pair * tab.M + s]) return;           // the antipode carries this point (R-10)
   const int p = pair / tab.ns, q = pair % tab.ns;
   const cplx* FA = fhat + ((size_t)xl * tab.ns + p) * N3;
   const cplx* FB = fhat + ((size_t)xl * tab.ns + q) * N3;
@@ -380,8 +412,9 @@ __global__ void __launch_bounds__(32 * NW) k_nyq2(V1Tables t, DevTables tab, con
   const int zbit = (which == 0) ? 4 : (which == 1 ? 1 : 2);
   const int ooff = (which == 0) ? NL::UZ : (which == 1 ? NL::UXP : NL::UY);
   auto next_job = [&](int s) {                   // first s' >= s in this warp's sequence with a job to run
-    while (s < tab.M && (t.smask[s] & zbit)) {
-      if (act) {
+    const unsigned char* skip = t.sskip + (size_t)pair * tab.M;
+    while (s < tab.M && ((t.smask[s] & zbit) || skip[s])) {
+      if (act && !skip[s]) {
         cplx* out = nyq + ((size_t)item * tab.M + s) * NL::STRIDE + ooff;
 #pragma unroll
         for (int j = 0; j < N; ++j) out[j * N + ln] = make_double2(0.0, 0.0);
@@ -478,7 +511,10 @@ __global__ void __launch_bounds__(32 * W) k_xy(V1Tables t, DevTables tab, const 
     }
     cp_async_commit();
   };
-  issue(0);
+  const unsigned char* skip = t.sskip + (size_t)pair * tab.M;
+  auto next_s = [&](int s) { while (s < tab.M && skip[s]) ++s; return s; };     // sphere points run for this pair (R-10)
+  int s = next_s(0);
+  if (s < tab.M) issue(s);
   // start from the Nyquist-field product written by k_wterm
   double acc[N];
   {
@@ -486,7 +522,8 @@ __global__ void __launch_bounds__(32 * W) k_xy(V1Tables t, DevTables tab, const 
 #pragma unroll
     for (int j = 0; j < N; ++j) acc[j] = w0[j * N];
   }
-  for (int s = 0; s < tab.M; ++s) {
+  while (s < tab.M) {
+    const int sn = next_s(s + 1);
     cp_async_wait_all();
     __syncwarp();
     cplx X[N];
@@ -499,12 +536,13 @@ __global__ void __launch_bounds__(32 * W) k_xy(V1Tables t, DevTables tab, const 
     __syncwarp();
     if (act) job_pass2_in<N, true>(buf, ln, szs, sxb, X);
     __syncwarp();
-    if (s + 1 < tab.M) issue(s + 1);         // the tile is free: the next job's data arrives during pass 2
+    if (sn < tab.M) issue(sn);               // the tile is free: the next job's data arrives during pass 2
     if (act) {
       fft_reg<N, +1>(X);
 #pragma unroll
       for (int j = 0; j < N; ++j) acc[j] = fma(X[j].x, X[j].y, acc[j]);
     }
+    s = sn;
   }
   // forward y and x passes of the real plane S_r(., ., cz) (steps 6-7, after R-1)
   if (act) {
@@ -734,7 +772,7 @@ __device__ __forceinline__ void wterm_planes(const cplx* __restrict__ b_, int ha
 
 template <int N>
 __global__ void __launch_bounds__(WtermSmem<N>::THREADS, 2 / WtermSmem<N>::NH) k_wterm(const cplx* __restrict__ nyq, int M, double* __restrict__ S, const unsigned char* __restrict__ full, int npairs,
-        const unsigned char* __restrict__ smask) {
+        const unsigned char* __restrict__ smask, const unsigned char* __restrict__ sskip) {
   constexpr int H = N / 2, N2 = N * N, N3 = N2 * N;
   typedef NyqLayout<N> NL;
   typedef WtermSmem<N> WS;
@@ -746,10 +784,11 @@ __global__ void __launch_bounds__(WtermSmem<N>::THREADS, 2 / WtermSmem<N>::NH) k
   const bool act = tx < H && ty < H;
   const int cz0 = blockIdx.x * CZB;
   const cplx* nbase = nyq + (size_t)blockIdx.y * M * NL::STRIDE;
+  const unsigned char* skip = sskip + (size_t)(blockIdx.y % npairs) * M;
   auto issue = [&](int s) {
     cplx* dst = sm + (size_t)(s % NS) * WS::WORDS;
     const cplx* nq = nbase + (size_t)s * NL::STRIDE;
-    const int mask = smask[s];                       // vanishing fields are not staged
+    const int mask = skip[s] ? 7 : smask[s];         // vanishing fields and skipped points (R-10) are not staged
     for (int e = threadIdx.x; e < WS::COPIES; e += NT) {
       if (e < N2) {
         const int cy = e / N, cx = e % N;
@@ -777,7 +816,7 @@ __global__ void __launch_bounds__(WtermSmem<N>::THREADS, 2 / WtermSmem<N>::NH) k
     if (s + NS - 1 < M) issue(s + NS - 1); else cp_async_commit();
     if (!act) continue;
     const cplx* b_ = sm + (size_t)(s % NS) * WS::WORDS;
-    switch (smask[s]) {                              // uniform over the block
+    switch (skip[s] ? 7 : smask[s]) {                // uniform over the block
       case 0: wterm_planes<N, 0>(b_, half, tx, ty, acc); break;
       case 1: wterm_planes<N, 1>(b_, half, tx, ty, acc); break;
       case 2: wterm_planes<N, 2>(b_, half, tx, ty, acc); break;
@@ -959,7 +998,13 @@ FlopsV1 flops_v1(const dgfs_ctx* c) {
 
 double flops_per_pair_eval_v1(const dgfs_ctx* c, int pair) {
   const FlopsV1 f = flops_v1(c);
-  return c->N_rho * (c->full[pair] ? f.per_r_full : f.per_r) + f.tail;
+  if (c->full[pair]) return c->N_rho * f.per_r_full + f.tail;
+  // same-species VHS pairs run one point of every antipodal couple (R-10): the s-proportional kernels scale
+  int run = 0;
+  for (int s2 = 0; s2 < c->M; ++s2) run += !c->v1_sskip[(size_t)pair * c->M + s2];
+  const double frac = (double)run / c->M;
+  const double fwd = c->N * (c->N + 1.0) * 5.0 * c->N * log2((double)c->N);     // forward passes in k_xy: once per plane
+  return c->N_rho * (f.zshift + frac * (f.nyq + f.wterm + f.xy - fwd) + fwd + f.acc) + f.tail;
 }
 
 template <int N>
@@ -983,6 +1028,15 @@ static int collide_v1_impl(dgfs_ctx* c, const double* f, double* out, int nx, bo
   int nfull = 0;
   for (int pr = 0; pr < c->npairs; ++pr) nfull += c->full[pr];
   const int nvhs = c->npairs - nfull;
+  // share of the sphere points actually run, summed over the VHS pairs / over all pairs (R-10)
+  double run_vhs = 0.0, run_all = 0.0;
+  for (int pr = 0; pr < c->npairs; ++pr) {
+    int run = 0;
+    for (int s2 = 0; s2 < c->M; ++s2) run += !c->v1_sskip[(size_t)pr * c->M + s2];
+    run_all += (double)run / c->M;
+    if (!c->full[pr]) run_vhs += (double)run / c->M;
+  }
+  const double fwd_xy = N * (N + 1.0) * 5.0 * N * log2((double)N);      // forward passes inside k_xy, once per plane
   const int ns = c->ns, np = c->npairs, nz = c->v1_nz, nz0 = c->v1_nz0;
   const size_t smem_plane = plane_smem_per_warp<N>() * W;
   const size_t smem_final = plane_smem_per_warp<N>() * 2;
@@ -1028,14 +1082,14 @@ static int collide_v1_impl(dgfs_ctx* c, const double* f, double* out, int nx, bo
       if (nz > nz0)
       { ProfScope ps(c->prof, st, "k_zshift", items * fl.zshift);
         k_zshift<N><<<dim3(hpen_blocks, nz - nz0, nb), 128, 0, st>>>(c->v1, ns, fhh, Gz, r, 0); }
-      { ProfScope ps(c->prof, st, "k_nyq1d", items * c->M * 16.0 * N2);
+      { ProfScope ps(c->prof, st, "k_nyq1d", nb * run_all * c->M * 16.0 * N2);
         k_nyq1d<N><<<(items * c->M + 3) / 4, 128, 0, st>>>(c->v1, c->tab, fhat, nyq, r, items * c->M); }
-      { ProfScope ps(c->prof, st, "k_nyq2", items * (fl.nyq - c->M * 16.0 * N2));
+      { ProfScope ps(c->prof, st, "k_nyq2", nb * run_all * (fl.nyq - c->M * 16.0 * N2));
         k_nyq2<N, 2><<<dim3(3, items), 64, smem_nyq, st>>>(c->v1, c->tab, fhh, nyqy, nyq, r); }
       if (nvhs > 0) {
-        { ProfScope ps(c->prof, st, "k_wterm", nb * nvhs * fl.wterm);
-          k_wterm<N><<<dim3(N / WtermSmem<N>::CZB, items), WtermSmem<N>::THREADS, smem_wt, st>>>(nyq, c->M, S, c->tab.full, np, c->v1.smask); }
-        { ProfScope ps(c->prof, st, "k_xy", nb * nvhs * fl.xy);
+        { ProfScope ps(c->prof, st, "k_wterm", nb * run_vhs * fl.wterm);
+          k_wterm<N><<<dim3(N / WtermSmem<N>::CZB, items), WtermSmem<N>::THREADS, smem_wt, st>>>(nyq, c->M, S, c->tab.full, np, c->v1.smask, c->v1.sskip); }
+        { ProfScope ps(c->prof, st, "k_xy", nb * (run_vhs * (fl.xy - fwd_xy) + nvhs * fwd_xy));
           k_xy<N, W><<<dim3((N + W - 1) / W, items), 32 * W, smem_xy, st>>>(c->v1, c->tab, Gz, nyq, S, T + (size_t)(r % RG) * slot_stride, r); }
         if ((r + 1) % RG == 0 || r + 1 == c->N_rho) {
           const int r0 = (r / RG) * RG, nr = r + 1 - r0;

@@ -108,8 +108,8 @@ struct dgfs_ctx {
   int *d_v1_zsp = nullptr, *d_v1_zmap = nullptr;
   dgfs::cplx *d_v1_hz = nullptr, *d_v1_hxy = nullptr;
   double *d_v1_szv = nullptr, *d_v1_sxy = nullptr;
-  std::vector<unsigned char> v1_smask;
-  unsigned char* d_v1_smask = nullptr;
+  std::vector<unsigned char> v1_smask, v1_sskip;
+  unsigned char *d_v1_smask = nullptr, *d_v1_sskip = nullptr;
   dgfs::V1Tables v1{};
   // workspace (grown on demand)
   void* ws = nullptr;

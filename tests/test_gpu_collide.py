@@ -121,6 +121,28 @@ def test_v0_pipeline_on_vss_pairs(torch_cuda, monkeypatch, N, alpha):
     _small_radial_rule(torch_cuda, N, 3, 12, len(alpha), alpha)
 
 
+def test_v1_antipodal_symmetry_switch(torch_cuda, monkeypatch):
+    """R-10: same-species VHS pairs run one point of every antipodal couple with the summed weight.  With the
+    switch off every point is run; both agree with the oracle, and with each other far below the tolerance."""
+    torch = torch_cuda
+    from oracle.collide import collide_pairs
+    cfg = _rand_cfg("t", 2, 16, 3, 32, (1.0, 1.0), (0.6, 0.8), (1.0, 2.0), seed=41)     # unequal weights in the rule
+    rng = np.random.default_rng(41)
+    f = make_points(cfg, range(cfg.nx)) * (1.0 + 0.3 * rng.uniform(-1, 1, (cfg.nx, 2, 16 ** 3)))
+    Qo = collide_pairs(_oracle_tables(cfg), f)
+    fd = torch.from_numpy(f).cuda()
+    with _gpu_op(cfg) as op:
+        Q_on = op.collide_pairs(fd).cpu().numpy()
+        fl_on = op.flops_per_pair_eval(0, 0), op.flops_per_pair_eval(0, 1)
+    monkeypatch.setenv("DGFS_V1_ANTIPODAL", "0")
+    with _gpu_op(cfg) as op:
+        Q_off = op.collide_pairs(fd).cpu().numpy()
+        fl_off = op.flops_per_pair_eval(0, 0), op.flops_per_pair_eval(0, 1)
+    assert _pair_errs(Q_on, Qo).max() < TOL and _pair_errs(Q_off, Qo).max() < TOL
+    assert _pair_errs(Q_on, Q_off).max() < 1e-12
+    assert fl_on[0] < 0.62 * fl_off[0] and fl_on[1] == fl_off[1]          # only the diagonal pair gets cheaper
+
+
 def test_v1_user_sphere_rule_without_symmetry(torch_cuda):
     """A caller-supplied sigma set with no shared sigma_z values (every z shift is its own job)."""
     torch = torch_cuda
