@@ -131,6 +131,29 @@ int build_tables_v1(dgfs_ctx* c) {
       }
     }
   }
+  // R-11, VHS pairs (p,q) and (q,p): the antipode exchanges their shifted fields, A'_s' = B_s and B'_s' = A_s, so
+  // their products agree point by point on the sphere, and when every point has an antipode of the SAME weight
+  // the sums S_r^(qp) = S_r^(pq) agree too.  (q,p), q > p, then runs no plane job at all: its forward z pass reads
+  // the buffer of (p,q) and applies its own b_r.
+  c->v1_tsrc.resize(np);
+  for (int pr = 0; pr < np; ++pr) c->v1_tsrc[pr] = pr;
+  {
+    const char* ap = getenv("DGFS_V1_ANTIPODAL");
+    bool sym = !(ap && atoi(ap) == 0);
+    for (int s2 = 0; sym && s2 < M; ++s2) {
+      bool found = false;
+      for (int s3 = 0; s3 < M && !found; ++s3)
+        found = c->sigma[3 * s3] == -c->sigma[3 * s2] && c->sigma[3 * s3 + 1] == -c->sigma[3 * s2 + 1] &&
+                c->sigma[3 * s3 + 2] == -c->sigma[3 * s2 + 2] && c->w_sigma[s3] == c->w_sigma[s2];
+      sym = found;
+    }
+    for (int p = 0; sym && p < ns; ++p)
+      for (int q = p + 1; q < ns; ++q) {
+        if (c->full[p * ns + q] || c->full[q * ns + p]) continue;
+        c->v1_tsrc[q * ns + p] = p * ns + q;
+        for (int s2 = 0; s2 < M; ++s2) c->v1_sskip[(size_t)(q * ns + p) * M + s2] = 1;
+      }
+  }
   // sphere points with a vanishing component (every point of the octahedron and of the icosahedron has one):
   // sin(0) = 0, so that axis contributes no anti-Hermitian part at all
   c->v1_smask.assign(M, 0);
@@ -140,6 +163,7 @@ int build_tables_v1(dgfs_ctx* c) {
   int rc;
   if ((rc = upload(c, &c->d_v1_smask, c->v1_smask, "upload sphere masks"))) return rc;
   if ((rc = upload(c, &c->d_v1_sskip, c->v1_sskip, "upload antipode masks"))) return rc;
+  if ((rc = upload(c, &c->d_v1_tsrc, c->v1_tsrc, "upload pair sources"))) return rc;
   if ((rc = upload(c, &c->d_v1_zsp, c->v1_zsp, "upload z-job species"))) return rc;
   if ((rc = upload(c, &c->d_v1_zmap, c->v1_zmap, "upload z-job map"))) return rc;
   if ((rc = upload(c, &c->d_v1_hz, hz, "upload z factors"))) return rc;
@@ -148,13 +172,13 @@ int build_tables_v1(dgfs_ctx* c) {
   if ((rc = upload(c, &c->d_v1_sxy, sxy, "upload x,y scalars"))) return rc;
   V1Tables& t = c->v1;
   t.nz = nz; t.zsp = c->d_v1_zsp; t.zmap = c->d_v1_zmap; t.hz = c->d_v1_hz; t.szv = c->d_v1_szv;
-  t.hxy = c->d_v1_hxy; t.sxy = c->d_v1_sxy; t.smask = c->d_v1_smask; t.sskip = c->d_v1_sskip;
+  t.hxy = c->d_v1_hxy; t.sxy = c->d_v1_sxy; t.smask = c->d_v1_smask; t.sskip = c->d_v1_sskip; t.tsrc = c->d_v1_tsrc;
   return DGFS_OK;
 }
 
 void free_tables_v1(dgfs_ctx* c) {
   cudaFree(c->d_v1_zsp); cudaFree(c->d_v1_zmap); cudaFree(c->d_v1_hz); cudaFree(c->d_v1_szv);
-  cudaFree(c->d_v1_hxy); cudaFree(c->d_v1_sxy); cudaFree(c->d_v1_smask); cudaFree(c->d_v1_sskip);
+  cudaFree(c->d_v1_hxy); cudaFree(c->d_v1_sxy); cudaFree(c->d_v1_smask); cudaFree(c->d_v1_sskip); cudaFree(c->d_v1_tsrc);
 }
 
 // ---------------------------------------------------------------- device code -------------------
@@ -483,7 +507,7 @@ __global__ void __launch_bounds__(32 * W) k_xy(V1Tables t, DevTables tab, const 
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
   const int cz = blockIdx.x * W + warp, item = blockIdx.y;
   const int pair = item % tab.npairs, xl = item / tab.npairs;
-  if (cz >= N || tab.full[pair]) return;
+  if (cz >= N || tab.full[pair] || t.tsrc[pair] != pair) return;      // R-11: (q,p) uses the buffer of (p,q)
   cplx* buf = sm + (size_t)warp * JS::WORDS;
   const bool act = lane < N;
   const int ln = act ? lane : 0;
@@ -772,13 +796,14 @@ __device__ __forceinline__ void wterm_planes(const cplx* __restrict__ b_, int ha
 
 template <int N>
 __global__ void __launch_bounds__(WtermSmem<N>::THREADS, 2 / WtermSmem<N>::NH) k_wterm(const cplx* __restrict__ nyq, int M, double* __restrict__ S, const unsigned char* __restrict__ full, int npairs,
-        const unsigned char* __restrict__ smask, const unsigned char* __restrict__ sskip) {
+        const unsigned char* __restrict__ smask, const unsigned char* __restrict__ sskip, const int* __restrict__ tsrc) {
   constexpr int H = N / 2, N2 = N * N, N3 = N2 * N;
   typedef NyqLayout<N> NL;
   typedef WtermSmem<N> WS;
   constexpr int CZG = WS::CZG, CZB = WS::CZB, NT = WS::THREADS, NS = WS::STAGES;
   extern __shared__ cplx sm[];
-  if (full[blockIdx.y % npairs]) return;            // pairs with a full b table take k_xy_full (uniform per block)
+  // pairs with a full b table take k_xy_full, transposed pairs reuse the other's S_r (uniform per block)
+  if (full[blockIdx.y % npairs] || tsrc[blockIdx.y % npairs] != (int)(blockIdx.y % npairs)) return;
   const int half = threadIdx.x / 256, tt = threadIdx.x % 256;
   const int tx = tt % 16, ty = tt / 16;
   const bool act = tx < H && ty < H;
@@ -843,8 +868,8 @@ __global__ void __launch_bounds__(WtermSmem<N>::THREADS, 2 / WtermSmem<N>::NH) k
 // decimation-in-frequency step, then a length-N/2 transform in registers), so that the accumulators of
 // the whole group stay in registers and QG is touched once per group.  FIRST: store, do not accumulate.
 template <int N, bool FIRST>
-__global__ void __launch_bounds__(256) k_zfwd_acc(DevTables tab, const cplx* __restrict__ T, size_t slot_stride,
-                                                  cplx* __restrict__ QGh, size_t qstride, int r0, int nr) {
+__global__ void __launch_bounds__(256) k_zfwd_acc(DevTables tab, const int* __restrict__ tsrc, const cplx* __restrict__ T,
+                                                  size_t slot_stride, cplx* __restrict__ QGh, size_t qstride, int r0, int nr) {
   constexpr int H = N / 2, NPH = N * (H + 1);
   const int par = threadIdx.x >> 7;
   const int pid = blockIdx.x * 128 + (threadIdx.x & 127);
@@ -856,7 +881,7 @@ __global__ void __launch_bounds__(256) k_zfwd_acc(DevTables tab, const cplx* __r
 #pragma unroll
   for (int k = 0; k < H; ++k) acc[k] = make_double2(0.0, 0.0);
   for (int sl = 0; sl < nr; ++sl) {
-    const cplx* src = T + (size_t)sl * slot_stride + (size_t)item * (N * NPH) + pid;
+    const cplx* src = T + (size_t)sl * slot_stride + (size_t)(item - pair + tsrc[pair]) * (N * NPH) + pid;   // R-11
     cplx u[H];
     if (par == 0) {
 #pragma unroll
@@ -999,6 +1024,7 @@ FlopsV1 flops_v1(const dgfs_ctx* c) {
 double flops_per_pair_eval_v1(const dgfs_ctx* c, int pair) {
   const FlopsV1 f = flops_v1(c);
   if (c->full[pair]) return c->N_rho * f.per_r_full + f.tail;
+  if (c->v1_tsrc[pair] != pair) return c->N_rho * f.acc + f.tail;      // R-11: only the forward z pass and step 10
   // same-species VHS pairs run one point of every antipodal couple (R-10): the s-proportional kernels scale
   int run = 0;
   for (int s2 = 0; s2 < c->M; ++s2) run += !c->v1_sskip[(size_t)pair * c->M + s2];
@@ -1030,11 +1056,13 @@ static int collide_v1_impl(dgfs_ctx* c, const double* f, double* out, int nx, bo
   const int nvhs = c->npairs - nfull;
   // share of the sphere points actually run, summed over the VHS pairs / over all pairs (R-10)
   double run_vhs = 0.0, run_all = 0.0;
+  int nrun_vhs = 0;                                                     // VHS pairs that run plane jobs (R-11)
   for (int pr = 0; pr < c->npairs; ++pr) {
     int run = 0;
     for (int s2 = 0; s2 < c->M; ++s2) run += !c->v1_sskip[(size_t)pr * c->M + s2];
     run_all += (double)run / c->M;
     if (!c->full[pr]) run_vhs += (double)run / c->M;
+    if (!c->full[pr] && c->v1_tsrc[pr] == pr) ++nrun_vhs;
   }
   const double fwd_xy = N * (N + 1.0) * 5.0 * N * log2((double)N);      // forward passes inside k_xy, once per plane
   const int ns = c->ns, np = c->npairs, nz = c->v1_nz, nz0 = c->v1_nz0;
@@ -1088,14 +1116,14 @@ static int collide_v1_impl(dgfs_ctx* c, const double* f, double* out, int nx, bo
         k_nyq2<N, 2><<<dim3(3, items), 64, smem_nyq, st>>>(c->v1, c->tab, fhh, nyqy, nyq, r); }
       if (nvhs > 0) {
         { ProfScope ps(c->prof, st, "k_wterm", nb * run_vhs * fl.wterm);
-          k_wterm<N><<<dim3(N / WtermSmem<N>::CZB, items), WtermSmem<N>::THREADS, smem_wt, st>>>(nyq, c->M, S, c->tab.full, np, c->v1.smask, c->v1.sskip); }
-        { ProfScope ps(c->prof, st, "k_xy", nb * (run_vhs * (fl.xy - fwd_xy) + nvhs * fwd_xy));
+          k_wterm<N><<<dim3(N / WtermSmem<N>::CZB, items), WtermSmem<N>::THREADS, smem_wt, st>>>(nyq, c->M, S, c->tab.full, np, c->v1.smask, c->v1.sskip, c->v1.tsrc); }
+        { ProfScope ps(c->prof, st, "k_xy", nb * (run_vhs * (fl.xy - fwd_xy) + nrun_vhs * fwd_xy));
           k_xy<N, W><<<dim3((N + W - 1) / W, items), 32 * W, smem_xy, st>>>(c->v1, c->tab, Gz, nyq, S, T + (size_t)(r % RG) * slot_stride, r); }
         if ((r + 1) % RG == 0 || r + 1 == c->N_rho) {
           const int r0 = (r / RG) * RG, nr = r + 1 - r0;
           ProfScope ps(c->prof, st, "k_zfwd_acc", nb * nvhs * fl.acc * nr);
-          if (r0 == 0) k_zfwd_acc<N, true><<<dim3(hp_blocks, items), 256, 0, st>>>(c->tab, T, slot_stride, QG, qstride, r0, nr);
-          else k_zfwd_acc<N, false><<<dim3(hp_blocks, items), 256, 0, st>>>(c->tab, T, slot_stride, QG, qstride, r0, nr);
+          if (r0 == 0) k_zfwd_acc<N, true><<<dim3(hp_blocks, items), 256, 0, st>>>(c->tab, c->v1.tsrc, T, slot_stride, QG, qstride, r0, nr);
+          else k_zfwd_acc<N, false><<<dim3(hp_blocks, items), 256, 0, st>>>(c->tab, c->v1.tsrc, T, slot_stride, QG, qstride, r0, nr);
         }
       }
       if (nfull > 0) {

@@ -19,6 +19,7 @@ struct V1Tables {
   const double* szv;         // [r][nz]              anti-Hermitian z scalar (1/N folded)
   const cplx* hxy;           // [pair][r][s][side][2][N]   x factors then y factors
   const double* sxy;         // [pair][r][s][side][2]      anti-Hermitian x, y scalars
+  const int* tsrc;           // [pair]  pair whose S_r (buffer T) this pair uses: itself, or its transpose (q,p) -> (p,q) (R-11)
   const unsigned char* sskip; // [pair][s]  1: sphere point not run for this pair, its antipode carries both weights (R-10)
   const unsigned char* smask; // [s]  bit d set: sigma_{s,d} = 0, so s_d = 0 for every pair and radial node and
                              //      the Nyquist field of that axis (ux', uy, uz for d = x, y, z) vanishes identically
