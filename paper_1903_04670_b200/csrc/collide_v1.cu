@@ -154,6 +154,45 @@ int build_tables_v1(dgfs_ctx* c) {
         for (int s2 = 0; s2 < M; ++s2) c->v1_sskip[(size_t)(q * ns + p) * M + s2] = 1;
       }
   }
+  // The same two symmetries for pairs with a full table b_rs: the products agree, P_s' = (w_s' / w_s) P_s, but b_rs'
+  // differs from b_rs, so every (pair, s) keeps its own multiply-accumulate in k_zfwd_full and only the plane jobs
+  // and their forward x,y passes are shared: (p,p) runs one point per antipodal couple, (q,p) runs none.
+  c->v1_fsrc_s.resize((size_t)np * M);
+  c->v1_fscale.assign((size_t)np * M, 1.0);
+  for (int pr = 0; pr < np; ++pr) for (int s2 = 0; s2 < M; ++s2) c->v1_fsrc_s[(size_t)pr * M + s2] = s2;
+  {
+    const char* ap = getenv("DGFS_V1_ANTIPODAL");
+    bool all = !(ap && atoi(ap) == 0);
+    std::vector<int> anti(M, -1);
+    for (int s2 = 0; s2 < M; ++s2) {
+      for (int s3 = 0; s3 < M; ++s3)
+        if (c->sigma[3 * s3] == -c->sigma[3 * s2] && c->sigma[3 * s3 + 1] == -c->sigma[3 * s2 + 1] &&
+            c->sigma[3 * s3 + 2] == -c->sigma[3 * s2 + 2]) { anti[s2] = s3; break; }
+      if (anti[s2] < 0) all = false;
+    }
+    for (int p = 0; all && p < ns; ++p) {
+      const int dp = p * ns + p;
+      if (c->full[dp])
+        for (int s2 = 0; s2 < M; ++s2) {
+          const int s3 = anti[s2];
+          if (s3 > s2) {                    // s2 runs, s3 reads its buffer
+            c->v1_sskip[(size_t)dp * M + s3] = 1;
+            c->v1_fsrc_s[(size_t)dp * M + s3] = s2;
+            c->v1_fscale[(size_t)dp * M + s3] = c->w_sigma[s3] / c->w_sigma[s2];
+          }
+        }
+      for (int q = p + 1; q < ns; ++q) {
+        const int pq = p * ns + q, qp = q * ns + p;
+        if (!c->full[pq] || !c->full[qp]) continue;
+        c->v1_tsrc[qp] = pq;
+        for (int s2 = 0; s2 < M; ++s2) {
+          c->v1_sskip[(size_t)qp * M + s2] = 1;
+          c->v1_fsrc_s[(size_t)qp * M + s2] = anti[s2];
+          c->v1_fscale[(size_t)qp * M + s2] = c->w_sigma[s2] / c->w_sigma[anti[s2]];
+        }
+      }
+    }
+  }
   // sphere points with a vanishing component (every point of the octahedron and of the icosahedron has one):
   // sin(0) = 0, so that axis contributes no anti-Hermitian part at all
   c->v1_smask.assign(M, 0);
@@ -164,6 +203,8 @@ int build_tables_v1(dgfs_ctx* c) {
   if ((rc = upload(c, &c->d_v1_smask, c->v1_smask, "upload sphere masks"))) return rc;
   if ((rc = upload(c, &c->d_v1_sskip, c->v1_sskip, "upload antipode masks"))) return rc;
   if ((rc = upload(c, &c->d_v1_tsrc, c->v1_tsrc, "upload pair sources"))) return rc;
+  if ((rc = upload(c, &c->d_v1_fsrc_s, c->v1_fsrc_s, "upload product sources"))) return rc;
+  if ((rc = upload(c, &c->d_v1_fscale, c->v1_fscale, "upload product scales"))) return rc;
   if ((rc = upload(c, &c->d_v1_zsp, c->v1_zsp, "upload z-job species"))) return rc;
   if ((rc = upload(c, &c->d_v1_zmap, c->v1_zmap, "upload z-job map"))) return rc;
   if ((rc = upload(c, &c->d_v1_hz, hz, "upload z factors"))) return rc;
@@ -172,13 +213,13 @@ int build_tables_v1(dgfs_ctx* c) {
   if ((rc = upload(c, &c->d_v1_sxy, sxy, "upload x,y scalars"))) return rc;
   V1Tables& t = c->v1;
   t.nz = nz; t.zsp = c->d_v1_zsp; t.zmap = c->d_v1_zmap; t.hz = c->d_v1_hz; t.szv = c->d_v1_szv;
-  t.hxy = c->d_v1_hxy; t.sxy = c->d_v1_sxy; t.smask = c->d_v1_smask; t.sskip = c->d_v1_sskip; t.tsrc = c->d_v1_tsrc;
+  t.hxy = c->d_v1_hxy; t.sxy = c->d_v1_sxy; t.smask = c->d_v1_smask; t.sskip = c->d_v1_sskip; t.tsrc = c->d_v1_tsrc; t.fsrc_s = c->d_v1_fsrc_s; t.fscale = c->d_v1_fscale;
   return DGFS_OK;
 }
 
 void free_tables_v1(dgfs_ctx* c) {
   cudaFree(c->d_v1_zsp); cudaFree(c->d_v1_zmap); cudaFree(c->d_v1_hz); cudaFree(c->d_v1_szv);
-  cudaFree(c->d_v1_hxy); cudaFree(c->d_v1_sxy); cudaFree(c->d_v1_smask); cudaFree(c->d_v1_sskip); cudaFree(c->d_v1_tsrc);
+  cudaFree(c->d_v1_hxy); cudaFree(c->d_v1_sxy); cudaFree(c->d_v1_smask); cudaFree(c->d_v1_sskip); cudaFree(c->d_v1_tsrc); cudaFree(c->d_v1_fsrc_s); cudaFree(c->d_v1_fscale);
 }
 
 // ---------------------------------------------------------------- device code -------------------
@@ -618,7 +659,7 @@ __global__ void __launch_bounds__(32 * W) k_xy_full(V1Tables t, DevTables tab, c
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
   const int cz = blockIdx.x * W + warp, item = blockIdx.y;
   const int pair = item % tab.npairs, xl = item / tab.npairs;
-  if (cz >= N || !tab.full[pair]) return;
+  if (cz >= N || !tab.full[pair] || t.tsrc[pair] != pair) return;     // (q,p) reads the products of (p,q)
   cplx* buf = sm + (size_t)warp * FS::WORDS;
   const bool act = lane < N;
   const int ln = act ? lane : 0;
@@ -650,8 +691,12 @@ __global__ void __launch_bounds__(32 * W) k_xy_full(V1Tables t, DevTables tab, c
     }
     cp_async_commit();
   };
-  issue(0);
-  for (int s = 0; s < tab.M; ++s) {
+  const unsigned char* skip = t.sskip + (size_t)pair * tab.M;
+  auto next_s = [&](int s) { while (s < tab.M && skip[s]) ++s; return s; };     // points run for this pair (R-10)
+  int s = next_s(0);
+  if (s < tab.M) issue(s);
+  while (s < tab.M) {
+    const int sn = next_s(s + 1);
     cp_async_wait_all();
     __syncwarp();
     cplx X[N];
@@ -688,13 +733,14 @@ __global__ void __launch_bounds__(32 * W) k_xy_full(V1Tables t, DevTables tab, c
       for (int i = 0; i < N; ++i) X[i] = buf[ln * P + i];          // lane = ky
     }
     __syncwarp();
-    if (s + 1 < tab.M) issue(s + 1);                       // tile and tables are free again
+    if (sn < tab.M) issue(sn);                             // tile and tables are free again
     if (act) {
       fft_reg<N, -1>(X);                                   // forward x pass
       cplx* o = Tf + ((size_t)item * tab.M + s) * N3 + (size_t)cz * N2 + ln;
 #pragma unroll
       for (int k = 0; k < N; ++k) o[k * N] = X[k];         // [cz][kx][ky]
     }
+    s = sn;
   }
 }
 
@@ -702,8 +748,8 @@ __global__ void __launch_bounds__(32 * W) k_xy_full(V1Tables t, DevTables tab, c
 //   QG[item][kz][kx][ky] (+)= w_r sum_s b_rs(k) fft_z( Tf[item][s][.][kx][ky] );  thread pair per pencil as in
 // k_zfwd_acc, the sum over s stays in registers.  b is read in SPEC layout [r][s][kz][kx][ky].
 template <int N, bool FIRST>
-__global__ void __launch_bounds__(256) k_zfwd_full(DevTables tab, const cplx* __restrict__ Tf, cplx* __restrict__ QG,
-                                                   size_t qstride, int r) {
+__global__ void __launch_bounds__(256) k_zfwd_full(DevTables tab, V1Tables t, const cplx* __restrict__ Tf,
+                                                   cplx* __restrict__ QG, size_t qstride, int r) {
   constexpr int H = N / 2, N2 = N * N, N3 = N2 * N;
   const int par = threadIdx.x >> 7;
   const int pid = blockIdx.x * 128 + (threadIdx.x & 127);
@@ -714,7 +760,9 @@ __global__ void __launch_bounds__(256) k_zfwd_full(DevTables tab, const cplx* __
 #pragma unroll
   for (int k = 0; k < H; ++k) acc[k] = make_double2(0.0, 0.0);
   for (int s = 0; s < tab.M; ++s) {
-    const cplx* src = Tf + ((size_t)item * tab.M + s) * N3 + pid;
+    // the transformed product of (pair, s): its own, or the one it shares (R-10 / R-11)
+    const cplx* src = Tf + ((size_t)(item - pair + t.tsrc[pair]) * tab.M + t.fsrc_s[(size_t)pair * tab.M + s]) * N3 + pid;
+    const double fs = t.fscale[(size_t)pair * tab.M + s];
     cplx u[H];
     if (par == 0) {
 #pragma unroll
@@ -726,7 +774,10 @@ __global__ void __launch_bounds__(256) k_zfwd_full(DevTables tab, const cplx* __
     fft_reg<H, -1>(u);
     const cplx* bf = tab.bfull[pair] + ((size_t)r * tab.M + s) * N3 + pid;
 #pragma unroll
-    for (int k = 0; k < H; ++k) acc[k] = cfma(bf[(size_t)(2 * k + par) * N2], u[k], acc[k]);
+    for (int k = 0; k < H; ++k) {
+      const cplx b = bf[(size_t)(2 * k + par) * N2];
+      acc[k] = cfma(make_double2(fs * b.x, fs * b.y), u[k], acc[k]);
+    }
   }
   cplx* dst = QG + (size_t)item * qstride + pid;
 #pragma unroll
@@ -1023,7 +1074,12 @@ FlopsV1 flops_v1(const dgfs_ctx* c) {
 
 double flops_per_pair_eval_v1(const dgfs_ctx* c, int pair) {
   const FlopsV1 f = flops_v1(c);
-  if (c->full[pair]) return c->N_rho * f.per_r_full + f.tail;
+  if (c->full[pair]) {
+    int run = 0;
+    for (int s2 = 0; s2 < c->M; ++s2) run += !c->v1_sskip[(size_t)pair * c->M + s2];
+    const double frac = (double)run / c->M;
+    return c->N_rho * ((frac > 0 ? f.zshift : 0.0) + frac * (f.nyq + f.xy_full) + f.acc_full) + f.tail;
+  }
   if (c->v1_tsrc[pair] != pair) return c->N_rho * f.acc + f.tail;      // R-11: only the forward z pass and step 10
   // same-species VHS pairs run one point of every antipodal couple (R-10): the s-proportional kernels scale
   int run = 0;
@@ -1127,11 +1183,11 @@ static int collide_v1_impl(dgfs_ctx* c, const double* f, double* out, int nx, bo
         }
       }
       if (nfull > 0) {
-        { ProfScope ps(c->prof, st, "k_xy_full", nb * nfull * fl.xy_full);
+        { ProfScope ps(c->prof, st, "k_xy_full", nb * (run_all - run_vhs) * fl.xy_full);
           k_xy_full<N, W><<<dim3((N + W - 1) / W, items), 32 * W, smem_xyf, st>>>(c->v1, c->tab, Gz, nyq, Tf, r); }
         { ProfScope ps(c->prof, st, "k_zfwd_full", nb * nfull * fl.acc_full);
-          if (r == 0) k_zfwd_full<N, true><<<dim3(pen_blocks, items), 256, 0, st>>>(c->tab, Tf, QG, qstride, r);
-          else k_zfwd_full<N, false><<<dim3(pen_blocks, items), 256, 0, st>>>(c->tab, Tf, QG, qstride, r); }
+          if (r == 0) k_zfwd_full<N, true><<<dim3(pen_blocks, items), 256, 0, st>>>(c->tab, c->v1, Tf, QG, qstride, r);
+          else k_zfwd_full<N, false><<<dim3(pen_blocks, items), 256, 0, st>>>(c->tab, c->v1, Tf, QG, qstride, r); }
       }
     }
     // step 10

@@ -20,6 +20,9 @@ struct V1Tables {
   const cplx* hxy;           // [pair][r][s][side][2][N]   x factors then y factors
   const double* sxy;         // [pair][r][s][side][2]      anti-Hermitian x, y scalars
   const int* tsrc;           // [pair]  pair whose S_r (buffer T) this pair uses: itself, or its transpose (q,p) -> (p,q) (R-11)
+  const int* fsrc_s;         // [pair][s]  full-table pairs: sphere point whose transformed product P_s (buffer Tf of pair
+                             //            tsrc[pair]) equals this one's up to the factor fscale (R-10 / R-11)
+  const double* fscale;      // [pair][s]
   const unsigned char* sskip; // [pair][s]  1: sphere point not run for this pair, its antipode carries both weights (R-10)
   const unsigned char* smask; // [s]  bit d set: sigma_{s,d} = 0, so s_d = 0 for every pair and radial node and
                              //      the Nyquist field of that axis (ux', uy, uz for d = x, y, z) vanishes identically
