@@ -25,9 +25,9 @@ UNIT = "pair-evals/s"
 # pipe is also measured live with dgfs_measure_fp64_peak (dependency-free DFMA chains) and reported.
 FP64_PEAK_NOMINAL_TFLOPS = 148 * 64 * 2 * 1.965e9 / 1e12
 PAPER_P100_PAIR_EVALS_PER_S = 1.0 / 0.01057      # Table 1 P:316 (N=32, N_rho=32, M=12), 1 x P100
-# dram__bytes_read.sum + dram__bytes_write.sum of one k_xy launch over 512 (point, pair) items at the c2
-# operating point, from the `ncu --set full` capture summarised in profiles/r01_v1_ncu.md
-NCU_DRAM_BYTES_PER_ITEM = {"k_xy": (748.2e6 + 132.3e6) / 512}
+# dram__bytes_read.sum + dram__bytes_write.sum of one k_xy launch over 512 points (all pairs, one radial node) at
+# the c2 operating point, from the `ncu --set full` capture summarised in profiles/r01_v1_ncu.md
+NCU_DRAM_BYTES_PER_POINT = {"k_xy": (2.842e9 + 0.4463e9) / 512}
 
 
 def parse():
@@ -254,11 +254,11 @@ def main():
             "flops_per_launch": top["flops"] / top["launches"],
             "whole_step_tflops": flops_step / (ms_per_step * 1e-3) / 1e12 / 1.0,
             "whole_step_frac": flops_step / (ms_per_step * 1e-3) / 1e12 / FP64_PEAK_NOMINAL_TFLOPS,
-            "traffic": (NCU_DRAM_BYTES_PER_ITEM[top["name"]] * (nx * cfg.ns * cfg.ns * cfg.N_rho / top["launches"] * args.steps)
-                        if top["name"] in NCU_DRAM_BYTES_PER_ITEM and (cfg.N, cfg.N_rho, cfg.M) == (32, 32, 12) else None),
+            "traffic": (NCU_DRAM_BYTES_PER_POINT[top["name"]] * (nx * cfg.N_rho / top["launches"] * args.steps)
+                        if top["name"] in NCU_DRAM_BYTES_PER_POINT and (cfg.N, cfg.N_rho, cfg.M) == (32, 32, 12) else None),
             "traffic_note": "DRAM bytes per launch of the dominant kernel, scaled from the ncu capture in "
-                            "profiles/r01_v1_ncu.md (1.72 MB per (point, pair) item); algorithmic bytes per item: "
-                            "1.18 MB z-shifted planes + 0.26 MB S + 0.28 MB T",
+                            "profiles/r01_v1_ncu.md (6.42 MB per point and radial node); algorithmic bytes per point: "
+                            "4.72 MB z-shifted half planes + 0.79 MB S + 0.83 MB T for the three pairs that run",
             "kernels": [{"name": p["name"], "launches": p["launches"], "ms": round(p["ms"], 3),
                          "tflops": (p["flops"] / (p["ms"] * 1e-3) / 1e12 if p["ms"] > 0 else None)} for p in prof],
         }
