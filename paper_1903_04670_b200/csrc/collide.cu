@@ -87,8 +87,10 @@ static int collide_impl(dgfs_ctx* c, const double* f, double* out, int nx, bool 
   double fl_shift = 0, fl_zprod = 0, fl_acc = 0;
   for (int pr = 0; pr < np; ++pr) {
     const double M = c->M;
-    fl_shift += M * (2.0 * fft3 * 2.0 / 3.0 + 12.0 * N3);
-    fl_zprod += M * (2.0 * fft3 / 3.0 + 6.0 * N3) + (c->full[pr] ? M : 1.0) * fft3 / 3.0;
+    double run = 0;
+    for (int s = 0; s < c->M; ++s) run += !c->v0_sskip[(size_t)pr * c->M + s];
+    fl_shift += run * (2.0 * fft3 * 2.0 / 3.0 + 12.0 * N3);
+    fl_zprod += run * (2.0 * fft3 / 3.0 + 6.0 * N3) + (c->full[pr] ? M : (run > 0 ? 1.0 : 0.0)) * fft3 / 3.0;
     fl_acc += (c->full[pr] ? M * (fft3 * 2.0 / 3.0 + 8.0 * N3) : (fft3 * 2.0 / 3.0 + 4.0 * N3));
   }
   for (int x0 = 0; x0 < nx; x0 += pl.nbx) {
@@ -255,6 +257,11 @@ extern "C" double dgfs_flops_per_pair_eval(const dgfs_ctx* c, int p, int q) {
   const double N3 = c->N3, fft3 = 15.0 * N3 * log2((double)c->N);
   const double tail = 2.0 * fft3 + 11.0 * N3 + fft3 / c->ns;
   const double rs = (double)c->N_rho * c->M;
-  if (c->full[p * c->ns + q]) return rs * (3.0 * fft3 + 26.0 * N3) + tail;             // verbatim Algo 2
-  return rs * (2.0 * fft3 + 22.0 * N3) + c->N_rho * (fft3 + 4.0 * N3) + tail;           // with R-1
+  const int pair = p * c->ns + q;
+  if (c->full[pair]) return rs * (3.0 * fft3 + 26.0 * N3) + tail;                        // verbatim Algo 2
+  // with R-1; R-10 / R-11: only `run` of the M sphere points are shifted and multiplied, a transposed pair none
+  int run = 0;
+  for (int s = 0; s < c->M; ++s) run += !c->v0_sskip[(size_t)pair * c->M + s];
+  const double fwd = (c->v0_tsrc[pair] == pair) ? fft3 + 4.0 * N3 : fft3 * 2.0 / 3.0 + 4.0 * N3;
+  return (double)c->N_rho * run * (2.0 * fft3 + 22.0 * N3) + c->N_rho * fwd + tail;
 }

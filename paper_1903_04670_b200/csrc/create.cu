@@ -102,7 +102,7 @@ __device__ __forceinline__ void spec_freq(int idx, int N, int& kx, int& ky, int&
 
 // phase[pair][r][s][side][d][j]
 __global__ void k_phase(cplx* out, int ns, int N, int N_rho, int M, double L, const double* mass,
-                        const double* rho, const double* sigma, const double* w_sigma) {
+                        const double* rho, const double* sigma, const double* w_sigma, const double* wfac) {
   const long total = (long)ns * ns * N_rho * M * 2 * 3 * N;
   const double pi = 3.14159265358979323846;
   for (long i = blockIdx.x * (long)blockDim.x + threadIdx.x; i < total; i += (long)gridDim.x * blockDim.x) {
@@ -116,7 +116,7 @@ __global__ void k_phase(cplx* out, int ns, int N, int N_rho, int M, double L, co
     double theta = mu * (pi * rho[r] / L) * sigma[s * 3 + d] * (double)signed_freq(j, N);
     double sn, cs; sincos(theta, &sn, &cs);
     double scale = 1.0;
-    if (d == 0) { scale = 1.0 / ((double)N * N * N); if (side == 0) scale *= w_sigma[s]; }
+    if (d == 0) { scale = 1.0 / ((double)N * N * N); if (side == 0) scale *= w_sigma[s] * wfac[(size_t)(p * ns + q) * M + s]; }
     out[i] = make_double2(cs * scale, sn * scale);
   }
 }
@@ -332,12 +332,46 @@ int build_tables(dgfs_ctx* c) {
     if ((rc = dev_upload(c, &d_sigpre, c->sigma_pre.data(), c->sigma_pre.size(), "upload sigma_pre"))) return rc;
     if ((rc = dev_upload(c, &d_wpre, c->w_pre.data(), c->w_pre.size(), "upload w_pre"))) return rc;
   }
+  // v0 pipeline: antipodal symmetries of VHS pairs (R-10, R-11; same reasoning as in collide_v1.cu)
+  c->v0_sskip.assign((size_t)np * M, 0);
+  c->v0_wfac.assign((size_t)np * M, 1.0);
+  c->v0_tsrc.resize(np);
+  for (int pr = 0; pr < np; ++pr) c->v0_tsrc[pr] = pr;
+  {
+    const char* ap = getenv("DGFS_V1_ANTIPODAL");
+    const bool on = !(ap && atoi(ap) == 0);
+    std::vector<int> anti(M, -1);
+    bool sym_w = on;
+    for (int s2 = 0; s2 < M; ++s2) {
+      for (int s3 = 0; s3 < M; ++s3)
+        if (c->sigma[3 * s3] == -c->sigma[3 * s2] && c->sigma[3 * s3 + 1] == -c->sigma[3 * s2 + 1] &&
+            c->sigma[3 * s3 + 2] == -c->sigma[3 * s2 + 2]) { anti[s2] = s3; break; }
+      if (anti[s2] < 0 || c->w_sigma[anti[s2]] != c->w_sigma[s2]) sym_w = false;
+    }
+    for (int p = 0; on && p < ns; ++p) {
+      const int dp = p * ns + p;
+      if (!c->full[dp])
+        for (int s2 = 0; s2 < M; ++s2)
+          if (anti[s2] > s2) {
+            c->v0_sskip[(size_t)dp * M + anti[s2]] = 1;
+            c->v0_wfac[(size_t)dp * M + s2] = (c->w_sigma[s2] + c->w_sigma[anti[s2]]) / c->w_sigma[s2];
+          }
+      for (int q = p + 1; sym_w && q < ns; ++q) {
+        if (c->full[p * ns + q] || c->full[q * ns + p]) continue;
+        c->v0_tsrc[q * ns + p] = p * ns + q;
+        for (int s2 = 0; s2 < M; ++s2) c->v0_sskip[(size_t)(q * ns + p) * M + s2] = 1;
+      }
+    }
+  }
+  if ((rc = dev_upload(c, &c->d_v0_sskip, c->v0_sskip.data(), c->v0_sskip.size(), "upload antipode masks"))) return rc;
+  if ((rc = dev_upload(c, &c->d_v0_tsrc, c->v0_tsrc.data(), c->v0_tsrc.size(), "upload pair sources"))) return rc;
+  if ((rc = dev_upload(c, &c->d_v0_wfac, c->v0_wfac.data(), c->v0_wfac.size(), "upload weight factors"))) return rc;
   const int TB = 256;
   auto blocks = [&](long total) { long b = (total + TB - 1) / TB; return (int)(b > 65535 * 8 ? 65535 * 8 : b); };
 
   size_t nphase = (size_t)np * Nr * M * 2 * 3 * N;
   if ((rc = check_cuda(c, cudaMalloc((void**)&c->d_phase, nphase * sizeof(cplx)), "alloc phase table"))) return rc;
-  k_phase<<<blocks(nphase), TB>>>(c->d_phase, ns, N, Nr, M, c->L, d_mass, c->d_rho, c->d_sigma, d_wsig);
+  k_phase<<<blocks(nphase), TB>>>(c->d_phase, ns, N, Nr, M, c->L, d_mass, c->d_rho, c->d_sigma, d_wsig, c->d_v0_wfac);
 
   size_t nb = (size_t)np * Nr * c->K2n;
   if ((rc = check_cuda(c, cudaMalloc((void**)&c->d_bvhs, nb * sizeof(double)), "alloc b (VHS) table"))) return rc;
@@ -372,7 +406,7 @@ int build_tables(dgfs_ctx* c) {
   DevTables& t = c->tab;
   t.ns = ns; t.npairs = np; t.N = N; t.N3 = N3; t.N_rho = Nr; t.M = M; t.K2n = c->K2n;
   t.phase = c->d_phase; t.bvhs = c->d_bvhs; t.bfull = c->d_bfull; t.closs = c->d_closs;
-  t.w_rho = c->d_w_rho; t.beta = c->d_beta; t.full = c->d_full;
+  t.w_rho = c->d_w_rho; t.beta = c->d_beta; t.full = c->d_full; t.sskip = c->d_v0_sskip; t.tsrc = c->d_v0_tsrc;
   return DGFS_OK;
 }
 
@@ -492,6 +526,7 @@ extern "C" void dgfs_destroy(dgfs_ctx* c) {
   cudaSetDevice(c->device);
   cudaFree(c->d_phase); cudaFree(c->d_bvhs); cudaFree(c->d_closs); cudaFree(c->d_w_rho); cudaFree(c->d_beta);
   cudaFree(c->d_rho); cudaFree(c->d_sigma); cudaFree(c->d_full); cudaFree(c->d_bfull);
+  cudaFree(c->d_v0_sskip); cudaFree(c->d_v0_tsrc); cudaFree(c->d_v0_wfac);
   for (auto p : c->h_bfull) cudaFree(p);
   cudaFree(c->ws); cudaFree(c->dg_ws);
   free_tables_v1(c);

@@ -27,6 +27,9 @@ struct DevTables {
   const double* w_rho;          // [N_rho]
   const double* beta;           // [pair]      beta_pq (Eq. 6)
   const unsigned char* full;    // [pair]      1 = uses bfull and per-s forward transforms
+  // v0 pipeline, VHS pairs (R-10, R-11): sphere points not run, pair whose summed products are used
+  const unsigned char* sskip;   // [pair][s]
+  const int* tsrc;              // [pair]
 };
 
 }  // namespace dgfs
@@ -98,6 +101,12 @@ struct dgfs_ctx {
   double* d_rho = nullptr;
   double* d_sigma = nullptr;
   unsigned char* d_full = nullptr;
+  std::vector<unsigned char> v0_sskip;      // antipodal symmetries of VHS pairs for the v0 pipeline
+  std::vector<int> v0_tsrc;
+  std::vector<double> v0_wfac;              // [pair][s] weight factor of the points that run
+  unsigned char* d_v0_sskip = nullptr;
+  int* d_v0_tsrc = nullptr;
+  double* d_v0_wfac = nullptr;
   dgfs::DevTables tab{};
   // v1 pipeline (collide_v1.cu): tables built by build_tables_v1, used for N <= 32
   bool use_v1 = false;

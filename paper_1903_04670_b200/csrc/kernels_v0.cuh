@@ -84,7 +84,9 @@ __global__ void __launch_bounds__(32 * W) k_plane_fwd(DevTables tab, const cplx*
   cplx* o = out + (size_t)item * N3 + (size_t)kz * N2;
   const int kzs = sfreq(kz, N);
   for (int sl = 0; sl < nsl; ++sl) {
-    const cplx* in = T + ((size_t)item * Tslices + sl) * N3 + (size_t)kz * N2;
+    // R-11: the transposed VHS pair (q,p) reads the summed products of (p,q)
+    const int sitem = (MODE == 1 && !full) ? item - pair + tab.tsrc[pair] : item;
+    const cplx* in = T + ((size_t)sitem * Tslices + sl) * N3 + (size_t)kz * N2;
     const double* bv = tab.bvhs + ((size_t)pair * tab.N_rho + r) * tab.K2n;
     const cplx* bf = (MODE == 1 && full) ? tab.bfull[pair] + ((size_t)r * tab.M + sl) * N3 + (size_t)kz * N2 : nullptr;
     warp_plane_fft<N, -1>(
@@ -125,6 +127,7 @@ __global__ void __launch_bounds__(32 * W) k_shift_xy(DevTables tab, const cplx* 
   const int p = pair / tab.ns, q = pair % tab.ns;
   for (int job = warp; job < 2 * tab.M; job += W) {
     const int s = job >> 1, side = job & 1;
+    if (tab.sskip[(size_t)pair * tab.M + s]) continue;       // R-10 / R-11: the antipode (or the transposed pair) carries it
     const cplx* in = fhat + ((size_t)xl * tab.ns + (side ? q : p)) * N3 + (size_t)lz * N2;
     const cplx* ph = tab.phase + ((((size_t)pair * tab.N_rho + r) * tab.M + s) * 2 + side) * 3 * N;
     for (int j = lane; j < N; j += 32) qv[j] = cmul(ph[N + j], ph[2 * N + lz]);
@@ -181,7 +184,11 @@ __device__ __forceinline__ void z_prod_body(const DevTables& tab, const cplx* __
   const int tid = threadIdx.x;
   const int M = tab.M;
   bool fresh = true;
-  for (int s = 0; s < M; ++s) {
+  const unsigned char* skip = tab.sskip + (size_t)(item % tab.npairs) * M;
+  int last = M - 1;                                        // last sphere point this pair runs (R-10 / R-11)
+  while (last >= 0 && skip[last]) --last;
+  for (int s = 0; s <= last; ++s) {
+    if (skip[s]) continue;
     const cplx* ga = G + (((size_t)item * M + s) * 2) * N3 + pid;
     cplx a[H], b[H];
     half_inverse_z<N, PAR>(ga, a);
@@ -193,7 +200,7 @@ __device__ __forceinline__ void z_prod_body(const DevTables& tab, const cplx* __
       S[k * 256 + tid] = pr;
     }
     fresh = false;
-    if (full || s == M - 1) {
+    if (full || s == last) {
       // forward z transform of the accumulated samples (decimation in time over the thread pair)
       cplx y[H];
 #pragma unroll
