@@ -287,12 +287,13 @@ template <int N>
 struct JobSmem {
   static constexpr int P = N + 1;
   static constexpr int TILE = N * P;
-  static constexpr int HI = TILE;            // [2][N]  factor along the pass-1 index, per side
-  static constexpr int HM = TILE + 2 * N;    // [2][N]  factor along the pass-2 index, per side
-  static constexpr int VYH = TILE + 4 * N;   // [N]     lane format
-  static constexpr int VXP = TILE + 5 * N;   // [N]
-  static constexpr int VZP = TILE + 6 * N;   // [1]
-  static constexpr int WORDS = TILE + 6 * N + 2;
+  static constexpr int TS = N + 1;           // stride between the two sides' tables: the half warps read different banks
+  static constexpr int HI = TILE;            // [2][TS]  factor along the pass-1 index, per side
+  static constexpr int HM = TILE + 2 * TS;   // [2][TS]  factor along the pass-2 index, per side
+  static constexpr int VYH = TILE + 4 * TS;  // [N]     lane format
+  static constexpr int VXP = VYH + N;        // [N]
+  static constexpr int VZP = VXP + N;        // [1]
+  static constexpr int WORDS = VZP + 2;
 };
 
 // 1-D Nyquist corrections of one (item, s) per warp (file header: the s s h, s h s, h s s and s s s terms):
@@ -371,7 +372,7 @@ __device__ __forceinline__ void job_pass1(cplx* buf, int ln, int side, int m, do
     for (int i = 0; i < N; ++i) v[i] = buf[i * P + ln];
   } else {
 #pragma unroll
-    for (int i = 0; i < N; ++i) v[i] = cmul(buf[i * P + ln], buf[JS::HI + side * N + i]);
+    for (int i = 0; i < N; ++i) v[i] = cmul(buf[i * P + ln], buf[JS::HI + side * JS::TS + i]);
   }
   if (CORR) {
     const cplx c1 = buf[JS::VYH + ln];
@@ -381,8 +382,8 @@ __device__ __forceinline__ void job_pass1(cplx* buf, int ln, int side, int m, do
   fft_reg<N, +1>(v);
   // complex h[m] for m >= 1; for the packed lane m = 0 the real h[0], h[H] scale Re (column 0) and
   // Im (column H) separately
-  const cplx hy0 = buf[JS::HM + side * N + m];
-  const double hyH = buf[JS::HM + side * N + H].x;
+  const cplx hy0 = buf[JS::HM + side * JS::TS + m];
+  const double hyH = buf[JS::HM + side * JS::TS + H].x;
   const double ya = scale * hy0.x, yb = (m == 0) ? 0.0 : -scale * hy0.y, yc = (m == 0) ? 0.0 : scale * hy0.y,
                yd = (m == 0) ? scale * hyH : scale * hy0.x;
   if (real_m) {
@@ -462,9 +463,9 @@ __global__ void __launch_bounds__(32 * NW) k_nyq2(V1Tables t, DevTables tab, con
       else if (which == 1) { hiA = hzA; hiB = hzB; hmA = hx + N; hmB = hx + 3 * N; }
       else { hiA = hzA; hiB = hzB; hmA = hx; hmB = hx + 2 * N; }
       cp_async16(&buf[JS::HI + ln], hiA + ln);
-      cp_async16(&buf[JS::HI + N + ln], hiB + ln);
+      cp_async16(&buf[JS::HI + JS::TS + ln], hiB + ln);
       cp_async16(&buf[JS::HM + ln], hmA + ln);
-      cp_async16(&buf[JS::HM + N + ln], hmB + ln);
+      cp_async16(&buf[JS::HM + JS::TS + ln], hmB + ln);
       if (ln == 0) cp_async16(&buf[JS::VZP], nyq + ((size_t)item * tab.M + s) * NL::STRIDE + NL::VT);
     }
     cp_async_commit();
@@ -566,9 +567,9 @@ __global__ void __launch_bounds__(32 * W) k_xy(V1Tables t, DevTables tab, const 
       for (int i = 0; i < N; ++i) cp_async16(&buf[i * P + ln], g + i * H);
       const cplx* hx = hbase + (size_t)s * 4 * N;          // [side][x|y][N]
       cp_async16(&buf[JS::HI + ln], hx + ln);               // h_x side A
-      cp_async16(&buf[JS::HI + N + ln], hx + 2 * N + ln);   // h_x side B
+      cp_async16(&buf[JS::HI + JS::TS + ln], hx + 2 * N + ln);   // h_x side B
       cp_async16(&buf[JS::HM + ln], hx + N + ln);           // h_y side A
-      cp_async16(&buf[JS::HM + N + ln], hx + 3 * N + ln);   // h_y side B
+      cp_async16(&buf[JS::HM + JS::TS + ln], hx + 3 * N + ln);   // h_y side B
       const cplx* nq = nbase + (size_t)s * NL::STRIDE;
       cp_async16(&buf[JS::VYH + ln], nq + NL::VYH + ln);
       cp_async16(&buf[JS::VXP + ln], nq + NL::VXP + ln);
@@ -596,7 +597,7 @@ __global__ void __launch_bounds__(32 * W) k_xy(V1Tables t, DevTables tab, const 
       // sigma_x = 0: h_x is the constant w_s / N (side A) or 1 / N; sigma_y = 0: h_y is the constant 1 / N
       const int mk = t.smask[s];
       const bool ux_ = (mk & 1) != 0, ry_ = (mk & 2) != 0;
-      job_pass1<N, true>(buf, ln, side, m, szs, ux_ ? buf[JS::HI + side * N].x : 1.0, ux_, ry_);
+      job_pass1<N, true>(buf, ln, side, m, szs, ux_ ? buf[JS::HI + side * JS::TS].x : 1.0, ux_, ry_);
     }
     __syncwarp();
     if (act) job_pass2_in<N, true>(buf, ln, szs, sxb, X);
@@ -677,9 +678,9 @@ __global__ void __launch_bounds__(32 * W) k_xy_full(V1Tables t, DevTables tab, c
       for (int i = 0; i < N; ++i) cp_async16(&buf[i * P + ln], g + i * H);
       const cplx* hx = hbase + (size_t)s * 4 * N;          // [side][x|y][N]
       cp_async16(&buf[JS::HI + ln], hx + ln);
-      cp_async16(&buf[JS::HI + N + ln], hx + 2 * N + ln);
+      cp_async16(&buf[JS::HI + JS::TS + ln], hx + 2 * N + ln);
       cp_async16(&buf[JS::HM + ln], hx + N + ln);
-      cp_async16(&buf[JS::HM + N + ln], hx + 3 * N + ln);
+      cp_async16(&buf[JS::HM + JS::TS + ln], hx + 3 * N + ln);
       const cplx* nq = nbase + (size_t)s * NL::STRIDE;
       cp_async16(&buf[JS::VYH + ln], nq + NL::VYH + ln);
       cp_async16(&buf[JS::VXP + ln], nq + NL::VXP + ln);
@@ -704,7 +705,7 @@ __global__ void __launch_bounds__(32 * W) k_xy_full(V1Tables t, DevTables tab, c
       // sigma_x = 0: h_x is the constant w_s / N (side A) or 1 / N; sigma_y = 0: h_y is the constant 1 / N
       const int mk = t.smask[s];
       const bool ux_ = (mk & 1) != 0, ry_ = (mk & 2) != 0;
-      job_pass1<N, true>(buf, ln, side, m, szs, ux_ ? buf[JS::HI + side * N].x : 1.0, ux_, ry_);
+      job_pass1<N, true>(buf, ln, side, m, szs, ux_ ? buf[JS::HI + side * JS::TS].x : 1.0, ux_, ry_);
     }
     __syncwarp();
     if (act) {
