@@ -1,6 +1,7 @@
-// collide_v1.cu -- v1 pipeline of dgfs_collide for pairs whose b_rs does not depend on s (VHS,
-// table_mode 0): Algorithm 2 of PAPER.md with the exact rearrangements of DESIGN.md
-// section 5 (R-1, R-2, R-4, R-5, R-6, R-7).
+// collide_v1.cu -- v1 pipeline of dgfs_collide (N <= 32): Algorithm 2 of PAPER.md with the exact
+// rearrangements of DESIGN.md section 5 (R-1 .. R-11).  The description below is the path of pairs whose b_rs
+// does not depend on s (VHS, table_mode 0); pairs with a full table share the first three kernels and take
+// k_xy_full / k_zfwd_full afterwards (described there).
 //
 // What is computed per pair (p,q), point x and radial node r (steps 2-8):
 //   S_r(c) = sum_s w_s Re[ A_rs(c) B_rs(c) ],   A_rs = ifft3(e^{+i mu_q a_rs} f^_p),  B_rs = ifft3(e^{-i mu_p a_rs} f^_q)
@@ -24,7 +25,9 @@
 //             (lane = pencil, FFTs in registers, one transposition through shared memory), the product
 //             and the sum over s in registers, then the forward x,y passes of the real plane S_r(., ., cz)
 //   k_zfwd_acc  forward z pass, QG += w_r b_r .
-// Steps 1 and 10 reuse the v0 kernels.
+// Steps 1 and 10 reuse the v0 kernels.  Sphere points with a zero component (R-9) skip the fields and factors
+// that vanish; same-species pairs run one point per antipodal couple (R-10) and a transposed pair (q,p) reuses
+// the summed products of (p,q) (R-11): see build_tables_v1.
 #include <cmath>
 #include <cstdio>
 #include <cstdlib>
@@ -277,7 +280,6 @@ __device__ __forceinline__ void cp_async16(void* smem, const void* gmem) {
 }
 __device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;\n" ::); }
 __device__ __forceinline__ void cp_async_wait_all() { asm volatile("cp.async.wait_group 0;\n" ::: "memory"); }
-__device__ __forceinline__ void cp_async_wait_one() { asm volatile("cp.async.wait_group 1;\n" ::: "memory"); }
 template <int PENDING>
 __device__ __forceinline__ void cp_async_wait_pending() { asm volatile("cp.async.wait_group %0;\n" ::"n"(PENDING) : "memory"); }
 
@@ -1039,7 +1041,7 @@ size_t workspace_bytes_v1(const dgfs_ctx* c, int nx) { return plan_v1(c, nx).tot
 // algorithmic FLOPs of the executed algorithm: a 1-D transform of length N counts
 // 5 N log2 N, pointwise work counts the real operations of the formulas in this file's header.
 namespace {
-struct FlopsV1 { double zshift, nyq, xy, wterm, acc, xy_full, acc_full, per_r, per_r_full, tail; };
+struct FlopsV1 { double zshift, nyq, xy, wterm, acc, xy_full, acc_full, tail; };
 FlopsV1 flops_v1(const dgfs_ctx* c) {
   const double N = c->N, N2 = N * N, N3 = N2 * N, H = N / 2, M = c->M;
   const double fft1 = 5.0 * N * log2(N), fft3 = 3.0 * N2 * fft1;
@@ -1062,12 +1064,10 @@ FlopsV1 flops_v1(const dgfs_ctx* c) {
   f.xy = N * (M * (2.0 * N * fft1 + 4.0 * N2 + 12.0 * N) + fac * N2) + N * (N + 1.0) * fft1;
   f.wterm = wops * N3 + N3;
   f.acc = N * (H + 1.0) * (fft1 + 4.0 * N);         // forward z pass and QG += w_r b_r . on the Hermitian half
-  f.per_r = f.zshift + f.nyq + f.xy + f.wterm + f.acc;
   // full-table pairs: four passes per plane job, W (10 per element) and the complex product (8), then per s
   // a forward z pass and the complex multiply-accumulate with b_rs (8 per mode)
   f.xy_full = N * (M * (4.0 * N * fft1 + 20.0 * N2 + 12.0 * N) + fac * N2);
   f.acc_full = M * (N2 * fft1 + 8.0 * N3);
-  f.per_r_full = f.zshift + f.nyq + f.xy_full + f.acc_full;
   f.tail = 2.0 * fft3 + 11.0 * N3 + fft3 / c->ns;
   return f;
 }
