@@ -39,6 +39,8 @@ def parse():
     ap.add_argument("--workload", default="c2")
     ap.add_argument("--nx", type=int, default=0, help="override the batch size (debugging only; reported)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--nyquist-filter", action="store_true",
+                    help="time the variant operator Q(P f_p, P f_q) (dgfs_params.nyquist_filter); not the headline metric")
     return ap.parse_args()
 
 
@@ -178,7 +180,7 @@ def main():
         f_np = make_points(rcfg, xs)
     f_host = torch.from_numpy(f_np).pin_memory()
     q_host = torch.empty_like(f_host).pin_memory()
-    op = Dgfs.from_config(cfg, device=local)
+    op = Dgfs.from_config(cfg, device=local, nyquist_filter=args.nyquist_filter)
     op.reserve(nx)
     f_dev = f_host.cuda()
     q_dev = torch.empty_like(f_dev)
@@ -275,7 +277,8 @@ def main():
             "vs_baseline": value / world / PAPER_P100_PAIR_EVALS_PER_S if cfg.name == "c2" else None,
             "vs_baseline_note": "per-GPU value / 94.6 pair-evals/s: paper Table 1 (P:316), 1 x Tesla P100, same "
                                 "(N, N_rho, M) operating point, BKW workload; context, not the target",
-            "dtype": "f64", "data": "synthetic", "config": workload_desc(cfg, nx, world),
+            "dtype": "f64", "data": "synthetic",
+            "config": dict(workload_desc(cfg, nx, world), **({"variant": "nyquist_filter"} if args.nyquist_filter else {})),
             "clocks": sampler.summary(),
             "e2e": {"value": evals_per_step / (e2e_ms * 1e-3), "unit": UNIT, "ms_per_step": e2e_ms,
                     "h2d_bytes_per_step": nbytes, "d2h_bytes_per_step": nbytes,

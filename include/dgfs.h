@@ -63,6 +63,12 @@ typedef struct dgfs_params {
   const double *sigma_pre; /* [M_pre*3]                                                           */
   const double *w_pre;     /* [M_pre]                                                             */
   int device;              /* CUDA device ordinal                                                 */
+  int nyquist_filter;      /* 0 (default): Algorithm 2 as printed.  1: the operator is applied to the
+                              inputs with their three Nyquist planes (l_d = -N/2) removed,
+                              Q(P f_p, P f_q) with P = prod_d (1 - E_d), (E_d f)(c) = (-1)^{c_d} mean over
+                              c_d' of (-1)^{c_d'} f.  A different discrete operator:
+                              every shifted field is then exactly real, so the Nyquist-field kernels of
+                              the N <= 32 pipeline are not run.                                    */
 } dgfs_params;
 
 /* Algorithm 1: quadratures, truncation radius (Eq. 9), prefactors (Eq. 6) and the

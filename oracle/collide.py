@@ -47,3 +47,18 @@ def collide_pairs(tab: Tables, f: np.ndarray) -> np.ndarray:
 def collide(tab: Tables, f: np.ndarray) -> np.ndarray:
     """f[nx][ns][N^3] -> Q[nx][ns][N^3] = sum_q beta_pq Q^(pq)   (right-hand side of Eq. 1)."""
     return collide_pairs(tab, f).sum(axis=2)
+
+
+def nyquist_filter(f: np.ndarray, N: int) -> np.ndarray:
+    """P f: the samples with the three Nyquist planes of their spectrum (index N/2 along any axis, frequency
+    -N/2) set to zero.  f[..., N^3] -> same shape.  Not part of the paper's algorithm: the operator
+    Q(P f_p, P f_q) is the variant of SURVEY.md section 8(f) item 2 (`dgfs_params.nyquist_filter`), for which
+    every shifted field of Algorithm 2 is exactly real.  Written spectrally here; the CUDA path does it in
+    physical space (alternating means), so the two share no formula."""
+    shape = f.shape
+    g = np.fft.fftn(f.reshape(shape[:-1] + (N, N, N)), axes=(-3, -2, -1))
+    H = N // 2
+    g[..., H, :, :] = 0.0
+    g[..., :, H, :] = 0.0
+    g[..., :, :, H] = 0.0
+    return np.real(np.fft.ifftn(g, axes=(-3, -2, -1))).reshape(shape)

@@ -40,7 +40,7 @@ class _Params(C.Structure):
         ("prefactor", _dp), ("N", C.c_int), ("N_rho", C.c_int), ("M", C.c_int),
         ("L", C.c_double), ("R", C.c_double), ("sigma", _dp), ("w_sigma", _dp),
         ("table_mode", C.c_int), ("M_pre", C.c_int), ("sigma_pre", _dp), ("w_pre", _dp),
-        ("device", C.c_int),
+        ("device", C.c_int), ("nyquist_filter", C.c_int),
     ]
 
 
@@ -150,7 +150,7 @@ def dgfs_last_error(ctx=None):
 
 
 def dgfs_create(mass, omega, alpha, N, N_rho, M, L, kn=None, prefactor=None, R=0.0, sigma=None,
-                w_sigma=None, table_mode=0, sigma_pre=None, w_pre=None, device=0):
+                w_sigma=None, table_mode=0, sigma_pre=None, w_pre=None, device=0, nyquist_filter=False):
     """Algorithm 1 on the device.  Returns the opaque context handle."""
     lib = load_library()
     ns = len(np.asarray(mass).reshape(-1))
@@ -169,6 +169,7 @@ def dgfs_create(mass, omega, alpha, N, N_rho, M, L, kn=None, prefactor=None, R=0
     p.table_mode = int(table_mode)
     p.M_pre = 0 if w_pre is None else len(np.asarray(w_pre).reshape(-1))
     p.device = int(device)
+    p.nyquist_filter = int(bool(nyquist_filter))
     out = C.c_void_p()
     rc = lib.dgfs_create(C.byref(p), C.byref(out))
     _check(None, rc)

@@ -19,6 +19,45 @@
 
 namespace dgfs {
 
+// dgfs_params::nyquist_filter: P f = prod_d (1 - E_d) f, (E_d f)(c) = (-1)^{c_d} (1/N) sum_{c_d'} (-1)^{c_d'} f:
+// removes the spectral planes l_d = -N/2 without a transform.  One pass per axis; thread per pencil of that axis.
+// AXIS 0: stride N^2 (cx), 1: stride N (cy), 2: stride 1 (cz).
+template <int N, int AXIS>
+__global__ void __launch_bounds__(128) k_nyq_filter(const double* src, double* dst) {
+  constexpr int N2 = N * N, N3 = N2 * N;
+  const int pid = blockIdx.x * 128 + threadIdx.x;
+  if (pid >= N2) return;
+  const int a = pid / N, b = pid % N;
+  const size_t base = (size_t)blockIdx.y * N3 + (AXIS == 0 ? (size_t)a * N + b : AXIS == 1 ? (size_t)a * N2 + b : (size_t)a * N2 + (size_t)b * N);
+  constexpr size_t stride = AXIS == 0 ? N2 : AXIS == 1 ? N : 1;
+  double v[N], m = 0.0;
+#pragma unroll
+  for (int i = 0; i < N; ++i) { v[i] = src[base + i * stride]; m += (i & 1) ? -v[i] : v[i]; }
+  m *= 1.0 / N;
+#pragma unroll
+  for (int i = 0; i < N; ++i) dst[base + i * stride] = (i & 1) ? v[i] + m : v[i] - m;
+}
+
+template <int N>
+static void nyquist_filter_impl(const double* src, double* dst, int narr, cudaStream_t st) {
+  const dim3 grid((N * N + 127) / 128, narr);
+  k_nyq_filter<N, 2><<<grid, 128, 0, st>>>(src, dst);
+  k_nyq_filter<N, 1><<<grid, 128, 0, st>>>(dst, dst);
+  k_nyq_filter<N, 0><<<grid, 128, 0, st>>>(dst, dst);
+}
+
+int launch_nyquist_filter(dgfs_ctx* c, const double* src, double* dst, int narr, cudaStream_t st) {
+  switch (c->N) {
+    case 8: nyquist_filter_impl<8>(src, dst, narr, st); break;
+    case 16: nyquist_filter_impl<16>(src, dst, narr, st); break;
+    case 24: nyquist_filter_impl<24>(src, dst, narr, st); break;
+    case 32: nyquist_filter_impl<32>(src, dst, narr, st); break;
+    case 48: nyquist_filter_impl<48>(src, dst, narr, st); break;
+    default: return set_error(c, DGFS_ENOSUP, "unsupported N");
+  }
+  return DGFS_OK;
+}
+
 // ------------------------------------------------------------------ host orchestration ---------
 int ensure_workspace(dgfs_ctx* c, size_t bytes) {
   if (bytes <= c->ws_bytes) return DGFS_OK;
@@ -49,6 +88,7 @@ ChunkPlan plan_chunks(const dgfs_ctx* c, int nx) {
   pl.off_qg = off;   off += items * arr;
   pl.off_g = off;    off += nbx * g_per_point;
   pl.off_t = off;    off += items * tsl * arr;
+  pl.off_fp = off;   off += c->nyq_filter ? nbx * c->ns * (arr / 2) : 0;      // filtered inputs (real)
   pl.total = off;
   return pl;
 }
@@ -97,6 +137,11 @@ static int collide_impl(dgfs_ctx* c, const double* f, double* out, int nx, bool 
     const int nb = (nx - x0 < pl.nbx) ? nx - x0 : pl.nbx;
     const int items = nb * np;
     const double* fc = f + (size_t)x0 * ns * N3;
+    if (c->nyq_filter) {         // the operator acts on P f (dgfs_params::nyquist_filter)
+      double* fp = (double*)(ws + pl.off_fp);
+      if ((rc = launch_nyquist_filter(c, fc, fp, nb * ns, st))) return rc;
+      fc = fp;
+    }
     // S1: f^ for every species of every point of the chunk (R-2: once per species, not per pair)
     { ProfScope ps(c->prof, st, "k_zfwd_real", nb * ns * fft3 / 3.0);
       k_zfwd_real<N><<<dim3(pen_blocks, nb * ns), 128, 0, st>>>(fc, T); }

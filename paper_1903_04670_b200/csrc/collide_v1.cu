@@ -1001,7 +1001,7 @@ __global__ void __launch_bounds__(64) k_final_xy_h(DevTables tab, const cplx* __
 namespace {
 struct PlanV1 {
   int nbx;
-  size_t off_fhat, off_fhh, off_nyqy, off_qg, off_gz, off_nyq, off_s, off_t, off_tf, qstride, total;
+  size_t off_fhat, off_fhh, off_nyqy, off_qg, off_gz, off_nyq, off_s, off_t, off_tf, off_fp, nyq_bytes, qstride, total;
 };
 PlanV1 plan_v1(const dgfs_ctx* c, int nx) {
   PlanV1 pl{};
@@ -1024,13 +1024,15 @@ PlanV1 plan_v1(const dgfs_ctx* c, int nx) {
   pl.qstride = (c->any_full ? arr : half_arr) / sizeof(cplx);
   pl.off_qg = take(items * pl.qstride * sizeof(cplx));
   pl.off_gz = take(gz > g2 ? gz : g2);
-  pl.off_nyq = take(items * c->M * nyq_stride * sizeof(cplx));
+  pl.nyq_bytes = items * c->M * nyq_stride * sizeof(cplx);
+  pl.off_nyq = take(pl.nyq_bytes);
   pl.off_s = take(items * N3 * sizeof(double));
   // T: forward-transformed planes of a group of radial nodes; also the z-pass scratch of step 1
   const size_t tg = (size_t)c->v1_rgroup * items * half_arr, t1 = (size_t)nbx * c->ns * arr;
   pl.off_t = take(tg > t1 ? tg : t1);
   // Tf: per-s forward-transformed planes of the full-table pairs
   pl.off_tf = take(c->any_full ? items * c->M * arr : 0);
+  pl.off_fp = take(c->nyq_filter ? (size_t)nbx * c->ns * N3 * sizeof(double) : 0);     // filtered inputs
   pl.total = off;
   return pl;
 }
@@ -1074,7 +1076,8 @@ FlopsV1 flops_v1(const dgfs_ctx* c) {
 }  // namespace
 
 double flops_per_pair_eval_v1(const dgfs_ctx* c, int pair) {
-  const FlopsV1 f = flops_v1(c);
+  FlopsV1 f = flops_v1(c);
+  if (c->nyq_filter) f.nyq = f.wterm = 0.0;              // those kernels are not run (dgfs_params::nyquist_filter)
   if (c->full[pair]) {
     int run = 0;
     for (int s2 = 0; s2 < c->M; ++s2) run += !c->v1_sskip[(size_t)pair * c->M + s2];
@@ -1150,8 +1153,17 @@ static int collide_v1_impl(dgfs_ctx* c, const double* f, double* out, int nx, bo
   for (int x0 = 0; x0 < nx; x0 += pl.nbx) {
     const int nb = (nx - x0 < pl.nbx) ? nx - x0 : pl.nbx;
     const int items = nb * np;
-    const double* fc = f + (size_t)x0 * ns * N3;
+    const double* fc = f + (size_t)x0 * ns * N3;       // (or the filtered copy, below)
     const size_t slot_stride = (size_t)items * N2 * (H + 1);
+    if (c->nyq_filter) {
+      // dgfs_params::nyquist_filter: the operator acts on P f; every Nyquist field is then zero, so the kernels that
+      // build and multiply them are not run and their buffers are cleared once per chunk
+      double* fp = (double*)(ws + pl.off_fp);
+      if ((rc = launch_nyquist_filter(c, fc, fp, nb * ns, st))) return rc;
+      fc = fp;
+      cudaMemsetAsync(nyq, 0, pl.nyq_bytes, st);
+      cudaMemsetAsync(S, 0, (size_t)items * N3 * sizeof(double), st);
+    }
     // step 1, once per species (R-2), plus the half-packed copy
     { ProfScope ps(c->prof, st, "k_zfwd_real", nb * ns * fft3 / 3.0);
       k_zfwd_real<N><<<dim3(pen_blocks, nb * ns), 128, 0, st>>>(fc, T); }
@@ -1167,11 +1179,14 @@ static int collide_v1_impl(dgfs_ctx* c, const double* f, double* out, int nx, bo
       if (nz > nz0)
       { ProfScope ps(c->prof, st, "k_zshift", items * fl.zshift);
         k_zshift<N><<<dim3(hpen_blocks, nz - nz0, nb), 128, 0, st>>>(c->v1, ns, fhh, Gz, r, 0); }
+      if (!c->nyq_filter) {
       { ProfScope ps(c->prof, st, "k_nyq1d", nb * run_all * c->M * 16.0 * N2);
         k_nyq1d<N><<<(items * c->M + 3) / 4, 128, 0, st>>>(c->v1, c->tab, fhat, nyq, r, items * c->M); }
       { ProfScope ps(c->prof, st, "k_nyq2", nb * run_all * (fl.nyq - c->M * 16.0 * N2));
         k_nyq2<N, 2><<<dim3(3, items), 64, smem_nyq, st>>>(c->v1, c->tab, fhh, nyqy, nyq, r); }
+      }
       if (nvhs > 0) {
+        if (!c->nyq_filter)
         { ProfScope ps(c->prof, st, "k_wterm", nb * run_vhs * fl.wterm);
           k_wterm<N><<<dim3(N / WtermSmem<N>::CZB, items), WtermSmem<N>::THREADS, smem_wt, st>>>(nyq, c->M, S, c->tab.full, np, c->v1.smask, c->v1.sskip, c->v1.tsrc); }
         { ProfScope ps(c->prof, st, "k_xy", nb * (run_vhs * (fl.xy - fwd_xy) + nrun_vhs * fwd_xy));

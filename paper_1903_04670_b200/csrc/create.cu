@@ -467,6 +467,7 @@ extern "C" int dgfs_create(const dgfs_params* P, dgfs_ctx** out) {
   dgfs_ctx* c = new dgfs_ctx();
   c->device = P->device; c->ns = ns; c->npairs = np; c->N = N; c->N3 = N * N * N; c->N_rho = P->N_rho; c->M = P->M;
   c->L = P->L; c->table_mode = P->table_mode;
+  c->nyq_filter = P->nyquist_filter != 0;
   c->K2n = 3 * (N / 2) * (N / 2) + 1;
   c->mass.assign(P->mass, P->mass + ns);
   c->omega.assign(P->omega, P->omega + np);

@@ -85,6 +85,7 @@ struct dgfs_ctx {
   int ns = 0, N = 0, N_rho = 0, M = 0, npairs = 0, N3 = 0, K2n = 0;
   double L = 0, R = 0;
   int table_mode = 0;
+  bool nyq_filter = false;               // dgfs_params::nyquist_filter
   bool any_full = false;
   std::vector<double> mass, omega, alpha, kn, beta, gam, eta, rho, w_rho, sigma, w_sigma;
   std::vector<double> sigma_pre, w_pre;
@@ -148,11 +149,13 @@ int build_tables(dgfs_ctx* c);
 // collide.cu
 struct ChunkPlan {
   int nbx;                 // spatial points per chunk
-  size_t off_fhat, off_qg, off_g, off_t, total;
+  size_t off_fhat, off_qg, off_g, off_t, off_fp, total;
 };
 ChunkPlan plan_chunks(const dgfs_ctx* c, int nx);
 int run_collide(dgfs_ctx* c, const double* f, double* out, int nx, bool pairs_out, cudaStream_t st);
 int ensure_workspace(dgfs_ctx* c, size_t bytes);
+// P f = prod_d (1 - E_d) f on `narr` arrays of N^3 values (dgfs_params::nyquist_filter): src -> dst
+int launch_nyquist_filter(dgfs_ctx* c, const double* src, double* dst, int narr, cudaStream_t st);
 // collide_v1.cu
 int build_tables_v1(dgfs_ctx* c);
 void free_tables_v1(dgfs_ctx* c);

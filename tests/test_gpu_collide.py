@@ -143,6 +143,24 @@ def test_v1_antipodal_symmetry_switch(torch_cuda, monkeypatch):
     assert fl_on[0] < 0.62 * fl_off[0] and fl_on[1] == fl_off[1]          # only the diagonal pair gets cheaper
 
 
+@pytest.mark.parametrize("N,alpha,M", [(16, (1.0, 1.0), 12), (8, (1.0, 1.3), 6), (32, (1.0, 1.0), 12), (48, (1.0, 1.0), 6)])
+def test_nyquist_filter_mode(torch_cuda, N, alpha, M):
+    """dgfs_params.nyquist_filter = 1: Q(P f_p, P f_q); the oracle filters the inputs spectrally and runs
+    Algorithm 2 unchanged, the library filters in physical space and skips its Nyquist-field kernels."""
+    torch = torch_cuda
+    from oracle.collide import collide_pairs, nyquist_filter
+    cfg = _rand_cfg("t", 2, N, 2, M, alpha, (0.6, 0.8), (1.0, 2.0), seed=77 + N)
+    rng = np.random.default_rng(N)
+    f = make_points(cfg, range(cfg.nx)) * (1.0 + 0.3 * rng.uniform(-1, 1, (cfg.nx, 2, N ** 3)))
+    Qo = collide_pairs(_oracle_tables(cfg), nyquist_filter(f, N))
+    with _gpu_op(cfg, nyquist_filter=True) as op:
+        Qg = op.collide_pairs(torch.from_numpy(f).cuda()).cpu().numpy()
+    with _gpu_op(cfg) as op:
+        Qu = op.collide_pairs(torch.from_numpy(f).cuda()).cpu().numpy()
+    assert _pair_errs(Qg, Qo).max() < TOL
+    assert _pair_errs(Qu, Qo).max() > 1e-6            # the unfiltered operator is a different one on rough inputs
+
+
 def test_v1_user_sphere_rule_without_symmetry(torch_cuda):
     """A caller-supplied sigma set with no shared sigma_z values (every z shift is its own job)."""
     torch = torch_cuda

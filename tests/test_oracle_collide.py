@@ -222,3 +222,37 @@ def test_stored_golden_file_matches_oracle():
     for ent in gold["samples"]:
         x, p, q, z = ent["x"], ent["p"], ent["q"], ent["z"]
         assert abs(Qpq[x, p, q, z] - ent["Q"]) <= 1e-13 * gold["maxabs"][x][p][q]
+
+
+def test_nyquist_filter_is_the_projection_it_claims():
+    """oracle.collide.nyquist_filter (variant of SURVEY 8(f) item 2): a projection that removes exactly the
+    three Nyquist planes; equal to the separable alternating-mean form prod_d (1 - E_d); after it every
+    shifted field of Algorithm 2 is real (the reason the variant exists)."""
+    from oracle.collide import nyquist_filter
+    from oracle.tables import precompute
+    N = 8
+    rng = np.random.default_rng(3)
+    f = rng.uniform(0.1, 1.0, (2, N ** 3))
+    Pf = nyquist_filter(f, N)
+    assert np.max(np.abs(nyquist_filter(Pf, N) - Pf)) < 1e-14                      # P^2 = P
+    g = np.fft.fftn(Pf.reshape(2, N, N, N), axes=(1, 2, 3))
+    H = N // 2
+    assert max(np.abs(g[:, H]).max(), np.abs(g[:, :, H]).max(), np.abs(g[:, :, :, H]).max()) < 1e-12
+    g0 = np.fft.fftn(f.reshape(2, N, N, N), axes=(1, 2, 3))
+    keep = np.ones((N, N, N), bool); keep[H] = False; keep[:, H] = False; keep[:, :, H] = False
+    assert np.max(np.abs((g - g0)[:, keep])) < 1e-12                               # the other modes are untouched
+    # separable physical-space form: (1 - E_d) f = f - (-1)^c mean((-1)^c f) along each axis
+    h = f.reshape(2, N, N, N).copy()
+    sg = (-1.0) ** np.arange(N)
+    for ax in (1, 2, 3):
+        shp = [1, 1, 1, 1]; shp[ax] = N
+        s = sg.reshape(shp)
+        h = h - s * np.mean(s * h, axis=ax, keepdims=True)
+    assert np.max(np.abs(h.reshape(2, -1) - Pf)) < 1e-14
+    # shifted fields of filtered inputs are real
+    tab = precompute(N, 3, 6, 5.0, (1.0, 2.0), ((0.5, 0.5), (0.5, 0.5)), ((1.0, 1.0), (1.0, 1.0)))
+    FT = np.fft.fftn(Pf[0].reshape(N, N, N))
+    for r in range(3):
+        for s_ in range(6):
+            A = np.fft.ifftn(np.exp(1j * 0.4 * tab.a[r, s_].reshape(N, N, N)) * FT)
+            assert np.abs(A.imag).max() < 1e-13 * np.abs(A.real).max()
