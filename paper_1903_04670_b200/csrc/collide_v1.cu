@@ -166,7 +166,9 @@ int build_tables_v1(dgfs_ctx* c) {
   {
     const char* ap = getenv("DGFS_V1_ANTIPODAL");
     bool all = !(ap && atoi(ap) == 0);
-    std::vector<int> anti(M, -1);
+    std::vector<int>& anti = c->v1_anti;
+    anti.assign(M, -1);
+    c->v1_tpartner.assign(np, -1);
     for (int s2 = 0; s2 < M; ++s2) {
       for (int s3 = 0; s3 < M; ++s3)
         if (c->sigma[3 * s3] == -c->sigma[3 * s2] && c->sigma[3 * s3 + 1] == -c->sigma[3 * s2 + 1] &&
@@ -188,6 +190,7 @@ int build_tables_v1(dgfs_ctx* c) {
         const int pq = p * ns + q, qp = q * ns + p;
         if (!c->full[pq] || !c->full[qp]) continue;
         c->v1_tsrc[qp] = pq;
+        c->v1_tpartner[pq] = qp;
         for (int s2 = 0; s2 < M; ++s2) {
           c->v1_sskip[(size_t)qp * M + s2] = 1;
           c->v1_fsrc_s[(size_t)qp * M + s2] = anti[s2];
@@ -208,6 +211,8 @@ int build_tables_v1(dgfs_ctx* c) {
   if ((rc = upload(c, &c->d_v1_tsrc, c->v1_tsrc, "upload pair sources"))) return rc;
   if ((rc = upload(c, &c->d_v1_fsrc_s, c->v1_fsrc_s, "upload product sources"))) return rc;
   if ((rc = upload(c, &c->d_v1_fscale, c->v1_fscale, "upload product scales"))) return rc;
+  if ((rc = upload(c, &c->d_v1_anti, c->v1_anti, "upload antipodes"))) return rc;
+  if ((rc = upload(c, &c->d_v1_tpartner, c->v1_tpartner, "upload pair partners"))) return rc;
   if ((rc = upload(c, &c->d_v1_zsp, c->v1_zsp, "upload z-job species"))) return rc;
   if ((rc = upload(c, &c->d_v1_zmap, c->v1_zmap, "upload z-job map"))) return rc;
   if ((rc = upload(c, &c->d_v1_hz, hz, "upload z factors"))) return rc;
@@ -216,13 +221,13 @@ int build_tables_v1(dgfs_ctx* c) {
   if ((rc = upload(c, &c->d_v1_sxy, sxy, "upload x,y scalars"))) return rc;
   V1Tables& t = c->v1;
   t.nz = nz; t.zsp = c->d_v1_zsp; t.zmap = c->d_v1_zmap; t.hz = c->d_v1_hz; t.szv = c->d_v1_szv;
-  t.hxy = c->d_v1_hxy; t.sxy = c->d_v1_sxy; t.smask = c->d_v1_smask; t.sskip = c->d_v1_sskip; t.tsrc = c->d_v1_tsrc; t.fsrc_s = c->d_v1_fsrc_s; t.fscale = c->d_v1_fscale;
+  t.hxy = c->d_v1_hxy; t.sxy = c->d_v1_sxy; t.smask = c->d_v1_smask; t.sskip = c->d_v1_sskip; t.tsrc = c->d_v1_tsrc; t.fsrc_s = c->d_v1_fsrc_s; t.fscale = c->d_v1_fscale; t.anti = c->d_v1_anti; t.tpartner = c->d_v1_tpartner;
   return DGFS_OK;
 }
 
 void free_tables_v1(dgfs_ctx* c) {
   cudaFree(c->d_v1_zsp); cudaFree(c->d_v1_zmap); cudaFree(c->d_v1_hz); cudaFree(c->d_v1_szv);
-  cudaFree(c->d_v1_hxy); cudaFree(c->d_v1_sxy); cudaFree(c->d_v1_smask); cudaFree(c->d_v1_sskip); cudaFree(c->d_v1_tsrc); cudaFree(c->d_v1_fsrc_s); cudaFree(c->d_v1_fscale);
+  cudaFree(c->d_v1_hxy); cudaFree(c->d_v1_sxy); cudaFree(c->d_v1_smask); cudaFree(c->d_v1_sskip); cudaFree(c->d_v1_tsrc); cudaFree(c->d_v1_fsrc_s); cudaFree(c->d_v1_fscale); cudaFree(c->d_v1_anti); cudaFree(c->d_v1_tpartner);
 }
 
 // ---------------------------------------------------------------- device code -------------------
@@ -747,9 +752,14 @@ __global__ void __launch_bounds__(32 * W) k_xy_full(V1Tables t, DevTables tab, c
   }
 }
 
-// Forward z pass and steps 7-8 of a full-table pair for one radial node:
-//   QG[item][kz][kx][ky] (+)= w_r sum_s b_rs(k) fft_z( Tf[item][s][.][kx][ky] );  thread pair per pencil as in
-// k_zfwd_acc, the sum over s stays in registers.  b is read in SPEC layout [r][s][kz][kx][ky].
+// Forward z pass and steps 7-8 of the full-table pairs for one radial node, driven by the products that
+// were actually computed: block (pencils, SOURCE item).  For every sphere point s the source pair ran,
+//   u = fft_z( Tf[item][s][.][kx][ky] )  once, then
+//   QG[item]          += w_r b^(pq)_rs  u                      its own term
+//   QG[item]          += w_r f b^(pq)_rs' u                    same-species pair: the antipode s' it stands for (R-10)
+//   QG[partner item]  += w_r f b^(qp)_rs' u                    the transposed pair, which ran nothing (R-11)
+// with f = fscale of the target (ratio of sphere weights).  Thread pair per pencil as in k_zfwd_acc; the sums
+// over s stay in registers.  b is read in SPEC layout [r][s][kz][kx][ky].
 template <int N, bool FIRST>
 __global__ void __launch_bounds__(256) k_zfwd_full(DevTables tab, V1Tables t, const cplx* __restrict__ Tf,
                                                    cplx* __restrict__ QG, size_t qstride, int r) {
@@ -757,15 +767,17 @@ __global__ void __launch_bounds__(256) k_zfwd_full(DevTables tab, V1Tables t, co
   const int par = threadIdx.x >> 7;
   const int pid = blockIdx.x * 128 + (threadIdx.x & 127);
   const int item = blockIdx.y, pair = item % tab.npairs;
-  if (pid >= N2 || !tab.full[pair]) return;
+  if (pid >= N2 || !tab.full[pair] || t.tsrc[pair] != pair) return;
+  const int M = tab.M;
+  const int partner = t.tpartner[pair];                 // pair that reads this one's products, or -1
+  const unsigned char* skip = t.sskip + (size_t)pair * M;
   const double scale = tab.w_rho[r];
-  cplx acc[H];
+  cplx acc[H], acc2[H];
 #pragma unroll
-  for (int k = 0; k < H; ++k) acc[k] = make_double2(0.0, 0.0);
-  for (int s = 0; s < tab.M; ++s) {
-    // the transformed product of (pair, s): its own, or the one it shares (R-10 / R-11)
-    const cplx* src = Tf + ((size_t)(item - pair + t.tsrc[pair]) * tab.M + t.fsrc_s[(size_t)pair * tab.M + s]) * N3 + pid;
-    const double fs = t.fscale[(size_t)pair * tab.M + s];
+  for (int k = 0; k < H; ++k) acc[k] = acc2[k] = make_double2(0.0, 0.0);
+  for (int s = 0; s < M; ++s) {
+    if (skip[s]) continue;
+    const cplx* src = Tf + ((size_t)item * M + s) * N3 + pid;
     cplx u[H];
     if (par == 0) {
 #pragma unroll
@@ -775,19 +787,34 @@ __global__ void __launch_bounds__(256) k_zfwd_full(DevTables tab, V1Tables t, co
       for (int j = 0; j < H; ++j) u[j] = twiddle_mul<N, -1>(csub(src[(size_t)j * N2], src[(size_t)(j + H) * N2]), j);
     }
     fft_reg<H, -1>(u);
-    const cplx* bf = tab.bfull[pair] + ((size_t)r * tab.M + s) * N3 + pid;
+    const int sa = t.anti[s];
+    const cplx* bf = tab.bfull[pair] + ((size_t)r * M + s) * N3 + pid;
+    // same-species pair: s also stands for its antipode
+    const bool twin = sa >= 0 && skip[sa] && t.fsrc_s[(size_t)pair * M + sa] == s;
+    const cplx* bt = twin ? tab.bfull[pair] + ((size_t)r * M + sa) * N3 + pid : nullptr;
+    const double ft = twin ? t.fscale[(size_t)pair * M + sa] : 0.0;
+    const cplx* bp = (partner >= 0) ? tab.bfull[partner] + ((size_t)r * M + sa) * N3 + pid : nullptr;
+    const double fp = (partner >= 0) ? t.fscale[(size_t)partner * M + sa] : 0.0;
 #pragma unroll
     for (int k = 0; k < H; ++k) {
-      const cplx b = bf[(size_t)(2 * k + par) * N2];
-      acc[k] = cfma(make_double2(fs * b.x, fs * b.y), u[k], acc[k]);
+      const size_t o = (size_t)(2 * k + par) * N2;
+      cplx b = bf[o];
+      if (twin) { const cplx b2 = bt[o]; b.x = fma(ft, b2.x, b.x); b.y = fma(ft, b2.y, b.y); }
+      acc[k] = cfma(b, u[k], acc[k]);
+      if (partner >= 0) { const cplx b3 = bp[o]; acc2[k] = cfma(make_double2(fp * b3.x, fp * b3.y), u[k], acc2[k]); }
     }
   }
   cplx* dst = QG + (size_t)item * qstride + pid;
+  cplx* dst2 = QG + (size_t)(item - pair + (partner >= 0 ? partner : pair)) * qstride + pid;
 #pragma unroll
   for (int k = 0; k < H; ++k) {
-    cplx* d = dst + (size_t)(2 * k + par) * N2;
-    const cplx o = FIRST ? make_double2(0.0, 0.0) : *d;
-    *d = make_double2(fma(scale, acc[k].x, o.x), fma(scale, acc[k].y, o.y));
+    const size_t o = (size_t)(2 * k + par) * N2;
+    const cplx q1 = FIRST ? make_double2(0.0, 0.0) : dst[o];
+    dst[o] = make_double2(fma(scale, acc[k].x, q1.x), fma(scale, acc[k].y, q1.y));
+    if (partner >= 0) {
+      const cplx q2 = FIRST ? make_double2(0.0, 0.0) : dst2[o];
+      dst2[o] = make_double2(fma(scale, acc2[k].x, q2.x), fma(scale, acc2[k].y, q2.y));
+    }
   }
 }
 

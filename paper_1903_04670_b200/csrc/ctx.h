@@ -114,9 +114,9 @@ struct dgfs_ctx {
   int v1_chunk = 512;                    // spatial points per launch group (large launches amortise the tails)
   int v1_rgroup = 16;                    // radial nodes per forward-z / QG accumulation launch
   int v1_nz = 0, v1_nz0 = 0;             // z jobs; the last v1_nz0 of them have sigma_z = 0
-  std::vector<int> v1_zsp, v1_zmap, v1_tsrc, v1_fsrc_s;
+  std::vector<int> v1_zsp, v1_zmap, v1_tsrc, v1_fsrc_s, v1_anti, v1_tpartner;
   std::vector<double> v1_fscale;
-  int *d_v1_zsp = nullptr, *d_v1_zmap = nullptr, *d_v1_tsrc = nullptr, *d_v1_fsrc_s = nullptr;
+  int *d_v1_zsp = nullptr, *d_v1_zmap = nullptr, *d_v1_tsrc = nullptr, *d_v1_fsrc_s = nullptr, *d_v1_anti = nullptr, *d_v1_tpartner = nullptr;
   double* d_v1_fscale = nullptr;
   dgfs::cplx *d_v1_hz = nullptr, *d_v1_hxy = nullptr;
   double *d_v1_szv = nullptr, *d_v1_sxy = nullptr;

@@ -20,6 +20,8 @@ struct V1Tables {
   const cplx* hxy;           // [pair][r][s][side][2][N]   x factors then y factors
   const double* sxy;         // [pair][r][s][side][2]      anti-Hermitian x, y scalars
   const int* tsrc;           // [pair]  pair whose S_r (buffer T) this pair uses: itself, or its transpose (q,p) -> (p,q) (R-11)
+  const int* anti;           // [s]     antipode of sphere point s, or -1
+  const int* tpartner;       // [pair]  full-table pair whose products this pair also serves (its transpose), or -1
   const int* fsrc_s;         // [pair][s]  full-table pairs: sphere point whose transformed product P_s (buffer Tf of pair
                              //            tsrc[pair]) equals this one's up to the factor fscale (R-10 / R-11)
   const double* fscale;      // [pair][s]
