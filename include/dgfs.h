@@ -158,6 +158,10 @@ typedef struct dgfs_mesh1d {
  * f: device, [ne][K][ns][N^3], updated in place. */
 int dgfs_step(dgfs_ctx *c, const dgfs_mesh1d *mesh, double *f, double dt, int nsteps, void *stream);
 
+/* nsteps forward-Euler steps f <- f + dt L(f) of the same equation (the time stepping of the paper's
+ * Couette case, Table 2).  Same arguments, layout and error behaviour as dgfs_step. */
+int dgfs_step_euler(dgfs_ctx *c, const dgfs_mesh1d *mesh, double *f, double dt, int nsteps, void *stream);
+
 /* The spatial right-hand side alone (verification of D1-D3): rhs = -c_x d/dx f with upwind
  * fluxes and diffuse walls, no collisions.  f, rhs: device, [ne][K][ns][N^3]. */
 int dgfs_advect_rhs(dgfs_ctx *c, const dgfs_mesh1d *mesh, const double *f, double *rhs, void *stream);

@@ -109,8 +109,13 @@ def advect_rhs(mesh: Mesh1D, f: np.ndarray, N: int, L: float, mass) -> np.ndarra
     return rhs
 
 
-def step(mesh: Mesh1D, f: np.ndarray, dt: float, nsteps: int, N: int, L: float, mass, collide=None) -> np.ndarray:
-    """nsteps SSP-RK3 steps.  collide(g[nx][ns][N^3]) -> Q[nx][ns][N^3] or None (free transport)."""
+def step(mesh: Mesh1D, f: np.ndarray, dt: float, nsteps: int, N: int, L: float, mass, collide=None,
+         scheme: str = "rk3") -> np.ndarray:
+    """nsteps steps of SSP-RK3 (scheme "rk3", reading DG-3) or of forward Euler (scheme "euler", the time
+    stepping of the paper's Couette case, Table 2).
+    collide(g[nx][ns][N^3]) -> Q[nx][ns][N^3] or None (free transport)."""
+    if scheme not in ("rk3", "euler"):
+        raise ValueError("scheme must be 'rk3' or 'euler'")
     ne, K, ns, N3 = f.shape
 
     def Lop(u):
@@ -121,6 +126,9 @@ def step(mesh: Mesh1D, f: np.ndarray, dt: float, nsteps: int, N: int, L: float, 
 
     u = f.copy()
     for _ in range(nsteps):
+        if scheme == "euler":
+            u = u + dt * Lop(u)
+            continue
         u1 = u + dt * Lop(u)
         u2 = 0.75 * u + 0.25 * (u1 + dt * Lop(u1))
         u = u / 3.0 + (2.0 / 3.0) * (u2 + dt * Lop(u2))

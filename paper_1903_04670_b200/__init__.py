@@ -6,7 +6,7 @@ and streams.  There is no CPU fallback: importing works anywhere (so the ABI can
 but creating a context without the built library or without a CUDA device raises.
 """
 from .api import (DgfsError, Dgfs, Mesh1D, load_library, library_path, exported_symbols,
-                  dgfs_create, dgfs_collide, dgfs_collide_pairs, dgfs_step, dgfs_advect_rhs,
+                  dgfs_create, dgfs_collide, dgfs_collide_pairs, dgfs_step, dgfs_step_euler, dgfs_advect_rhs,
                   dgfs_destroy, dgfs_reserve, dgfs_workspace_bytes, dgfs_get_quadrature,
                   dgfs_get_tables, dgfs_flops_per_pair_eval, dgfs_last_error,
                   dgfs_launch_count, dgfs_profile_enable, dgfs_profile_count, dgfs_profile_get,
@@ -15,7 +15,7 @@ from . import api
 
 __all__ = [
     "DgfsError", "Dgfs", "Mesh1D", "load_library", "library_path", "exported_symbols",
-    "dgfs_create", "dgfs_collide", "dgfs_collide_pairs", "dgfs_step", "dgfs_advect_rhs",
+    "dgfs_create", "dgfs_collide", "dgfs_collide_pairs", "dgfs_step", "dgfs_step_euler", "dgfs_advect_rhs",
     "dgfs_destroy", "dgfs_reserve", "dgfs_workspace_bytes", "dgfs_get_quadrature",
     "dgfs_get_tables", "dgfs_flops_per_pair_eval", "dgfs_last_error",
     "dgfs_launch_count", "dgfs_profile_enable", "dgfs_profile_count", "dgfs_profile_get",

@@ -17,7 +17,7 @@ _lib = None
 ABI_SYMBOLS = (
     "dgfs_create", "dgfs_destroy", "dgfs_last_error", "dgfs_collide", "dgfs_collide_pairs",
     "dgfs_workspace_bytes", "dgfs_reserve", "dgfs_get_quadrature", "dgfs_get_tables",
-    "dgfs_flops_per_pair_eval", "dgfs_step", "dgfs_advect_rhs",
+    "dgfs_flops_per_pair_eval", "dgfs_step", "dgfs_step_euler", "dgfs_advect_rhs",
     "dgfs_launch_count", "dgfs_profile_enable", "dgfs_profile_count", "dgfs_profile_get",
     "dgfs_profile_reset", "dgfs_collide_host", "dgfs_measure_fp64_peak",
 )
@@ -117,6 +117,8 @@ def load_library():
     lib.dgfs_profile_reset.restype = ip
     lib.dgfs_step.argtypes = [vp, C.POINTER(_Mesh), vp, C.c_double, ip, vp]
     lib.dgfs_step.restype = ip
+    lib.dgfs_step_euler.argtypes = [vp, C.POINTER(_Mesh), vp, C.c_double, ip, vp]
+    lib.dgfs_step_euler.restype = ip
     lib.dgfs_advect_rhs.argtypes = [vp, C.POINTER(_Mesh), vp, vp, vp]
     lib.dgfs_advect_rhs.restype = ip
     _lib = lib
@@ -288,6 +290,11 @@ def dgfs_step(ctx, mesh, f, dt, nsteps):
     _check(ctx, load_library().dgfs_step(ctx, C.byref(m), _dev(f, "f"), float(dt), int(nsteps), _stream_ptr()))
 
 
+def dgfs_step_euler(ctx, mesh, f, dt, nsteps):
+    m = mesh._c()
+    _check(ctx, load_library().dgfs_step_euler(ctx, C.byref(m), _dev(f, "f"), float(dt), int(nsteps), _stream_ptr()))
+
+
 def dgfs_advect_rhs(ctx, mesh, f, rhs):
     m = mesh._c()
     _check(ctx, load_library().dgfs_advect_rhs(ctx, C.byref(m), _dev(f, "f"), _dev(rhs, "rhs"), _stream_ptr()))
@@ -304,6 +311,8 @@ class Dgfs:
 
     @classmethod
     def from_config(cls, cfg, **kw):
+        if getattr(cfg, "kn", ()):
+            kw.setdefault("kn", cfg.kn)
         return cls(cfg.mass, cfg.omega, cfg.alpha, cfg.N, cfg.N_rho, cfg.M, cfg.L, **kw)
 
     def close(self):

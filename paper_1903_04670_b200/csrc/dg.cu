@@ -230,6 +230,33 @@ extern "C" int dgfs_advect_rhs(dgfs_ctx* c, const dgfs_mesh1d* mesh, const doubl
   return check_cuda(c, cudaGetLastError(), "dgfs_advect_rhs launch");
 }
 
+// Forward Euler (the time stepping of the paper's Couette case, Table 2): f <- f + dt L(f).  One stage
+// kernel per step (a = 0, b = 1); the stage reads the neighbour traces of its input, so it cannot run in place:
+// f and the scratch state w1 alternate, with one device copy at the end when nsteps is odd.
+extern "C" int dgfs_step_euler(dgfs_ctx* c, const dgfs_mesh1d* mesh, double* f, double dt, int nsteps, void* stream) {
+  if (!c) return DGFS_EINVAL;
+  if (!f) return set_error(c, DGFS_EINVAL, "dgfs_step_euler: f must not be NULL");
+  if (nsteps < 0) return set_error(c, DGFS_EINVAL, "dgfs_step_euler: nsteps must be >= 0");
+  if (!(dt > 0) || !std::isfinite(dt)) return set_error(c, DGFS_EINVAL, "dgfs_step_euler: dt must be positive");
+  cudaStream_t st = (cudaStream_t)stream;
+  DgOps ops; DgBuffers B;
+  int rc = dg_setup(c, mesh, "dgfs_step_euler", &ops, &B, st);
+  if (rc) return rc;
+  const int ne = mesh->ne, ns = c->ns, nx = ne * ops.K;
+  const double jac = 2.0 * ne / (mesh->x1 - mesh->x0);
+  const size_t bytes = (size_t)nx * ns * c->N * c->N * c->N * sizeof(double);
+  double* u = f;
+  double* v = B.w1;
+  for (int n = 0; n < nsteps; ++n) {
+    k_dg_wall<<<2 * ns, 256, 0, st>>>(u, B.Wt, B.nw, ne, ops.K, ns, c->N, c->L);
+    if ((rc = run_collide(c, u, B.Qb, nx, false, st))) return rc;                    // sum_q beta_pq Q^(pq), Eq. 1
+    stage(ops, u, u, B.Qb, v, B.Wt, B.nw, ne, ns, c->N, c->L, jac, dt, 0.0, 1.0, st);
+    double* t = u; u = v; v = t;
+  }
+  if (u != f && (rc = check_cuda(c, cudaMemcpyAsync(f, u, bytes, cudaMemcpyDeviceToDevice, st), "dgfs_step_euler copy"))) return rc;
+  return check_cuda(c, cudaGetLastError(), "dgfs_step_euler launch");
+}
+
 extern "C" int dgfs_step(dgfs_ctx* c, const dgfs_mesh1d* mesh, double* f, double dt, int nsteps, void* stream) {
   if (!c) return DGFS_EINVAL;
   if (!f) return set_error(c, DGFS_EINVAL, "dgfs_step: f must not be NULL");

@@ -107,3 +107,41 @@ def test_step_c3_one_step_sampled_elements(torch_cuda):
         api.dgfs_step(op.ctx, Mesh1D(cfg.ne, cfg.order, wall_T=cfg.wall_T), fd, cfg.dt, 1)
         fg = fd[:1].cpu().numpy()
     assert np.max(np.abs(fg[0] - fo[0])) < 1e-10 * np.max(np.abs(fo[0]))
+
+
+def test_couette_c01_euler_step(torch_cuda):
+    """Second workload: the paper's Couette case C-01 (Table 2: Ar-Kr-like
+    masses, all four pairs VSS, printed Knudsen numbers, walls moving at -+50 m/s, 4 elements of order 3, 32^3,
+    N_rho = 8, M = 12, forward Euler).  One Euler step of the whole slab against the oracle (all 16 nodes, both
+    walls), and nsteps = 2 in one call bit-equal to two calls of one step (odd / even buffer parity of the
+    Euler ping-pong)."""
+    torch = torch_cuda
+    from oracle import dg
+    from oracle.tables import precompute
+    from oracle.collide import collide
+    from paper_1903_04670_b200 import Dgfs, Mesh1D, api
+    cfg = get_config("couette")
+    f = make_dg_state(cfg)
+    tab = precompute(cfg.N, cfg.N_rho, cfg.M, cfg.L, cfg.mass, cfg.omega, cfg.alpha, kn=cfg.kn)
+    omesh = dg.Mesh1D(cfg.ne, cfg.order, wall_T=cfg.wall_T, wall_u=cfg.wall_u)
+    fo = dg.step(omesh, f, cfg.dt, 1, cfg.N, cfg.L, cfg.mass, collide=lambda g: collide(tab, g), scheme="euler")
+    mesh = Mesh1D(cfg.ne, cfg.order, wall_T=cfg.wall_T, wall_u=cfg.wall_u)
+    with Dgfs.from_config(cfg, device=0) as op:
+        fd = torch.from_numpy(f).cuda()
+        api.dgfs_step_euler(op.ctx, mesh, fd, cfg.dt, 1)
+        f1 = fd.cpu().numpy()
+        api.dgfs_step_euler(op.ctx, mesh, fd, cfg.dt, 1)
+        f2 = fd.clone()
+        fe = torch.from_numpy(f).cuda()
+        api.dgfs_step_euler(op.ctx, mesh, fe, cfg.dt, 2)
+        assert torch.equal(fe, f2)
+        api.dgfs_step_euler(op.ctx, mesh, fe, cfg.dt, 0)                     # no-op
+        assert torch.equal(fe, f2)
+        with pytest.raises(api.DgfsError):
+            api.dgfs_step_euler(op.ctx, mesh, fe, -1.0, 1)
+    assert np.max(np.abs(f1 - fo)) < 1e-10 * np.max(np.abs(fo))
+    # the step did something: the gas at the wall nodes picked up y momentum of the sign of its wall's velocity
+    c = -cfg.L + (np.arange(cfg.N) + 0.5) * 2.0 * cfg.L / cfg.N
+    cy = np.broadcast_to(c[None, :, None], (cfg.N,) * 3).reshape(-1)
+    for p in range(cfg.ns):
+        assert (f1[0, 0, p] * cy).sum() < 0.0 < (f1[-1, -1, p] * cy).sum()

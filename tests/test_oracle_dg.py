@@ -126,3 +126,35 @@ def test_rk3_is_third_order_in_time_on_a_linear_ode():
         u = dg.step(mesh, f, 1.0 / n, n, N, L, (1.0,), collide=lambda g: lam * g)
         errs.append(np.abs(u - np.exp(lam) * f).max() / np.abs(f).max())
     assert 6.5 < errs[0] / errs[1] < 9.5, errs
+
+
+def test_euler_scheme_is_the_closed_form_on_a_linear_ode():
+    """Same set-up with scheme "euler": n steps of size h on f' = lam f give (1 + h lam)^n f exactly (closed
+    form, not a restatement of the update), and the error against e^{lam} halves with the step (first order)."""
+    N, L = 4, 4.0
+    mesh = dg.Mesh1D(1, 1, wall_T=(1.0, 1.0))
+    f = np.empty((1, 2, 1, N ** 3))
+    f[:] = dg.wall_maxwellian(N, L, (0, 0, 0), 1.0, 1.0)
+    lam = -1.3
+    errs = []
+    for n in (16, 32):
+        u = dg.step(mesh, f, 1.0 / n, n, N, L, (1.0,), collide=lambda g: lam * g, scheme="euler")
+        assert np.abs(u - (1.0 + lam / n) ** n * f).max() < 1e-13 * np.abs(f).max()
+        errs.append(np.abs(u - np.exp(lam) * f).max() / np.abs(f).max())
+    assert 1.8 < errs[0] / errs[1] < 2.2, errs
+    with pytest.raises(ValueError):
+        dg.step(mesh, f, 0.1, 1, N, L, (1.0,), scheme="rk4")
+
+
+def test_euler_step_is_f_plus_dt_rhs():
+    """One Euler step of free transport on rough data equals f + dt advect_rhs(f) (ties scheme "euler" to the
+    pinned right-hand side)."""
+    rng = np.random.default_rng(5)
+    N, L = 4, 4.0
+    mesh = dg.Mesh1D(3, 2, wall_T=(0.9, 1.1), wall_u=((0, 0.1, 0), (0, -0.1, 0)))
+    f = np.empty((3, 3, 2, N ** 3))
+    for p, m in enumerate((1.0, 2.0)):
+        f[:, :, p] = dg.wall_maxwellian(N, L, (0, 0, 0), 1.0, m)
+    f *= 1.0 + 0.3 * rng.uniform(-1, 1, f.shape)
+    u = dg.step(mesh, f, 1e-2, 1, N, L, (1.0, 2.0), scheme="euler")
+    assert np.array_equal(u, f + 1e-2 * dg.advect_rhs(mesh, f, N, L, (1.0, 2.0)))

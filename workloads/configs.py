@@ -26,6 +26,10 @@ class Config:
     nsteps: int = 0
     wall_T: Tuple[float, float] = (1.0, 1.0)
     density: Tuple[float, ...] = field(default_factory=tuple)
+    # Couette case only
+    wall_u: Tuple[Tuple[float, float, float], Tuple[float, float, float]] = ((0.0, 0.0, 0.0), (0.0, 0.0, 0.0))
+    kn: Tuple[Tuple[float, ...], ...] = ()    # [ns][ns] Knudsen numbers (Eq. 5); () = all 1
+    scheme: str = "rk3"                       # time stepping of the DG cases: "rk3" | "euler"
 
     @property
     def ns(self) -> int:
@@ -60,6 +64,19 @@ CONFIGS = {
     # configs[4]: stress case
     "c4": Config("c4", 190304674, (1.0, 4.0), _full(0.5, 2), _full(1.0, 2),
                  N=48, L=7.0, N_rho=48, M=32, nx=2048, kind="bimaxwell"),
+    # Second workload: the paper's Couette case C-01, Table 2, in the
+    # paper's units (m_0 = 66.3e-27 kg, u_0 = 337.2 m/s, T_0 = 273 K, n_0 = 1.680e21 m^-3, H_0 = 1 mm): masses
+    # {66.3, 139.1}e-27 kg, VSS with the printed omega / alpha, Knudsen numbers as printed, walls at
+    # y velocity -+50 m/s and 273 K, gas initially at rest at 273 K with n = {1.680e21, 8.009e20} m^-3, 4 elements
+    # of order 3, 32^3 velocity grid on [-7, 7]^3, N_rho = 8, M = 12, forward Euler.  The paper does not print its
+    # time step: dt is this repository's choice.
+    "couette": Config("couette", 190304675, (1.0, 139.1 / 66.3), ((0.81, 0.805), (0.805, 0.80)),
+                      ((1.4, 1.36), (1.36, 1.32)),
+                      N=32, L=7.0, N_rho=8, M=12, nx=16, kind="couette",
+                      ne=4, order=3, dt=1.0e-3, nsteps=100, wall_T=(1.0, 1.0),
+                      density=(1.0, 8.009e20 / 1.680e21),
+                      wall_u=((0.0, -50.0 / 337.2, 0.0), (0.0, 50.0 / 337.2, 0.0)),
+                      kn=((0.793, 0.803), (0.555, 0.606)), scheme="euler"),
 }
 
 

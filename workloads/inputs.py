@@ -92,7 +92,7 @@ def make_points(cfg: Config, xs) -> np.ndarray:
 
 
 def make_dg_state(cfg: Config) -> np.ndarray:
-    """c3 initial state f[ne][K][ns][N^3], K = order+1 nodes per element (reading DG-4):
+    """Initial state of the DG cases, f[ne][K][ns][N^3], K = order+1 nodes per element.  c3 (reading DG-4):
     f_p = n_p (1 + 0.05 xi_{e,p}) Maxw(1, 0, 1; m_p), xi ~ U[-1,1] per (element, species),
     the same value at every node of the element."""
     K = cfg.order + 1
@@ -100,6 +100,8 @@ def make_dg_state(cfg: Config) -> np.ndarray:
     for e in range(cfg.ne):
         for p in range(cfg.ns):
             xi = 2.0 * float(splitmix64_uniform(cfg.seed, [e * cfg.ns + p])[0]) - 1.0
+            if cfg.kind == "couette":
+                xi = 0.0                       # Table 2: uniform gas at rest, T = T_0
             fp = maxwellian(cfg.N, cfg.L, cfg.density[p] * (1.0 + 0.05 * xi), (0.0, 0.0, 0.0), 1.0,
                             cfg.mass[p])
             out[e, :, p, :] = fp[None, :]
