@@ -5,7 +5,9 @@
 // inverse kernel e^{+2 pi i jk/N}; both UNNORMALISED (the 1/N^3 factors are folded into the tables).
 //
 // Decimation in time, radix 4 / 2 / 3 chosen at compile time; all indices are compile-time constants
-// after unrolling, so arrays live in registers and twiddles become literal operands.
+// after unrolling, so arrays live in registers and twiddles become literal operands.  Radix-2 and radix-4
+// butterflies are in multiply-add form (twiddle_pm): 24 instead of 28 FP64 instructions per general radix-4
+// butterfly, 392 instead of 432 per 32-point transform.
 #pragma once
 #include <cuda_runtime.h>
 #include "twiddle96.h"
@@ -52,6 +54,39 @@ __host__ __device__ __forceinline__ cplx twiddle_mul(cplx x, int k) {
   return make_double2(x.x * c - x.y * s, x.x * s + x.y * c);
 }
 
+// p = a + w x, m = a - w x with w = e^{DIR * 2 pi i k / N}, k known at compile time.  The product is never formed:
+// with t = Im w / Re w (or its inverse when |Re w| < |Im w|, so that |t| <= 1),
+//   w x = Re w * (x.re - t x.im, x.im + t x.re),
+// which takes two FMAs, and each of the four outputs one more: 6 instructions instead of 4 (product) + 4 (sums).
+template <int N, int DIR>
+__host__ __device__ __forceinline__ void twiddle_pm(cplx a, cplx x, int k, cplx& p, cplx& m) {
+  static_assert(96 % N == 0, "N must divide 96");
+  const int k96 = ((k * (96 / N)) % 96 + 96) % 96;
+  if (k96 == 0) { p = cadd(a, x); m = csub(a, x); return; }
+  if (k96 == 48) { p = csub(a, x); m = cadd(a, x); return; }
+  if (k96 == 24 || k96 == 72) {                          // w = +-i
+    const bool plus = (k96 == 24) == (DIR > 0);          // w = +i
+    const cplx u = make_double2(a.x - x.y, a.y + x.x), v = make_double2(a.x + x.y, a.y - x.x);
+    p = plus ? u : v;
+    m = plus ? v : u;
+    return;
+  }
+  const double c = cos96(k96);
+  const double s = (DIR > 0) ? sin96(k96) : -sin96(k96);
+  const bool big_c = (c < 0 ? -c : c) >= (s < 0 ? -s : s);
+  if (big_c) {
+    const double t = s / c;
+    const cplx xt = make_double2(fma(-t, x.y, x.x), fma(t, x.x, x.y));
+    p = make_double2(fma(c, xt.x, a.x), fma(c, xt.y, a.y));
+    m = make_double2(fma(-c, xt.x, a.x), fma(-c, xt.y, a.y));
+  } else {
+    const double t = c / s;
+    const cplx xt = make_double2(fma(t, x.x, -x.y), fma(t, x.y, x.x));
+    p = make_double2(fma(s, xt.x, a.x), fma(s, xt.y, a.y));
+    m = make_double2(fma(-s, xt.x, a.x), fma(-s, xt.y, a.y));
+  }
+}
+
 // out[0..N) = DFT_N of in[0], in[IS], ..., in[(N-1) IS]
 template <int N, int DIR, int IS>
 struct RegFFT {
@@ -65,21 +100,15 @@ struct RegFFT {
 #pragma unroll
     for (int k = 0; k < M; ++k) {
       if (R == 2) {
-        cplx a = t[0][k], b = twiddle_mul<N, DIR>(t[1][k], k);
-        out[k] = cadd(a, b);
-        out[k + M] = csub(a, b);
+        twiddle_pm<N, DIR>(t[0][k], t[1][k], k, out[k], out[k + M]);
       } else if (R == 4) {
-        cplx a = t[0][k];
-        cplx b = twiddle_mul<N, DIR>(t[1][k], k);
-        cplx c = twiddle_mul<N, DIR>(t[2][k], 2 * k);
-        cplx d = twiddle_mul<N, DIR>(t[3][k], 3 * k);
-        cplx ac0 = cadd(a, c), ac1 = csub(a, c), bd0 = cadd(b, d), bd1 = csub(b, d);
-        // multiply bd1 by DIR * i
-        cplx ibd1 = (DIR > 0) ? make_double2(-bd1.y, bd1.x) : make_double2(bd1.y, -bd1.x);
-        out[k] = cadd(ac0, bd0);
-        out[k + M] = cadd(ac1, ibd1);
-        out[k + 2 * M] = csub(ac0, bd0);
-        out[k + 3 * M] = csub(ac1, ibd1);
+        // w^{3k} d = w^k (w^{2k} d): both pairs take the twiddle w^{2k} first, then w^k (and w^k times DIR * i,
+        // i.e. w^{k + N/4}, for the odd outputs); every product is folded into the sums (twiddle_pm)
+        cplx ac0, ac1, e0, e1;
+        twiddle_pm<N, DIR>(t[0][k], t[2][k], 2 * k, ac0, ac1);         // a +- w^{2k} c
+        twiddle_pm<N, DIR>(t[1][k], t[3][k], 2 * k, e0, e1);           // b +- w^{2k} d
+        twiddle_pm<N, DIR>(ac0, e0, k, out[k], out[k + 2 * M]);
+        twiddle_pm<N, DIR>(ac1, e1, k + N / 4, out[k + M], out[k + 3 * M]);
       } else {  // R == 3
         cplx a = t[0][k];
         cplx b = twiddle_mul<N, DIR>(t[1][k], k);
