@@ -481,13 +481,15 @@ __global__ void __launch_bounds__(32 * NW) k_nyq2(V1Tables t, DevTables tab, con
     if (which == 0) return t.szv[(size_t)r * t.nz + zm[2 * s + side]];
     return sbase[s * 4 + side * 2 + (which == 1 ? 0 : 1)];
   };
-  // fields of an axis with sigma_{s,d} = 0 vanish identically (v1_tables.h): write zeros, run no job
+  // fields of an axis with sigma_{s,d} = 0 vanish identically (v1_tables.h): run no job; zeros are stored only for
+  // pairs with a full table (k_xy_full reads all three fields; k_wterm skips the masked ones)
+  const bool store_zeros = tab.full[pair] != 0;
   const int zbit = (which == 0) ? 4 : (which == 1 ? 1 : 2);
   const int ooff = (which == 0) ? NL::UZ : (which == 1 ? NL::UXP : NL::UY);
   auto next_job = [&](int s) {                   // first s' >= s in this warp's sequence with a job to run
     const unsigned char* skip = t.sskip + (size_t)pair * tab.M;
     while (s < tab.M && ((t.smask[s] & zbit) || skip[s])) {
-      if (act && !skip[s]) {
+      if (act && !skip[s] && store_zeros) {
         cplx* out = nyq + ((size_t)item * tab.M + s) * NL::STRIDE + ooff;
 #pragma unroll
         for (int j = 0; j < N; ++j) out[j * N + ln] = make_double2(0.0, 0.0);
