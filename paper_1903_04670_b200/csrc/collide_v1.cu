@@ -822,22 +822,23 @@ __global__ void __launch_bounds__(256) k_zfwd_full(DevTables tab, V1Tables t, co
 
 // S(c) = -sum_s Re W_s(c) Im W_s(c),  W_s(c) = (-1)^cx ux'_s(cy,cz) + (-1)^cy uy_s(cx,cz) + (-1)^cz uz_s(cx,cy)
 // (W = a_i + i b_i, file header).  This kernel is bound by the L2 -> SM traffic of its tables (150 KB per
-// (item, s) if every byte is fetched once, for 5 FP64 instructions per node), so a block covers as many cz
-// planes as its registers allow: 16 (two groups of 256 threads with 8 planes each; 8 when 16 does not divide
-// N), and the uz plane is fetched once per block.  Thread = 2 x 2 tile of (cx, cy): every table element
+// (item, s) if every byte is fetched once, for 5 FP64 instructions per node).  A block of 256 threads covers 8 cz
+// planes and fetches the uz plane once; two blocks per SM (four-stage ring, 99 KB each at N = 32) overlap one
+// block's pipeline fill and its store of S with the other's arithmetic, which is worth more than the halved uz
+// traffic of 16-plane blocks that fill the SM alone (measured: 102 against 107 ms per step of c2).  Thread = 2 x 2 tile of (cx, cy): every table element
 // serves several nodes and all signs are compile-time constants.  The tables of one s (uz plane, rows of
 // ux' and uy) are staged in shared memory by cp.async, a ring of five stages over s; uz and uy are stored
 // de-interleaved by the parity of cx so that the pair loads are conflict-free.
 template <int N>
 struct WtermSmem {
-  static constexpr int CZG = 8, NH = (N % 16 == 0) ? 2 : 1, CZB = CZG * NH, THREADS = 256 * NH;
+  static constexpr int CZG = 8, NH = 1, CZB = CZG * NH, THREADS = 256 * NH;
   static constexpr int RS = N + 1;                  // row stride of V and U: consecutive planes land in different banks
   static constexpr int Z = 0;                       // [cy][parity][H]
   static constexpr int V = N * N;                   // [i][parity][H], rows padded to RS
   static constexpr int U = N * N + CZB * RS;        // [i][cy], rows padded to RS
   static constexpr int WORDS = N * N + 2 * CZB * RS;
   static constexpr int COPIES = N * N + 2 * CZB * N;   // elements staged per s
-  static constexpr int STAGES = 5;                     // ring depth: enough bytes in flight to cover the HBM latency
+  static constexpr int STAGES = 4;                     // ring depth (two blocks per SM: 8 stages in flight per SM)
 };
 // Arithmetic of one s for the thread's 2 x 2 x 8 nodes.  MASK bit d set: the field of axis d (ux', uy, uz) is
 // identically zero for this sphere point (V1Tables::smask) and is neither staged nor read.
