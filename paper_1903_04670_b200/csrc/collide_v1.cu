@@ -827,7 +827,7 @@ __global__ void __launch_bounds__(256) k_zfwd_full(DevTables tab, V1Tables t, co
 // block's pipeline fill and its store of S with the other's arithmetic, which is worth more than the halved uz
 // traffic of 16-plane blocks that fill the SM alone (measured: 102 against 107 ms per step of c2).  Thread = 2 x 2 tile of (cx, cy): every table element
 // serves several nodes and all signs are compile-time constants.  The tables of one s (uz plane, rows of
-// ux' and uy) are staged in shared memory by cp.async, a ring of five stages over s; uz and uy are stored
+// ux' and uy) are staged in shared memory by cp.async, a ring of four stages over s; uz and uy are stored
 // de-interleaved by the parity of cx so that the pair loads are conflict-free.
 template <int N>
 struct WtermSmem {
