@@ -951,40 +951,73 @@ __global__ void __launch_bounds__(WtermSmem<N>::THREADS, 2 / WtermSmem<N>::NH) k
 // Thread pair per (kx,ky) pencil: parity 0 computes the even kz, parity 1 the odd kz (one radix-2
 // decimation-in-frequency step, then a length-N/2 transform in registers), so that the accumulators of
 // the whole group stay in registers and QG is touched once per group.  FIRST: store, do not accumulate.
+// The rows of T (64 pencils x N values of z per radial node) are staged in shared memory by cp.async, a ring of three
+// stages: the loads of the next two radial nodes are in flight while the current one is transformed, without holding
+// registers, and every element of T is fetched once (the two threads of a pencil read it from the stage).
+template <int N>
+struct ZaccSmem {
+  static constexpr int PB = 64, STAGES = 3, WORDS = N * PB;
+};
 template <int N, bool FIRST>
-__global__ void __launch_bounds__(256) k_zfwd_acc(DevTables tab, const int* __restrict__ tsrc, const cplx* __restrict__ T,
+__global__ void __launch_bounds__(128) k_zfwd_acc(DevTables tab, const int* __restrict__ tsrc, const cplx* __restrict__ T,
                                                   size_t slot_stride, cplx* __restrict__ QGh, size_t qstride, int r0, int nr) {
   constexpr int H = N / 2, NPH = N * (H + 1);
-  const int par = threadIdx.x >> 7;
-  const int pid = blockIdx.x * 128 + (threadIdx.x & 127);
+  typedef ZaccSmem<N> ZS;
+  constexpr int PB = ZS::PB, NS = ZS::STAGES;
+  extern __shared__ cplx sm[];
+  const int par = threadIdx.x >> 6, pl = threadIdx.x & 63;
+  const int pid0 = blockIdx.x * PB, pid = pid0 + pl;
   const int item = blockIdx.y, pair = item % tab.npairs;
-  if (pid >= NPH || tab.full[pair]) return;
-  const int kxs = sfreq(pid / (H + 1), N), kys = sfreq(pid % (H + 1), N);
+  if (tab.full[pair]) return;                                          // uniform per block
+  const cplx* tbase = T + (size_t)(item - pair + tsrc[pair]) * (N * NPH) + pid0;   // R-11
+  auto issue = [&](int sl) {
+    if (sl < nr) {
+      cplx* dstb = sm + (size_t)(sl % NS) * ZS::WORDS;
+      const cplx* srcb = tbase + (size_t)sl * slot_stride;
+#pragma unroll
+      for (int q = threadIdx.x; q < N * PB; q += 128) {
+        const int jj = q / PB, col = q % PB;
+        if (pid0 + col < NPH) cp_async16(&dstb[q], srcb + (size_t)jj * NPH + col);
+      }
+    }
+    cp_async_commit();
+  };
+#pragma unroll
+  for (int sl = 0; sl < NS - 1; ++sl) issue(sl);
+  const bool live = pid < NPH;
+  const int pc = live ? pid : 0;
+  const int kxs = sfreq(pc / (H + 1), N), kys = sfreq(pc % (H + 1), N);
   const int k2xy = kxs * kxs + kys * kys;
   cplx acc[H];
 #pragma unroll
   for (int k = 0; k < H; ++k) acc[k] = make_double2(0.0, 0.0);
   for (int sl = 0; sl < nr; ++sl) {
-    const cplx* src = T + (size_t)sl * slot_stride + (size_t)(item - pair + tsrc[pair]) * (N * NPH) + pid;   // R-11
-    cplx u[H];
-    if (par == 0) {
+    cp_async_wait_pending<NS - 2>();
+    __syncthreads();                            // stage sl has landed; the stage of sl - 1 is free
+    issue(sl + NS - 1);
+    if (live) {
+      const cplx* src = sm + (size_t)(sl % NS) * ZS::WORDS + pl;
+      cplx u[H];
+      if (par == 0) {
 #pragma unroll
-      for (int j = 0; j < H; ++j) u[j] = cadd(src[(size_t)j * NPH], src[(size_t)(j + H) * NPH]);
-    } else {
+        for (int j = 0; j < H; ++j) u[j] = cadd(src[j * PB], src[(j + H) * PB]);
+      } else {
 #pragma unroll
-      for (int j = 0; j < H; ++j) u[j] = twiddle_mul<N, -1>(csub(src[(size_t)j * NPH], src[(size_t)(j + H) * NPH]), j);
-    }
-    fft_reg<H, -1>(u);
-    const double* bv = tab.bvhs + ((size_t)pair * tab.N_rho + r0 + sl) * tab.K2n + k2xy;
-    const double scale = tab.w_rho[r0 + sl];
+        for (int j = 0; j < H; ++j) u[j] = twiddle_mul<N, -1>(csub(src[j * PB], src[(j + H) * PB]), j);
+      }
+      fft_reg<H, -1>(u);
+      const double* bv = tab.bvhs + ((size_t)pair * tab.N_rho + r0 + sl) * tab.K2n + k2xy;
+      const double scale = tab.w_rho[r0 + sl];
 #pragma unroll
-    for (int k = 0; k < H; ++k) {
-      const int kz = 2 * k + par, kzs = kz - (kz >= H ? N : 0);
-      const double b = scale * __ldg(&bv[kzs * kzs]);
-      acc[k].x = fma(b, u[k].x, acc[k].x);
-      acc[k].y = fma(b, u[k].y, acc[k].y);
+      for (int k = 0; k < H; ++k) {
+        const int kz = 2 * k + par, kzs = kz - (kz >= H ? N : 0);
+        const double b = scale * __ldg(&bv[kzs * kzs]);
+        acc[k].x = fma(b, u[k].x, acc[k].x);
+        acc[k].y = fma(b, u[k].y, acc[k].y);
+      }
     }
   }
+  if (!live) return;
   cplx* dst = QGh + (size_t)item * qstride + pid;
 #pragma unroll
   for (int k = 0; k < H; ++k) {
@@ -1162,6 +1195,7 @@ static int collide_v1_impl(dgfs_ctx* c, const double* f, double* out, int nx, bo
   const size_t smem_xyf = sizeof(cplx) * (size_t)W * FullSmem<N>::WORDS;
   const size_t smem_wt = sizeof(cplx) * (size_t)WtermSmem<N>::STAGES * WtermSmem<N>::WORDS;
   const size_t smem_nyq = sizeof(cplx) * (size_t)2 * JobSmem<N>::WORDS;
+  const size_t smem_zacc = sizeof(cplx) * (size_t)ZaccSmem<N>::STAGES * ZaccSmem<N>::WORDS;
   static bool attr_done = false;
   if (!attr_done) {
     cudaFuncSetAttribute(k_plane_fwd<N, W, 0>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_plane);
@@ -1171,12 +1205,14 @@ static int collide_v1_impl(dgfs_ctx* c, const double* f, double* out, int nx, bo
     cudaFuncSetAttribute(k_xy_full<N, W>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_xyf);
     cudaFuncSetAttribute(k_wterm<N>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_wt);
     cudaFuncSetAttribute(k_nyq2<N, 2>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_nyq);
+    cudaFuncSetAttribute(k_zfwd_acc<N, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_zacc);
+    cudaFuncSetAttribute(k_zfwd_acc<N, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_zacc);
     attr_done = true;
   }
   const int pen_blocks = (N2 + 127) / 128;
   const int hpen_blocks = (N * H + 127) / 128;
   const int plane_blocks = (N + W - 1) / W;
-  const int hp_blocks = (N * (H + 1) + 127) / 128;
+  const int hp_blocks = (N * (H + 1) + ZaccSmem<N>::PB - 1) / ZaccSmem<N>::PB;
   const int RG = c->v1_rgroup;
   const double fft3 = 15.0 * N3 * log2((double)N);
   const FlopsV1 fl = flops_v1(c);
@@ -1224,8 +1260,8 @@ static int collide_v1_impl(dgfs_ctx* c, const double* f, double* out, int nx, bo
         if ((r + 1) % RG == 0 || r + 1 == c->N_rho) {
           const int r0 = (r / RG) * RG, nr = r + 1 - r0;
           ProfScope ps(c->prof, st, "k_zfwd_acc", nb * nvhs * fl.acc * nr);
-          if (r0 == 0) k_zfwd_acc<N, true><<<dim3(hp_blocks, items), 256, 0, st>>>(c->tab, c->v1.tsrc, T, slot_stride, QG, qstride, r0, nr);
-          else k_zfwd_acc<N, false><<<dim3(hp_blocks, items), 256, 0, st>>>(c->tab, c->v1.tsrc, T, slot_stride, QG, qstride, r0, nr);
+          if (r0 == 0) k_zfwd_acc<N, true><<<dim3(hp_blocks, items), 128, smem_zacc, st>>>(c->tab, c->v1.tsrc, T, slot_stride, QG, qstride, r0, nr);
+          else k_zfwd_acc<N, false><<<dim3(hp_blocks, items), 128, smem_zacc, st>>>(c->tab, c->v1.tsrc, T, slot_stride, QG, qstride, r0, nr);
         }
       }
       if (nfull > 0) {
