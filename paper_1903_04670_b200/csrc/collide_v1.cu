@@ -258,25 +258,6 @@ __global__ void __launch_bounds__(256) k_pack_half(const cplx* __restrict__ fhat
   }
 }
 
-// Inverse z pass of h_z f^ for z job k = k0 + blockIdx.y of point blockIdx.z; thread per (lx, m) pencil.
-// in: fhh[xl][species][lz][lx][m];  out: Gz[xl][k][cz][lx][m].
-template <int N>
-__global__ void __launch_bounds__(128, 3) k_zshift(V1Tables t, int ns, const cplx* __restrict__ fhh, cplx* __restrict__ Gz, int r, int k0) {
-  constexpr int H = N / 2, NP = N * H;
-  const int pid = blockIdx.x * 128 + threadIdx.x;
-  if (pid >= NP) return;
-  const int k = k0 + blockIdx.y, xl = blockIdx.z;
-  const cplx* src = fhh + ((size_t)xl * ns + t.zsp[k]) * (size_t)(N * NP) + pid;
-  const cplx* hz = t.hz + ((size_t)r * t.nz + k) * N;
-  cplx v[N];
-#pragma unroll
-  for (int i = 0; i < N; ++i) v[i] = cmul(src[(size_t)i * NP], __ldg(&hz[i]));
-  fft_reg<N, +1>(v);
-  cplx* dst = Gz + ((size_t)xl * t.nz + k) * (size_t)(N * NP) + pid;
-#pragma unroll
-  for (int i = 0; i < N; ++i) dst[(size_t)i * NP] = v[i];
-}
-
 // 16-byte asynchronous copy global -> shared (LDGSTS): the data of the next plane job lands in shared
 // memory while the warp is still in the FFTs of the current one, without holding registers.
 __device__ __forceinline__ void cp_async16(void* smem, const void* gmem) {
@@ -287,6 +268,42 @@ __device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commi
 __device__ __forceinline__ void cp_async_wait_all() { asm volatile("cp.async.wait_group 0;\n" ::: "memory"); }
 template <int PENDING>
 __device__ __forceinline__ void cp_async_wait_pending() { asm volatile("cp.async.wait_group %0;\n" ::"n"(PENDING) : "memory"); }
+
+// Inverse z pass of h_z f^ for the z jobs k0 .. k0 + nk - 1 of point blockIdx.z that shift species blockIdx.y;
+// thread per (lx, m) pencil.  The block's 128 pencils of the half-packed spectrum are read ONCE into shared memory
+// (every job of a species starts from the same spectrum: 8 jobs per species and radial node at c2) and each job
+// multiplies, transforms in registers and stores its own array.
+// in: fhh[xl][species][lz][lx][m];  out: Gz[xl][k][cz][lx][m].
+template <int N>
+__global__ void __launch_bounds__(128, 3) k_zshift(V1Tables t, int ns, const cplx* __restrict__ fhh, cplx* __restrict__ Gz, int r, int k0, int nk) {
+  constexpr int H = N / 2, NP = N * H;
+  extern __shared__ cplx sm[];                       // [lz][128]
+  const int pid = blockIdx.x * 128 + threadIdx.x;
+  const int sp = blockIdx.y, xl = blockIdx.z;
+  int first = k0;
+  while (first < k0 + nk && t.zsp[first] != sp) ++first;
+  if (first == k0 + nk) return;                      // no job of this launch shifts this species (uniform)
+  const bool live = pid < NP;
+  if (live) {
+    const cplx* src = fhh + ((size_t)xl * ns + sp) * (size_t)(N * NP) + pid;
+#pragma unroll
+    for (int i = 0; i < N; ++i) cp_async16(&sm[i * 128 + threadIdx.x], src + (size_t)i * NP);
+  }
+  cp_async_commit();
+  cp_async_wait_all();                               // each thread reads back only what it copied itself
+  if (!live) return;
+  for (int k = first; k < k0 + nk; ++k) {
+    if (t.zsp[k] != sp) continue;
+    const cplx* hz = t.hz + ((size_t)r * t.nz + k) * N;
+    cplx v[N];
+#pragma unroll
+    for (int i = 0; i < N; ++i) v[i] = cmul(sm[i * 128 + threadIdx.x], __ldg(&hz[i]));
+    fft_reg<N, +1>(v);
+    cplx* dst = Gz + ((size_t)xl * t.nz + k) * (size_t)(N * NP) + pid;
+#pragma unroll
+    for (int i = 0; i < N; ++i) dst[(size_t)i * NP] = v[i];
+  }
+}
 
 // Per-warp shared memory of a plane job: the N x (N+1) tile (input columns, then the transposition) and
 // the job's small tables.
@@ -1196,6 +1213,7 @@ static int collide_v1_impl(dgfs_ctx* c, const double* f, double* out, int nx, bo
   const size_t smem_wt = sizeof(cplx) * (size_t)WtermSmem<N>::STAGES * WtermSmem<N>::WORDS;
   const size_t smem_nyq = sizeof(cplx) * (size_t)2 * JobSmem<N>::WORDS;
   const size_t smem_zacc = sizeof(cplx) * (size_t)ZaccSmem<N>::STAGES * ZaccSmem<N>::WORDS;
+  const size_t smem_zs = sizeof(cplx) * (size_t)N * 128;
   static bool attr_done = false;
   if (!attr_done) {
     cudaFuncSetAttribute(k_plane_fwd<N, W, 0>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_plane);
@@ -1205,6 +1223,7 @@ static int collide_v1_impl(dgfs_ctx* c, const double* f, double* out, int nx, bo
     cudaFuncSetAttribute(k_xy_full<N, W>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_xyf);
     cudaFuncSetAttribute(k_wterm<N>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_wt);
     cudaFuncSetAttribute(k_nyq2<N, 2>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_nyq);
+    cudaFuncSetAttribute(k_zshift<N>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_zs);
     cudaFuncSetAttribute(k_zfwd_acc<N, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_zacc);
     cudaFuncSetAttribute(k_zfwd_acc<N, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_zacc);
     attr_done = true;
@@ -1239,12 +1258,12 @@ static int collide_v1_impl(dgfs_ctx* c, const double* f, double* out, int nx, bo
       k_pack_half<N><<<(nb * ns * N2 * H + 255) / 256, 256, 0, st>>>(fhat, fhh, nyqy, nb * ns); }
     if (nz0 > 0) {     // the unshifted arrays (sigma_z = 0), the same for every radial node
       ProfScope ps(c->prof, st, "k_zshift", items * fl.zshift * nz0 / (nz - nz0 > 0 ? nz - nz0 : 1));
-      k_zshift<N><<<dim3(hpen_blocks, nz0, nb), 128, 0, st>>>(c->v1, ns, fhh, Gz, 0, nz - nz0);
+      k_zshift<N><<<dim3(hpen_blocks, ns, nb), 128, smem_zs, st>>>(c->v1, ns, fhh, Gz, 0, nz - nz0, nz0);
     }
     for (int r = 0; r < c->N_rho; ++r) {
       if (nz > nz0)
       { ProfScope ps(c->prof, st, "k_zshift", items * fl.zshift);
-        k_zshift<N><<<dim3(hpen_blocks, nz - nz0, nb), 128, 0, st>>>(c->v1, ns, fhh, Gz, r, 0); }
+        k_zshift<N><<<dim3(hpen_blocks, ns, nb), 128, smem_zs, st>>>(c->v1, ns, fhh, Gz, r, 0, nz - nz0); }
       if (!c->nyq_filter) {
       { ProfScope ps(c->prof, st, "k_nyq1d", nb * run_all * c->M * 16.0 * N2);
         k_nyq1d<N><<<(items * c->M + 3) / 4, 128, 0, st>>>(c->v1, c->tab, fhat, nyq, r, items * c->M); }
