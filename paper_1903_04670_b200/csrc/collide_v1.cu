@@ -911,10 +911,17 @@ __global__ void __launch_bounds__(WtermSmem<N>::THREADS, 2 / WtermSmem<N>::NH) k
   const int cz0 = blockIdx.x * CZB;
   const cplx* nbase = nyq + (size_t)blockIdx.y * M * NL::STRIDE;
   const unsigned char* skip = sskip + (size_t)(blockIdx.y % npairs) * M;
-  auto issue = [&](int s) {
-    cplx* dst = sm + (size_t)(s % NS) * WS::WORDS;
+  // which fields each sphere point has (7: none, or the point is not run for this pair, R-10), once per block in
+  // shared memory: the loop below then never waits for a global load before it can issue or branch
+  __shared__ unsigned char mk_s[256];
+  for (int i = threadIdx.x; i < M && i < 256; i += NT) mk_s[i] = skip[i] ? 7 : smask[i];
+  __syncthreads();
+  auto mk = [&](int s) -> int { return s < 256 ? (int)mk_s[s] : (skip[s] ? 7 : (int)smask[s]); };
+  auto next_a = [&](int s) { while (s < M && mk(s) == 7) ++s; return s; };      // next point with something to add
+  auto issue = [&](int s, int slot) {
+    cplx* dst = sm + (size_t)slot * WS::WORDS;
     const cplx* nq = nbase + (size_t)s * NL::STRIDE;
-    const int mask = skip[s] ? 7 : smask[s];         // vanishing fields and skipped points (R-10) are not staged
+    const int mask = mk(s);                          // vanishing fields are not staged
     for (int e = threadIdx.x; e < WS::COPIES; e += NT) {
       if (e < N2) {
         const int cy = e / N, cx = e % N;
@@ -932,17 +939,22 @@ __global__ void __launch_bounds__(WtermSmem<N>::THREADS, 2 / WtermSmem<N>::NH) k
   double acc[CZG][2][2];                      // [cz][cy][cx]
 #pragma unroll
   for (int i = 0; i < CZG; ++i) acc[i][0][0] = acc[i][0][1] = acc[i][1][0] = acc[i][1][1] = 0.0;
-  // ring of NS stages: groups 0 .. s + NS - 2 are committed when iteration s waits for group s (empty groups
-  // keep the count uniform at the end)
+  // ring of NS stages over the points that are run: job j uses stage j % NS; groups 0 .. j + NS - 2 are committed
+  // when job j waits for group j (empty groups keep the count uniform at the end)
+  int s_issue = next_a(0), j_issue = 0;
 #pragma unroll
-  for (int k = 0; k < NS - 1; ++k) { if (k < M) issue(k); else cp_async_commit(); }
-  for (int s = 0; s < M; ++s) {
+  for (int k = 0; k < NS - 1; ++k) {
+    if (s_issue < M) { issue(s_issue, j_issue % NS); s_issue = next_a(s_issue + 1); } else cp_async_commit();
+    ++j_issue;
+  }
+  for (int s = next_a(0), j = 0; s < M; s = next_a(s + 1), ++j) {
     cp_async_wait_pending<NS - 2>();
     __syncthreads();
-    if (s + NS - 1 < M) issue(s + NS - 1); else cp_async_commit();
+    if (s_issue < M) { issue(s_issue, j_issue % NS); s_issue = next_a(s_issue + 1); } else cp_async_commit();
+    ++j_issue;
     if (!act) continue;
-    const cplx* b_ = sm + (size_t)(s % NS) * WS::WORDS;
-    switch (skip[s] ? 7 : smask[s]) {                // uniform over the block
+    const cplx* b_ = sm + (size_t)(j % NS) * WS::WORDS;
+    switch (mk(s)) {                                 // uniform over the block
       case 0: wterm_planes<N, 0>(b_, half, tx, ty, acc); break;
       case 1: wterm_planes<N, 1>(b_, half, tx, ty, acc); break;
       case 2: wterm_planes<N, 2>(b_, half, tx, ty, acc); break;
@@ -950,7 +962,7 @@ __global__ void __launch_bounds__(WtermSmem<N>::THREADS, 2 / WtermSmem<N>::NH) k
       case 4: wterm_planes<N, 4>(b_, half, tx, ty, acc); break;
       case 5: wterm_planes<N, 5>(b_, half, tx, ty, acc); break;
       case 6: wterm_planes<N, 6>(b_, half, tx, ty, acc); break;
-      default: break;                                // all three fields vanish
+      default: break;
     }
   }
   if (!act) return;
