@@ -59,14 +59,28 @@ int launch_nyquist_filter(dgfs_ctx* c, const double* src, double* dst, int narr,
 }
 
 // ------------------------------------------------------------------ host orchestration ---------
-int ensure_workspace(dgfs_ctx* c, size_t bytes) {
+// Workspace growth is ordered on the caller's stream (stream-ordered allocator): the old block is released after
+// everything enqueued so far, the new one exists before anything enqueued later; no device-wide synchronisation.
+// Not possible while `st` is being captured into a CUDA graph: dgfs_reserve first (include/dgfs.h).
+int ensure_workspace(dgfs_ctx* c, size_t bytes, cudaStream_t st) {
   if (bytes <= c->ws_bytes) return DGFS_OK;
-  cudaError_t e = cudaDeviceSynchronize();
-  if (e != cudaSuccess) return check_cuda(c, e, "workspace sync");
-  cudaFree(c->ws);
+  cudaStreamCaptureStatus cap = cudaStreamCaptureStatusNone;
+  cudaStreamIsCapturing(st, &cap);
+  if (cap != cudaStreamCaptureStatusNone)
+    return set_error(c, DGFS_EINVAL, "workspace too small during stream capture: call dgfs_reserve before capturing");
+  if (!c->pool_set) {
+    cudaMemPool_t pool;
+    if (cudaDeviceGetDefaultMemPool(&pool, c->device) == cudaSuccess) {
+      unsigned long long keep = ~0ull;
+      cudaMemPoolSetAttribute(pool, cudaMemPoolAttrReleaseThreshold, &keep);
+    }
+    c->pool_set = true;
+  }
+  if (c->ev_last_set) cudaStreamWaitEvent(st, c->ev_last, 0);      // earlier calls on other streams still use the old block
+  if (c->ws) cudaFreeAsync(c->ws, st);
   c->ws = nullptr; c->ws_bytes = 0;
-  int rc = check_cuda(c, cudaMalloc(&c->ws, bytes), "workspace allocation");
-  if (rc) return rc;
+  int rc = check_cuda(c, cudaMallocAsync(&c->ws, bytes, st), "workspace allocation");
+  if (rc) { c->ws = nullptr; return rc; }
   c->ws_bytes = bytes;
   return DGFS_OK;
 }
@@ -98,7 +112,7 @@ static int collide_impl(dgfs_ctx* c, const double* f, double* out, int nx, bool 
   constexpr int N2 = N * N, N3 = N2 * N;
   constexpr int W = (N <= 32) ? 4 : 2;
   const ChunkPlan pl = plan_chunks(c, nx);
-  int rc = ensure_workspace(c, pl.total);
+  int rc = ensure_workspace(c, pl.total, st);
   if (rc) return rc;
   char* ws = (char*)c->ws;
   cplx* fhat = (cplx*)(ws + pl.off_fhat);
@@ -110,14 +124,13 @@ static int collide_impl(dgfs_ctx* c, const double* f, double* out, int nx, bool 
   const size_t smem_plane = plane_smem_per_warp<N>() * W;
   const size_t smem_final = plane_smem_per_warp<N>() * 2;
   const size_t smem_z = sizeof(cplx) * (N / 2) * 256;
-  static bool attr_done = false;
-  if (!attr_done) {
+  if (!c->v0_attr_done) {                 // per context, hence per device
     cudaFuncSetAttribute(k_plane_fwd<N, W, 0>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_plane);
     cudaFuncSetAttribute(k_plane_fwd<N, W, 1>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_plane);
     cudaFuncSetAttribute(k_shift_xy<N, W>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_plane);
     cudaFuncSetAttribute(k_final_xy<N>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_final);
     cudaFuncSetAttribute(k_z_prod<N>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_z);
-    attr_done = true;
+    c->v0_attr_done = true;
   }
   const int pen_blocks = (N2 + 127) / 128;
   const int plane_blocks = (N + W - 1) / W;
@@ -167,16 +180,25 @@ static int collide_impl(dgfs_ctx* c, const double* f, double* out, int nx, bool 
   return check_cuda(c, cudaGetLastError(), "collide launch");
 }
 
+// One call at a time owns the context's workspace (and, for v1, its auxiliary streams): a call first waits, on its
+// stream, for the last launch of the previous call, whichever stream that was issued on.
 int run_collide(dgfs_ctx* c, const double* f, double* out, int nx, bool pairs_out, cudaStream_t st) {
-  if (c->use_v1) return run_collide_v1(c, f, out, nx, pairs_out, st);
-  switch (c->N) {
-    case 8: return collide_impl<8>(c, f, out, nx, pairs_out, st);
-    case 16: return collide_impl<16>(c, f, out, nx, pairs_out, st);
-    case 24: return collide_impl<24>(c, f, out, nx, pairs_out, st);
-    case 32: return collide_impl<32>(c, f, out, nx, pairs_out, st);
-    case 48: return collide_impl<48>(c, f, out, nx, pairs_out, st);
+  cudaStreamCaptureStatus cap = cudaStreamCaptureStatusNone;
+  cudaStreamIsCapturing(st, &cap);
+  const bool capturing = cap != cudaStreamCaptureStatusNone;      // a captured graph orders its own nodes
+  if (!capturing && c->ev_last_set) cudaStreamWaitEvent(st, c->ev_last, 0);
+  int rc;
+  if (c->use_v1) rc = run_collide_v1(c, f, out, nx, pairs_out, st);
+  else switch (c->N) {
+    case 8: rc = collide_impl<8>(c, f, out, nx, pairs_out, st); break;
+    case 16: rc = collide_impl<16>(c, f, out, nx, pairs_out, st); break;
+    case 24: rc = collide_impl<24>(c, f, out, nx, pairs_out, st); break;
+    case 32: rc = collide_impl<32>(c, f, out, nx, pairs_out, st); break;
+    case 48: rc = collide_impl<48>(c, f, out, nx, pairs_out, st); break;
+    default: rc = set_error(c, DGFS_ENOSUP, "unsupported N");
   }
-  return set_error(c, DGFS_ENOSUP, "unsupported N");
+  if (!capturing && c->ev_last) { cudaEventRecord(c->ev_last, st); c->ev_last_set = true; }
+  return rc;
 }
 
 static size_t workspace_for(const dgfs_ctx* c, int nx) {
@@ -237,7 +259,7 @@ extern "C" int dgfs_collide_host(dgfs_ctx* c, const double* f_host, double* Q_ho
     }
     c->hp_pts = slab;
   }
-  if ((rc = ensure_workspace(c, workspace_for(c, slab)))) return rc;
+  if ((rc = ensure_workspace(c, workspace_for(c, slab), c->hp_stream[1]))) return rc;
   cudaStream_t s_in = c->hp_stream[0], s_k = c->hp_stream[1], s_out = c->hp_stream[2];
   int i = 0;
   for (int x0 = 0; x0 < nx; x0 += slab, ++i) {
@@ -268,7 +290,9 @@ extern "C" int dgfs_reserve(dgfs_ctx* c, int nx) {
   if (nx < 0) return set_error(c, DGFS_EINVAL, "dgfs_reserve: nx must be >= 0");
   if (nx == 0) return DGFS_OK;
   cudaSetDevice(c->device);
-  return ensure_workspace(c, workspace_for(c, nx));
+  int rc = ensure_workspace(c, workspace_for(c, nx), nullptr);
+  if (rc) return rc;
+  return check_cuda(c, cudaStreamSynchronize(nullptr), "dgfs_reserve");
 }
 extern "C" long long dgfs_launch_count(const dgfs_ctx* c) { return c ? c->prof.total_launches : 0; }
 extern "C" int dgfs_profile_enable(dgfs_ctx* c, int on) {

@@ -205,7 +205,20 @@ int build_tables_v1(dgfs_ctx* c) {
   for (int s2 = 0; s2 < M; ++s2)
     for (int d = 0; d < 3; ++d)
       if (c->sigma[3 * s2 + d] == 0.0) c->v1_smask[s2] |= (unsigned char)(1 << d);
+  // the plane jobs of every pair as a list the kernels walk without further look-ups
+  c->v1_jobs.assign((size_t)np * M, make_int4(0, 0, 0, 0));
+  c->v1_njobs.assign(np, 0);
+  for (int pr = 0; pr < np; ++pr) {
+    if (c->v1_tsrc[pr] != pr) continue;
+    for (int s2 = 0; s2 < M; ++s2) {
+      if (c->v1_sskip[(size_t)pr * M + s2]) continue;
+      c->v1_jobs[(size_t)pr * M + c->v1_njobs[pr]++] =
+          make_int4(s2, c->v1_zmap[((size_t)pr * M + s2) * 2], c->v1_zmap[((size_t)pr * M + s2) * 2 + 1], c->v1_smask[s2]);
+    }
+  }
   int rc;
+  if ((rc = upload(c, &c->d_v1_jobs, c->v1_jobs, "upload job lists"))) return rc;
+  if ((rc = upload(c, &c->d_v1_njobs, c->v1_njobs, "upload job counts"))) return rc;
   if ((rc = upload(c, &c->d_v1_smask, c->v1_smask, "upload sphere masks"))) return rc;
   if ((rc = upload(c, &c->d_v1_sskip, c->v1_sskip, "upload antipode masks"))) return rc;
   if ((rc = upload(c, &c->d_v1_tsrc, c->v1_tsrc, "upload pair sources"))) return rc;
@@ -222,12 +235,14 @@ int build_tables_v1(dgfs_ctx* c) {
   V1Tables& t = c->v1;
   t.nz = nz; t.zsp = c->d_v1_zsp; t.zmap = c->d_v1_zmap; t.hz = c->d_v1_hz; t.szv = c->d_v1_szv;
   t.hxy = c->d_v1_hxy; t.sxy = c->d_v1_sxy; t.smask = c->d_v1_smask; t.sskip = c->d_v1_sskip; t.tsrc = c->d_v1_tsrc; t.fsrc_s = c->d_v1_fsrc_s; t.fscale = c->d_v1_fscale; t.anti = c->d_v1_anti; t.tpartner = c->d_v1_tpartner;
+  t.jobs = c->d_v1_jobs; t.njobs = c->d_v1_njobs;
   return DGFS_OK;
 }
 
 void free_tables_v1(dgfs_ctx* c) {
   cudaFree(c->d_v1_zsp); cudaFree(c->d_v1_zmap); cudaFree(c->d_v1_hz); cudaFree(c->d_v1_szv);
   cudaFree(c->d_v1_hxy); cudaFree(c->d_v1_sxy); cudaFree(c->d_v1_smask); cudaFree(c->d_v1_sskip); cudaFree(c->d_v1_tsrc); cudaFree(c->d_v1_fsrc_s); cudaFree(c->d_v1_fscale); cudaFree(c->d_v1_anti); cudaFree(c->d_v1_tpartner);
+  cudaFree(c->d_v1_jobs); cudaFree(c->d_v1_njobs);
 }
 
 // ---------------------------------------------------------------- device code -------------------
@@ -273,9 +288,11 @@ __device__ __forceinline__ void cp_async_wait_pending() { asm volatile("cp.async
 // thread per (lx, m) pencil.  The block's 128 pencils of the half-packed spectrum are read ONCE into shared memory
 // (every job of a species starts from the same spectrum: 8 jobs per species and radial node at c2) and each job
 // multiplies, transforms in registers and stores its own array.
-// in: fhh[xl][species][lz][lx][m];  out: Gz[xl][k][cz][lx][m].
+// in: fhh[xl][species][lz][lx][m];  out: Gz[xl][k - kbase][cz][lx][m], kstride arrays per point (the jobs that depend
+// on the radial node and the sigma_z = 0 jobs, which do not, live in separate buffers: GzView below).
 template <int N>
-__global__ void __launch_bounds__(128, 3) k_zshift(V1Tables t, int ns, const cplx* __restrict__ fhh, cplx* __restrict__ Gz, int r, int k0, int nk) {
+__global__ void __launch_bounds__(128, 3) k_zshift(V1Tables t, int ns, const cplx* __restrict__ fhh, cplx* __restrict__ Gz, int r, int k0, int nk,
+                                                   int kbase, int kstride) {
   constexpr int H = N / 2, NP = N * H;
   extern __shared__ cplx sm[];                       // [lz][128]
   const int pid = blockIdx.x * 128 + threadIdx.x;
@@ -299,11 +316,22 @@ __global__ void __launch_bounds__(128, 3) k_zshift(V1Tables t, int ns, const cpl
 #pragma unroll
     for (int i = 0; i < N; ++i) v[i] = cmul(sm[i * 128 + threadIdx.x], __ldg(&hz[i]));
     fft_reg<N, +1>(v);
-    cplx* dst = Gz + ((size_t)xl * t.nz + k) * (size_t)(N * NP) + pid;
+    cplx* dst = Gz + ((size_t)xl * kstride + (k - kbase)) * (size_t)(N * NP) + pid;
 #pragma unroll
     for (int i = 0; i < N; ++i) dst[(size_t)i * NP] = v[i];
   }
 }
+
+// Where the z-shifted arrays of a chunk live: jobs 0 .. nzr-1 depend on the radial node (double-buffered, one buffer
+// per radial node in flight), jobs nzr .. nz-1 (sigma_z = 0) are written once per chunk.
+struct GzView {
+  const cplx* r;             // [xl][nzr][cz][lx][m]
+  const cplx* z0;            // [xl][nz - nzr][cz][lx][m]
+  int nzr, nz0;
+  __device__ __forceinline__ const cplx* job(int xl, int k, size_t arr) const {
+    return k < nzr ? r + ((size_t)xl * nzr + k) * arr : z0 + ((size_t)xl * nz0 + (k - nzr)) * arr;
+  }
+};
 
 // Per-warp shared memory of a plane job: the N x (N+1) tile (input columns, then the transposition) and
 // the job's small tables.
@@ -563,7 +591,7 @@ __global__ void __launch_bounds__(32 * NW) k_nyq2(V1Tables t, DevTables tab, con
 //           y pass: Z = a_r + i b_r;  acc[cy] += Re Z Im Z
 // in: S[item][cz][cy][cx] = -sum_s Re W Im W (k_wterm);  out: T[item][cz][kx][ky <= H] = fft_xy of S_r(., ., cz).
 template <int N, int W>
-__global__ void __launch_bounds__(32 * W) k_xy(V1Tables t, DevTables tab, const cplx* __restrict__ Gz,
+__global__ void __launch_bounds__(32 * W) __maxnreg__(W == 2 ? 200 : 255) k_xy(V1Tables t, DevTables tab, GzView Gz,
                                                const cplx* __restrict__ nyq, const double* __restrict__ S,
                                                cplx* __restrict__ T, int r) {
   constexpr int H = N / 2, NH = N * H, N2 = N * N;
@@ -582,31 +610,32 @@ __global__ void __launch_bounds__(32 * W) k_xy(V1Tables t, DevTables tab, const 
   const int side = ln / H, m = ln % H;
   const double szs = (cz & 1) ? -1.0 : 1.0;
   const double sxb = (ln & 1) ? -1.0 : 1.0;
-  const int* zm = t.zmap + (size_t)pair * tab.M * 2;
-  const cplx* gbase = Gz + (size_t)xl * t.nz * (size_t)(N * NH) + (size_t)cz * NH + m;
+  const size_t goff = (size_t)cz * NH + m;
   const cplx* hbase = t.hxy + (((size_t)pair * tab.N_rho + r) * tab.M) * 4 * N;
   const cplx* nbase = nyq + (size_t)item * tab.M * NL::STRIDE;
-  auto issue = [&](int s) {
+  // job = {s, z job of side A, z job of side B, smask[s]} (V1Tables::jobs): the entry of the next job is fetched a
+  // whole job ahead, so no look-up sits between the end of one job and the prefetch of the next
+  const int4* jl = t.jobs + (size_t)pair * tab.M;
+  const int nj = t.njobs[pair];
+  auto issue = [&](int4 jb) {
     if (act) {
-      const cplx* g = gbase + (size_t)zm[2 * s + side] * (size_t)(N * NH);
+      const cplx* g = Gz.job(xl, side ? jb.z : jb.y, (size_t)(N * NH)) + goff;
 #pragma unroll
       for (int i = 0; i < N; ++i) cp_async16(&buf[i * P + ln], g + i * H);
-      const cplx* hx = hbase + (size_t)s * 4 * N;          // [side][x|y][N]
+      const cplx* hx = hbase + (size_t)jb.x * 4 * N;       // [side][x|y][N]
       cp_async16(&buf[JS::HI + ln], hx + ln);               // h_x side A
       cp_async16(&buf[JS::HI + JS::TS + ln], hx + 2 * N + ln);   // h_x side B
       cp_async16(&buf[JS::HM + ln], hx + N + ln);           // h_y side A
       cp_async16(&buf[JS::HM + JS::TS + ln], hx + 3 * N + ln);   // h_y side B
-      const cplx* nq = nbase + (size_t)s * NL::STRIDE;
+      const cplx* nq = nbase + (size_t)jb.x * NL::STRIDE;
       cp_async16(&buf[JS::VYH + ln], nq + NL::VYH + ln);
       cp_async16(&buf[JS::VXP + ln], nq + NL::VXP + ln);
       if (ln == 0) cp_async16(&buf[JS::VZP], nq + NL::VZP + cz);
     }
     cp_async_commit();
   };
-  const unsigned char* skip = t.sskip + (size_t)pair * tab.M;
-  auto next_s = [&](int s) { while (s < tab.M && skip[s]) ++s; return s; };     // sphere points run for this pair (R-10)
-  int s = next_s(0);
-  if (s < tab.M) issue(s);
+  int mask = 0;
+  if (nj > 0) { const int4 j0 = __ldg(&jl[0]); issue(j0); mask = j0.w; }
   // start from the Nyquist-field product written by k_wterm
   double acc[N];
   {
@@ -614,27 +643,26 @@ __global__ void __launch_bounds__(32 * W) k_xy(V1Tables t, DevTables tab, const 
 #pragma unroll
     for (int j = 0; j < N; ++j) acc[j] = w0[j * N];
   }
-  while (s < tab.M) {
-    const int sn = next_s(s + 1);
+  for (int j = 0; j < nj; ++j) {
+    const int4 jn = __ldg(&jl[j + 1 < nj ? j + 1 : j]);          // used after pass 1: its latency hides behind it
     cp_async_wait_all();
     __syncwarp();
     cplx X[N];
     if (act) {
       // sigma_x = 0: h_x is the constant w_s / N (side A) or 1 / N; sigma_y = 0: h_y is the constant 1 / N
-      const int mk = t.smask[s];
-      const bool ux_ = (mk & 1) != 0, ry_ = (mk & 2) != 0;
+      const bool ux_ = (mask & 1) != 0, ry_ = (mask & 2) != 0;
       job_pass1<N, true>(buf, ln, side, m, szs, ux_ ? buf[JS::HI + side * JS::TS].x : 1.0, ux_, ry_);
     }
     __syncwarp();
     if (act) job_pass2_in<N, true>(buf, ln, szs, sxb, X);
     __syncwarp();
-    if (sn < tab.M) issue(sn);               // the tile is free: the next job's data arrives during pass 2
+    if (j + 1 < nj) issue(jn);               // the tile is free: the next job's data arrives during pass 2
     if (act) {
       fft_reg<N, +1>(X);
 #pragma unroll
-      for (int j = 0; j < N; ++j) acc[j] = fma(X[j].x, X[j].y, acc[j]);
+      for (int jj = 0; jj < N; ++jj) acc[jj] = fma(X[jj].x, X[jj].y, acc[jj]);
     }
-    s = sn;
+    mask = jn.w;
   }
   // forward y and x passes of the real plane S_r(., ., cz) (steps 6-7, after R-1)
   if (act) {
@@ -674,7 +702,7 @@ struct FullSmem {
   static constexpr int WORDS = UY + N;
 };
 template <int N, int W>
-__global__ void __launch_bounds__(32 * W) k_xy_full(V1Tables t, DevTables tab, const cplx* __restrict__ Gz,
+__global__ void __launch_bounds__(32 * W) k_xy_full(V1Tables t, DevTables tab, GzView Gz,
                                                     const cplx* __restrict__ nyq, cplx* __restrict__ Tf, int r) {
   constexpr int H = N / 2, NH = N * H, N2 = N * N, N3 = N2 * N;
   typedef NyqLayout<N> NL;
@@ -694,12 +722,12 @@ __global__ void __launch_bounds__(32 * W) k_xy_full(V1Tables t, DevTables tab, c
   const double szs = (cz & 1) ? -1.0 : 1.0;
   const double sxb = (ln & 1) ? -1.0 : 1.0;
   const int* zm = t.zmap + (size_t)pair * tab.M * 2;
-  const cplx* gbase = Gz + (size_t)xl * t.nz * (size_t)(N * NH) + (size_t)cz * NH + m;
+  const size_t goff = (size_t)cz * NH + m;
   const cplx* hbase = t.hxy + (((size_t)pair * tab.N_rho + r) * tab.M) * 4 * N;
   const cplx* nbase = nyq + (size_t)item * tab.M * NL::STRIDE;
   auto issue = [&](int s) {
     if (act) {
-      const cplx* g = gbase + (size_t)zm[2 * s + side] * (size_t)(N * NH);
+      const cplx* g = Gz.job(xl, zm[2 * s + side], (size_t)(N * NH)) + goff;
 #pragma unroll
       for (int i = 0; i < N; ++i) cp_async16(&buf[i * P + ln], g + i * H);
       const cplx* hx = hbase + (size_t)s * 4 * N;          // [side][x|y][N]
@@ -1092,8 +1120,8 @@ __global__ void __launch_bounds__(64) k_final_xy_h(DevTables tab, const cplx* __
 // ---------------------------------------------------------------- host orchestration ------------
 namespace {
 struct PlanV1 {
-  int nbx;
-  size_t off_fhat, off_fhh, off_nyqy, off_qg, off_gz, off_nyq, off_s, off_t, off_tf, off_fp, nyq_bytes, qstride, total;
+  int nbx, nbuf, tslots;
+  size_t off_fhat, off_fhh, off_nyqy, off_qg, off_gzr[2], off_gz0, off_nyq[2], off_s[2], off_t, off_tf, off_fp, nyq_bytes, qstride, total;
 };
 PlanV1 plan_v1(const dgfs_ctx* c, int nx) {
   PlanV1 pl{};
@@ -1103,9 +1131,12 @@ PlanV1 plan_v1(const dgfs_ctx* c, int nx) {
   if (nbx < 1) nbx = 1;
   if ((size_t)nbx * c->npairs > 65535) nbx = 65535 / c->npairs;
   pl.nbx = nbx;
+  // two-stream schedule: the buffers filled by the preparing kernels exist twice (radial nodes r and r + 1 in flight)
+  pl.nbuf = c->v1_overlap ? 2 : 1;
   const size_t items = (size_t)nbx * c->npairs;
   const size_t nyq_stride = 4 * N + 3 * N * N;
-  size_t gz = (size_t)nbx * c->v1_nz * (arr / 2), g2 = items * 2 * arr;
+  const size_t nzr = c->v1_nz - c->v1_nz0;
+  size_t gz = (size_t)nbx * nzr * (arr / 2), g2 = items * 2 * arr;
   size_t off = 0;
   auto take = [&](size_t bytes) { size_t o = off; off += (bytes + 255) & ~(size_t)255; return o; };
   pl.off_fhat = take((size_t)nbx * c->ns * arr);
@@ -1115,12 +1146,18 @@ PlanV1 plan_v1(const dgfs_ctx* c, int nx) {
   // QG per item: Hermitian half for VHS pairs, the whole spectrum for pairs with a full b table
   pl.qstride = (c->any_full ? arr : half_arr) / sizeof(cplx);
   pl.off_qg = take(items * pl.qstride * sizeof(cplx));
-  pl.off_gz = take(gz > g2 ? gz : g2);
+  pl.off_gzr[0] = take(gz > g2 ? gz : g2);               // also the scratch of step 10
+  pl.off_gzr[1] = pl.nbuf > 1 ? take(gz) : pl.off_gzr[0];
+  pl.off_gz0 = take((size_t)nbx * c->v1_nz0 * (arr / 2));
   pl.nyq_bytes = items * c->M * nyq_stride * sizeof(cplx);
-  pl.off_nyq = take(pl.nyq_bytes);
-  pl.off_s = take(items * N3 * sizeof(double));
-  // T: forward-transformed planes of a group of radial nodes; also the z-pass scratch of step 1
-  const size_t tg = (size_t)c->v1_rgroup * items * half_arr, t1 = (size_t)nbx * c->ns * arr;
+  pl.off_nyq[0] = take(pl.nyq_bytes);
+  pl.off_nyq[1] = pl.nbuf > 1 ? take(pl.nyq_bytes) : pl.off_nyq[0];
+  pl.off_s[0] = take(items * N3 * sizeof(double));
+  pl.off_s[1] = pl.nbuf > 1 ? take(items * N3 * sizeof(double)) : pl.off_s[0];
+  // T: forward-transformed planes of pl.nbuf groups of radial nodes (a ring: the forward z pass of one group runs
+  // while the plane jobs fill the next); also the z-pass scratch of step 1
+  pl.tslots = pl.nbuf * c->v1_rgroup;
+  const size_t tg = (size_t)pl.tslots * items * half_arr, t1 = (size_t)nbx * c->ns * arr;
   pl.off_t = take(tg > t1 ? tg : t1);
   // Tf: per-s forward-transformed planes of the full-table pairs
   pl.off_tf = take(c->any_full ? items * c->M * arr : 0);
@@ -1185,23 +1222,70 @@ double flops_per_pair_eval_v1(const dgfs_ctx* c, int pair) {
   return c->N_rho * (f.zshift + frac * (f.nyq + f.wterm + f.xy - fwd) + fwd + f.acc) + f.tail;
 }
 
+// Streams and events of the two-stream schedule (created with the context's v1 tables).
+int init_streams_v1(dgfs_ctx* c) {
+  const char* ov = getenv("DGFS_V1_OVERLAP");
+  // measured at c2 (profiles/r02_streams.md): with the auxiliary streams at high priority the preparing kernels
+  // displace the plane jobs instead of sharing the SMs with them (each of them fills the register file or the
+  // shared memory of an SM on its own), same step time; at equal priority only the tails overlap, 1 % faster.
+  // Off by default: one stream, per-kernel event times that add up.
+  c->v1_overlap = (ov && atoi(ov) != 0);
+  const char* xw = getenv("DGFS_V1_XYW");
+  c->v1_xyw = (xw && atoi(xw) == 2) ? 2 : 4;
+  if (!c->v1_overlap) return DGFS_OK;
+  int least = 0, greatest = 0;
+  cudaDeviceGetStreamPriorityRange(&least, &greatest);
+  const char* pr = getenv("DGFS_V1_AUX_PRIORITY");          // 1 (default): highest priority; 0: default priority
+  const int prio = (pr && atoi(pr) == 0) ? 0 : greatest;
+  int rc;
+  if ((rc = check_cuda(c, cudaStreamCreateWithPriority(&c->aux, cudaStreamNonBlocking, prio), "stream create"))) return rc;
+  if ((rc = check_cuda(c, cudaStreamCreateWithPriority(&c->aux2, cudaStreamNonBlocking, prio), "stream create"))) return rc;
+  cudaEvent_t* evs[] = {&c->ev_head, &c->ev_prep[0], &c->ev_prep[1], &c->ev_xy[0], &c->ev_xy[1],
+                        &c->ev_grp[0], &c->ev_grp[1], &c->ev_acc[0], &c->ev_acc[1]};
+  for (cudaEvent_t* e : evs)
+    if ((rc = check_cuda(c, cudaEventCreateWithFlags(e, cudaEventDisableTiming), "event create"))) return rc;
+  return DGFS_OK;
+}
+void free_streams_v1(dgfs_ctx* c) {
+  cudaEvent_t evs[] = {c->ev_head, c->ev_prep[0], c->ev_prep[1], c->ev_xy[0], c->ev_xy[1], c->ev_grp[0], c->ev_grp[1],
+                       c->ev_acc[0], c->ev_acc[1]};
+  for (cudaEvent_t e : evs) if (e) cudaEventDestroy(e);
+  if (c->aux) cudaStreamDestroy(c->aux);
+  if (c->aux2) cudaStreamDestroy(c->aux2);
+}
+
+// Schedule of one chunk (all launches asynchronous; `st` is the caller's stream):
+//   st  : step 1 | k_xy(0) | k_xy(1) | ...                         | step 10
+//   aux : z shifts with sigma_z = 0 | prep(0) | prep(1) | prep(2) ...      prep(r) = k_zshift, k_nyq1d, k_nyq2, k_wterm
+//   aux2:                                   forward z pass + QG accumulation of every finished group of radial nodes
+// prep(r) fills buffer r & 1 (z-shifted arrays, Nyquist fields, S) and waits for k_xy(r - 2) to have read it; k_xy(r)
+// waits for prep(r).  The preparing kernels are bound by memory traffic and latencies and leave the FP64 pipe mostly
+// idle, the plane jobs are bound by the FP64 pipe: on the same SMs at the same time they fill each other's gaps.  aux
+// and aux2 have the higher priority, so their blocks take the slots that k_xy blocks free.  With DGFS_V1_OVERLAP=0
+// the three streams are the caller's and the events are not used.
 template <int N>
 static int collide_v1_impl(dgfs_ctx* c, const double* f, double* out, int nx, bool pairs_out, cudaStream_t st) {
   constexpr int N2 = N * N, N3 = N2 * N, H = N / 2;
   constexpr int W = 4;
   const PlanV1 pl = plan_v1(c, nx);
-  int rc = ensure_workspace(c, pl.total);
+  int rc = ensure_workspace(c, pl.total, st);
   if (rc) return rc;
+  const bool ov = c->v1_overlap != 0;
+  cudaStream_t sa = ov ? c->aux : st, sz = ov ? c->aux2 : st;
+  auto wait = [&](cudaStream_t s, cudaEvent_t e) { if (ov) cudaStreamWaitEvent(s, e, 0); };
+  auto record = [&](cudaEvent_t e, cudaStream_t s) { if (ov) cudaEventRecord(e, s); };
   char* ws = (char*)c->ws;
   cplx* fhat = (cplx*)(ws + pl.off_fhat);
   cplx* fhh = (cplx*)(ws + pl.off_fhh);
   cplx* nyqy = (cplx*)(ws + pl.off_nyqy);
   cplx* QG = (cplx*)(ws + pl.off_qg);
-  cplx* Gz = (cplx*)(ws + pl.off_gz);
-  cplx* nyq = (cplx*)(ws + pl.off_nyq);
-  double* S = (double*)(ws + pl.off_s);
+  cplx* GzR[2] = {(cplx*)(ws + pl.off_gzr[0]), (cplx*)(ws + pl.off_gzr[1])};
+  cplx* Gz0 = (cplx*)(ws + pl.off_gz0);
+  cplx* nyqb[2] = {(cplx*)(ws + pl.off_nyq[0]), (cplx*)(ws + pl.off_nyq[1])};
+  double* Sb[2] = {(double*)(ws + pl.off_s[0]), (double*)(ws + pl.off_s[1])};
   cplx* T = (cplx*)(ws + pl.off_t);
   cplx* Tf = (cplx*)(ws + pl.off_tf);
+  cplx* G2 = GzR[0];
   const size_t qstride = pl.qstride;
   int nfull = 0;
   for (int pr = 0; pr < c->npairs; ++pr) nfull += c->full[pr];
@@ -1217,7 +1301,7 @@ static int collide_v1_impl(dgfs_ctx* c, const double* f, double* out, int nx, bo
     if (!c->full[pr] && c->v1_tsrc[pr] == pr) ++nrun_vhs;
   }
   const double fwd_xy = N * (N + 1.0) * 5.0 * N * log2((double)N);      // forward passes inside k_xy, once per plane
-  const int ns = c->ns, np = c->npairs, nz = c->v1_nz, nz0 = c->v1_nz0;
+  const int ns = c->ns, np = c->npairs, nz = c->v1_nz, nz0 = c->v1_nz0, nzr = nz - nz0;
   const size_t smem_plane = plane_smem_per_warp<N>() * W;
   const size_t smem_final = plane_smem_per_warp<N>() * 2;
   const size_t smem_xy = sizeof(cplx) * (size_t)W * JobSmem<N>::WORDS;
@@ -1226,19 +1310,19 @@ static int collide_v1_impl(dgfs_ctx* c, const double* f, double* out, int nx, bo
   const size_t smem_nyq = sizeof(cplx) * (size_t)2 * JobSmem<N>::WORDS;
   const size_t smem_zacc = sizeof(cplx) * (size_t)ZaccSmem<N>::STAGES * ZaccSmem<N>::WORDS;
   const size_t smem_zs = sizeof(cplx) * (size_t)N * 128;
-  static bool attr_done = false;
-  if (!attr_done) {
+  if (!c->v1_attr_done) {                 // per context, hence per device
     cudaFuncSetAttribute(k_plane_fwd<N, W, 0>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_plane);
     cudaFuncSetAttribute(k_plane_fwd<N, W, 1>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_plane);
     cudaFuncSetAttribute(k_final_xy_h<N>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_final);
     cudaFuncSetAttribute(k_xy<N, W>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_xy);
+    cudaFuncSetAttribute(k_xy<N, 2>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_xy / 2);
     cudaFuncSetAttribute(k_xy_full<N, W>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_xyf);
     cudaFuncSetAttribute(k_wterm<N>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_wt);
     cudaFuncSetAttribute(k_nyq2<N, 2>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_nyq);
     cudaFuncSetAttribute(k_zshift<N>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_zs);
     cudaFuncSetAttribute(k_zfwd_acc<N, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_zacc);
     cudaFuncSetAttribute(k_zfwd_acc<N, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_zacc);
-    attr_done = true;
+    c->v1_attr_done = true;
   }
   const int pen_blocks = (N2 + 127) / 128;
   const int hpen_blocks = (N * H + 127) / 128;
@@ -1258,8 +1342,10 @@ static int collide_v1_impl(dgfs_ctx* c, const double* f, double* out, int nx, bo
       double* fp = (double*)(ws + pl.off_fp);
       if ((rc = launch_nyquist_filter(c, fc, fp, nb * ns, st))) return rc;
       fc = fp;
-      cudaMemsetAsync(nyq, 0, pl.nyq_bytes, st);
-      cudaMemsetAsync(S, 0, (size_t)items * N3 * sizeof(double), st);
+      for (int b = 0; b < pl.nbuf; ++b) {
+        cudaMemsetAsync(nyqb[b], 0, pl.nyq_bytes, st);
+        cudaMemsetAsync(Sb[b], 0, (size_t)items * N3 * sizeof(double), st);
+      }
     }
     // step 1, once per species (R-2), plus the half-packed copy
     { ProfScope ps(c->prof, st, "k_zfwd_real", nb * ns * fft3 / 3.0);
@@ -1268,49 +1354,74 @@ static int collide_v1_impl(dgfs_ctx* c, const double* f, double* out, int nx, bo
       k_plane_fwd<N, W, 0><<<dim3(plane_blocks, nb * ns), 32 * W, smem_plane, st>>>(c->tab, T, 1, fhat, 0); }
     { ProfScope ps(c->prof, st, "k_pack_half", 0.0);
       k_pack_half<N><<<(nb * ns * N2 * H + 255) / 256, 256, 0, st>>>(fhat, fhh, nyqy, nb * ns); }
+    record(c->ev_head, st);
+    wait(sa, c->ev_head);
+    if (nvhs > 0) wait(sz, c->ev_head);
     if (nz0 > 0) {     // the unshifted arrays (sigma_z = 0), the same for every radial node
-      ProfScope ps(c->prof, st, "k_zshift", items * fl.zshift * nz0 / (nz - nz0 > 0 ? nz - nz0 : 1));
-      k_zshift<N><<<dim3(hpen_blocks, ns, nb), 128, smem_zs, st>>>(c->v1, ns, fhh, Gz, 0, nz - nz0, nz0);
+      ProfScope ps(c->prof, sa, "k_zshift", items * fl.zshift * nz0 / (nzr > 0 ? nzr : 1));
+      k_zshift<N><<<dim3(hpen_blocks, ns, nb), 128, smem_zs, sa>>>(c->v1, ns, fhh, Gz0, 0, nzr, nz0, nzr, nz0);
     }
+    int ngroups = 0;
     for (int r = 0; r < c->N_rho; ++r) {
-      if (nz > nz0)
-      { ProfScope ps(c->prof, st, "k_zshift", items * fl.zshift);
-        k_zshift<N><<<dim3(hpen_blocks, ns, nb), 128, smem_zs, st>>>(c->v1, ns, fhh, Gz, r, 0, nz - nz0); }
+      const int b = ov ? (r & 1) : 0;
+      // ---- prepare radial node r (stream sa)
+      if (r >= 2) wait(sa, c->ev_xy[b]);                     // the plane jobs of r - 2 have read buffer b
+      if (nzr > 0)
+      { ProfScope ps(c->prof, sa, "k_zshift", items * fl.zshift);
+        k_zshift<N><<<dim3(hpen_blocks, ns, nb), 128, smem_zs, sa>>>(c->v1, ns, fhh, GzR[b], r, 0, nzr, 0, nzr); }
       if (!c->nyq_filter) {
-      { ProfScope ps(c->prof, st, "k_nyq1d", nb * run_all * c->M * 16.0 * N2);
-        k_nyq1d<N><<<(items * c->M + 3) / 4, 128, 0, st>>>(c->v1, c->tab, fhat, nyq, r, items * c->M); }
-      { ProfScope ps(c->prof, st, "k_nyq2", nb * run_all * (fl.nyq - c->M * 16.0 * N2));
-        k_nyq2<N, 2><<<dim3(3, items), 64, smem_nyq, st>>>(c->v1, c->tab, fhh, nyqy, nyq, r); }
+      { ProfScope ps(c->prof, sa, "k_nyq1d", nb * run_all * c->M * 16.0 * N2);
+        k_nyq1d<N><<<(items * c->M + 3) / 4, 128, 0, sa>>>(c->v1, c->tab, fhat, nyqb[b], r, items * c->M); }
+      { ProfScope ps(c->prof, sa, "k_nyq2", nb * run_all * (fl.nyq - c->M * 16.0 * N2));
+        k_nyq2<N, 2><<<dim3(3, items), 64, smem_nyq, sa>>>(c->v1, c->tab, fhh, nyqy, nyqb[b], r); }
+      if (nvhs > 0)
+        { ProfScope ps(c->prof, sa, "k_wterm", nb * run_vhs * fl.wterm);
+          k_wterm<N><<<dim3(N / WtermSmem<N>::CZB, items), WtermSmem<N>::THREADS, smem_wt, sa>>>(nyqb[b], c->M, Sb[b], c->tab.full, np, c->v1.smask, c->v1.sskip, c->v1.tsrc); }
       }
+      record(c->ev_prep[b], sa);
+      // ---- plane jobs of radial node r (caller's stream)
+      wait(st, c->ev_prep[b]);
+      const GzView gv{GzR[b], Gz0, nzr, nz0};
       if (nvhs > 0) {
-        if (!c->nyq_filter)
-        { ProfScope ps(c->prof, st, "k_wterm", nb * run_vhs * fl.wterm);
-          k_wterm<N><<<dim3(N / WtermSmem<N>::CZB, items), WtermSmem<N>::THREADS, smem_wt, st>>>(nyq, c->M, S, c->tab.full, np, c->v1.smask, c->v1.sskip, c->v1.tsrc); }
+        const int g = r / RG, slot = r % pl.tslots;
+        if (r % RG == 0 && g >= 2) wait(st, c->ev_acc[g & 1]);       // the forward z pass of group g - 2 has read these slots
         { ProfScope ps(c->prof, st, "k_xy", nb * (run_vhs * (fl.xy - fwd_xy) + nrun_vhs * fwd_xy));
-          k_xy<N, W><<<dim3((N + W - 1) / W, items), 32 * W, smem_xy, st>>>(c->v1, c->tab, Gz, nyq, S, T + (size_t)(r % RG) * slot_stride, r); }
-        if ((r + 1) % RG == 0 || r + 1 == c->N_rho) {
-          const int r0 = (r / RG) * RG, nr = r + 1 - r0;
-          ProfScope ps(c->prof, st, "k_zfwd_acc", nb * nvhs * fl.acc * nr);
-          if (r0 == 0) k_zfwd_acc<N, true><<<dim3(hp_blocks, items), 128, smem_zacc, st>>>(c->tab, c->v1.tsrc, T, slot_stride, QG, qstride, r0, nr);
-          else k_zfwd_acc<N, false><<<dim3(hp_blocks, items), 128, smem_zacc, st>>>(c->tab, c->v1.tsrc, T, slot_stride, QG, qstride, r0, nr);
-        }
+          if (c->v1_xyw == 2)       // DGFS_V1_XYW=2: blocks of two warps, five per SM (ten warps at <= 204 registers)
+            k_xy<N, 2><<<dim3((N + 1) / 2, items), 64, smem_xy / 2, st>>>(c->v1, c->tab, gv, nyqb[b], Sb[b], T + (size_t)slot * slot_stride, r);
+          else
+            k_xy<N, W><<<dim3((N + W - 1) / W, items), 32 * W, smem_xy, st>>>(c->v1, c->tab, gv, nyqb[b], Sb[b], T + (size_t)slot * slot_stride, r); }
       }
       if (nfull > 0) {
         { ProfScope ps(c->prof, st, "k_xy_full", nb * (run_all - run_vhs) * fl.xy_full);
-          k_xy_full<N, W><<<dim3((N + W - 1) / W, items), 32 * W, smem_xyf, st>>>(c->v1, c->tab, Gz, nyq, Tf, r); }
+          k_xy_full<N, W><<<dim3((N + W - 1) / W, items), 32 * W, smem_xyf, st>>>(c->v1, c->tab, gv, nyqb[b], Tf, r); }
         { ProfScope ps(c->prof, st, "k_zfwd_full", nb * nfull * fl.acc_full);
           if (r == 0) k_zfwd_full<N, true><<<dim3(pen_blocks, items), 256, 0, st>>>(c->tab, c->v1, Tf, QG, qstride, r);
           else k_zfwd_full<N, false><<<dim3(pen_blocks, items), 256, 0, st>>>(c->tab, c->v1, Tf, QG, qstride, r); }
       }
+      record(c->ev_xy[b], st);
+      // ---- forward z pass and QG accumulation of a finished group of radial nodes (stream sz)
+      if (nvhs > 0 && ((r + 1) % RG == 0 || r + 1 == c->N_rho)) {
+        const int g = r / RG, r0 = g * RG, nr = r + 1 - r0;
+        record(c->ev_grp[g & 1], st);
+        wait(sz, c->ev_grp[g & 1]);
+        const cplx* Tg = T + (size_t)(r0 % pl.tslots) * slot_stride;
+        { ProfScope ps(c->prof, sz, "k_zfwd_acc", nb * nvhs * fl.acc * nr);
+          if (r0 == 0) k_zfwd_acc<N, true><<<dim3(hp_blocks, items), 128, smem_zacc, sz>>>(c->tab, c->v1.tsrc, Tg, slot_stride, QG, qstride, r0, nr);
+          else k_zfwd_acc<N, false><<<dim3(hp_blocks, items), 128, smem_zacc, sz>>>(c->tab, c->v1.tsrc, Tg, slot_stride, QG, qstride, r0, nr); }
+        record(c->ev_acc[g & 1], sz);
+        ngroups = g + 1;
+      }
     }
+    // join: the last groups' accumulation into QG (sz is in order, so the last event covers the earlier ones)
+    if (ngroups > 0) wait(st, c->ev_acc[(ngroups - 1) & 1]);
     // step 10
     { ProfScope ps(c->prof, st, "k_final_xy", items * (2.0 * fft3 * 2.0 / 3.0 + 6.0 * N3));
-      k_final_xy_h<N><<<dim3(N, items), 64, smem_final, st>>>(c->tab, fhat, QG, qstride, Gz); }
+      k_final_xy_h<N><<<dim3(N, items), 64, smem_final, st>>>(c->tab, fhat, QG, qstride, G2); }
     { ProfScope ps(c->prof, st, "k_z_final", items * (2.0 * fft3 / 3.0 + 5.0 * N3));
       if (pairs_out)
-        k_z_final<N, false><<<dim3(pen_blocks, items), 128, 0, st>>>(c->tab, Gz, fc, out + (size_t)x0 * np * N3);
+        k_z_final<N, false><<<dim3(pen_blocks, items), 128, 0, st>>>(c->tab, G2, fc, out + (size_t)x0 * np * N3);
       else
-        k_z_final<N, true><<<dim3(pen_blocks, nb * ns), 128, 0, st>>>(c->tab, Gz, fc, out + (size_t)x0 * ns * N3); }
+        k_z_final<N, true><<<dim3(pen_blocks, nb * ns), 128, 0, st>>>(c->tab, G2, fc, out + (size_t)x0 * ns * N3); }
   }
   return check_cuda(c, cudaGetLastError(), "collide (v1) launch");
 }

@@ -16,7 +16,7 @@
 
 namespace dgfs {
 
-static std::string g_create_error;
+static thread_local std::string g_create_error;   // per thread: dgfs_last_error(NULL) reports the calling thread's last failed dgfs_create
 
 int set_error(dgfs_ctx* c, int code, const std::string& msg) {
   if (c) c->err = msg; else g_create_error = msg;
@@ -516,7 +516,11 @@ extern "C" int dgfs_create(const dgfs_params* P, dgfs_ctx** out) {
     if (rg && atoi(rg) > 0) c->v1_rgroup = atoi(rg);
     if (c->v1_rgroup > c->N_rho) c->v1_rgroup = c->N_rho;
     rc = build_tables_v1(c);
+    if (rc == DGFS_OK) rc = init_streams_v1(c);
     if (rc != DGFS_OK) { g_create_error = c->err; dgfs_destroy(c); return rc; }
+  }
+  if ((rc = check_cuda(c, cudaEventCreateWithFlags(&c->ev_last, cudaEventDisableTiming), "event create")) != DGFS_OK) {
+    g_create_error = c->err; dgfs_destroy(c); return rc;
   }
   *out = c;
   return DGFS_OK;
@@ -531,6 +535,8 @@ extern "C" void dgfs_destroy(dgfs_ctx* c) {
   for (auto p : c->h_bfull) cudaFree(p);
   cudaFree(c->ws); cudaFree(c->dg_ws);
   free_tables_v1(c);
+  free_streams_v1(c);
+  if (c->ev_last) cudaEventDestroy(c->ev_last);
   for (int b = 0; b < 2; ++b) { cudaFree(c->hp_f[b]); cudaFree(c->hp_q[b]); }
   for (int i = 0; i < 3; ++i) {
     if (c->hp_stream[i]) cudaStreamDestroy(c->hp_stream[i]);

@@ -116,6 +116,10 @@ struct dgfs_ctx {
   int v1_nz = 0, v1_nz0 = 0;             // z jobs; the last v1_nz0 of them have sigma_z = 0
   std::vector<int> v1_zsp, v1_zmap, v1_tsrc, v1_fsrc_s, v1_anti, v1_tpartner;
   std::vector<double> v1_fscale;
+  std::vector<int4> v1_jobs;
+  std::vector<int> v1_njobs;
+  int4* d_v1_jobs = nullptr;
+  int* d_v1_njobs = nullptr;
   int *d_v1_zsp = nullptr, *d_v1_zmap = nullptr, *d_v1_tsrc = nullptr, *d_v1_fsrc_s = nullptr, *d_v1_anti = nullptr, *d_v1_tpartner = nullptr;
   double* d_v1_fscale = nullptr;
   dgfs::cplx *d_v1_hz = nullptr, *d_v1_hxy = nullptr;
@@ -123,6 +127,20 @@ struct dgfs_ctx {
   std::vector<unsigned char> v1_smask, v1_sskip;
   unsigned char *d_v1_smask = nullptr, *d_v1_sskip = nullptr;
   dgfs::V1Tables v1{};
+  // v1 pipeline, two-stream schedule (collide_v1.cu "host orchestration"): the kernels that prepare radial node
+  // r + 1 (z shifts, Nyquist fields, their product term; bound by memory and latency) run on `aux`, a
+  // high-priority stream of the library, while the plane jobs of radial node r (bound by the FP64 pipe) run on
+  // the caller's stream; double-buffered intermediates, ordered by these events
+  int v1_xyw = 4;                        // warps per k_xy block (DGFS_V1_XYW)
+  int v1_overlap = 0;                    // DGFS_V1_OVERLAP=1: three streams (default: everything on the caller's stream)
+  cudaStream_t aux = nullptr, aux2 = nullptr;
+  bool v1_attr_done = false, v0_attr_done = false;   // dynamic shared-memory opt-in, once per context (= per device)
+  cudaEvent_t ev_head = nullptr, ev_prep[2] = {nullptr, nullptr}, ev_xy[2] = {nullptr, nullptr};
+  cudaEvent_t ev_grp[2] = {nullptr, nullptr}, ev_acc[2] = {nullptr, nullptr};
+  // the workspace belongs to one call at a time: every call waits for the previous one's last launch
+  cudaEvent_t ev_last = nullptr;
+  bool ev_last_set = false;
+  bool pool_set = false;                 // release threshold of the stream-ordered allocator raised
   // workspace (grown on demand)
   void* ws = nullptr;
   size_t ws_bytes = 0;
@@ -153,12 +171,14 @@ struct ChunkPlan {
 };
 ChunkPlan plan_chunks(const dgfs_ctx* c, int nx);
 int run_collide(dgfs_ctx* c, const double* f, double* out, int nx, bool pairs_out, cudaStream_t st);
-int ensure_workspace(dgfs_ctx* c, size_t bytes);
+int ensure_workspace(dgfs_ctx* c, size_t bytes, cudaStream_t st);
 // P f = prod_d (1 - E_d) f on `narr` arrays of N^3 values (dgfs_params::nyquist_filter): src -> dst
 int launch_nyquist_filter(dgfs_ctx* c, const double* src, double* dst, int narr, cudaStream_t st);
 // collide_v1.cu
 int build_tables_v1(dgfs_ctx* c);
 void free_tables_v1(dgfs_ctx* c);
+int init_streams_v1(dgfs_ctx* c);
+void free_streams_v1(dgfs_ctx* c);
 size_t workspace_bytes_v1(const dgfs_ctx* c, int nx);
 int run_collide_v1(dgfs_ctx* c, const double* f, double* out, int nx, bool pairs_out, cudaStream_t st);
 double flops_per_pair_eval_v1(const dgfs_ctx* c, int pair);

@@ -26,6 +26,8 @@ struct V1Tables {
                              //            tsrc[pair]) equals this one's up to the factor fscale (R-10 / R-11)
   const double* fscale;      // [pair][s]
   const unsigned char* sskip; // [pair][s]  1: sphere point not run for this pair, its antipode carries both weights (R-10)
+  const int4* jobs;          // [pair][M]  plane jobs the pair runs, in order: {s, z job of side A, z job of side B, smask[s]}
+  const int* njobs;          // [pair]     how many (0 for a pair that reuses another pair's products)
   const unsigned char* smask; // [s]  bit d set: sigma_{s,d} = 0, so s_d = 0 for every pair and radial node and
                              //      the Nyquist field of that axis (ux', uy, uz for d = x, y, z) vanishes identically
 };
