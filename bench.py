@@ -1,15 +1,17 @@
 #!/usr/bin/env python
-"""Benchmark of the hot path: one step = one dgfs_collide over the whole spatial batch of config
-c2 (BASELINE.json configs[2]: N=32, N_rho=32, M=12, 2 species, 4096 points) per GPU.
+"""Benchmark of the hot path.  Default workload: config c2 of BASELINE.json (N=32, N_rho=32, M=12, 2 species, 4096
+points per GPU); one step = one dgfs_collide over the whole spatial batch.
 
-  python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference] [--workload c2] [--nx n]
+  python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference] [--workload c0|c1|c2|c3|c4|couette] [--nx n]
 
-Prints ONE JSON line (rank 0).  metric = pair-evals/s = spatial points x species pairs per second,
-whole job.  See DESIGN.md "Measurement" for the roofline arithmetic.
+c3 / couette: one step = one dgfs_step (SSP-RK3, three collide calls) / dgfs_step_euler step of the DG slab.
+Prints ONE JSON line (rank 0).  metric = pair-evals/s = spatial points x species pairs per second, whole job.
+See DESIGN.md section 8 for the roofline arithmetic.
 """
 import argparse
 import dataclasses
 import json
+import multiprocessing as mp
 import os
 import sys
 import threading
@@ -21,13 +23,12 @@ if ROOT not in sys.path:
 
 METRIC = "collision evals/s (spatial pts x species pairs) at N=32"
 UNIT = "pair-evals/s"
-# FP64 DFMA pipe: 148 SMs x 64 DFMA/clk/SM x 2 flop x 1.965 GHz.  The same
-# pipe is also measured live with dgfs_measure_fp64_peak (dependency-free DFMA chains) and reported.
+# FP64 DFMA pipe: 148 SMs x 64 DFMA/clk/SM x 2 flop x 1.965 GHz.  The same pipe is also
+# measured live with dgfs_measure_fp64_peak (dependency-free DFMA chains) and reported beside it.
 FP64_PEAK_NOMINAL_TFLOPS = 148 * 64 * 2 * 1.965e9 / 1e12
 PAPER_P100_PAIR_EVALS_PER_S = 1.0 / 0.01057      # Table 1 P:316 (N=32, N_rho=32, M=12), 1 x P100
-# dram__bytes_read.sum + dram__bytes_write.sum of one k_xy launch over 512 points (all pairs, one radial node) at
-# the c2 operating point, from the `ncu --set full` capture summarised in profiles/r01_v1_ncu.md
-NCU_DRAM_BYTES_PER_POINT = {"k_xy": (2.842e9 + 0.4463e9) / 512}
+HBM_FALLBACK_GBS = 6650.0                        # B200_PROFILING.md fallback when MEASURED_PEAKS.json is absent
+TRAFFIC_JSON = os.path.join(ROOT, "profiles", "r02_traffic.json")
 
 
 def parse():
@@ -36,9 +37,11 @@ def parse():
     ap.add_argument("--steps", type=int, default=3)
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
-    ap.add_argument("--workload", default="c2")
+    ap.add_argument("--workload", default="c2", choices=["c0", "c1", "c2", "c3", "c4", "couette"])
     ap.add_argument("--nx", type=int, default=0, help="override the batch size (debugging only; reported)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--precision", default="f64", choices=["f64", "f32"],
+                    help="f32: dgfs_params.precision = 1 (SURVEY 8(f) item 1; not the headline metric)")
     ap.add_argument("--nyquist-filter", action="store_true",
                     help="time the variant operator Q(P f_p, P f_q) (dgfs_params.nyquist_filter); not the headline metric")
     return ap.parse_args()
@@ -88,63 +91,145 @@ class ClockSampler(threading.Thread):
                 "reasons": sorted(self.reasons), "samples": len(s)}
 
 
-def oracle_sample(cfg, n_points):
-    """Time the oracle, as it stands, on n_points points of the workload (all pairs), taken alternately from
-    the start and from the middle of the batch (both halves of the c2 mix).  Returns (pair_evals, seconds, cores)."""
-    from workloads import make_points
-    from oracle.tables import precompute
-    from oracle.collide import collide_pairs
+# ------------------------------------------------------------------------------ the CPU oracle, timed
+_ORACLE = {}
+
+
+def _oracle_eval(task):
+    from oracle.collide import collide_pair
+    x, p, q = task
+    return float(collide_pair(_ORACLE["tab"], p, q, _ORACLE["f"][x, p], _ORACLE["f"][x, q])[0])
+
+
+def cpu_model():
+    try:
+        for line in open("/proc/cpuinfo"):
+            if line.startswith("model name"):
+                return line.split(":", 1)[1].strip()
+    except OSError:
+        pass
+    return "unknown"
+
+
+def sample_state(cfg, n_points):
+    """n_points spatial points of the workload for the oracle: alternately from the start and from the middle of a
+    homogeneous batch (both halves of the c2 mix); the first DOF of a DG state."""
+    from workloads import make_points, make_dg_state
+    if cfg.kind in ("dg", "couette"):
+        f = make_dg_state(cfg).reshape(-1, cfg.ns, cfg.N ** 3)
+        return f[:: max(1, f.shape[0] // n_points)][:n_points].copy()
     xs = [(i // 2) + (cfg.nx // 2 if i % 2 else 0) for i in range(n_points)]
-    f = make_points(cfg, xs)
-    tab = precompute(cfg.N, cfg.N_rho, cfg.M, cfg.L, cfg.mass, cfg.omega, cfg.alpha)   # create: untimed
+    return make_points(cfg, xs)
+
+
+def oracle_sample(cfg, n_points, tab=None):
+    """Time the oracle, as it stands, on n_points points of the workload, all pairs: one oracle.collide.collide_pair
+    per (point, pair), spread over all host cores by a forked process pool (tables built before, untimed).
+    Returns (pair_evals, seconds, workers, tables)."""
+    from oracle.tables import precompute
+    f = sample_state(cfg, n_points)
+    if tab is None:
+        vss = any(a != 1.0 for row in cfg.alpha for a in row)
+        kn = {"kn": cfg.kn} if cfg.kn else {}
+        tab = precompute(cfg.N, cfg.N_rho, cfg.M, cfg.L, cfg.mass, cfg.omega, cfg.alpha,
+                         workers=(os.cpu_count() or 1) if vss else 1, **kn)   # create: untimed
+    tasks = [(x, p, q) for x in range(f.shape[0]) for p in range(cfg.ns) for q in range(cfg.ns)]
+    workers = max(1, min(os.cpu_count() or 1, len(tasks)))
+    _ORACLE["tab"], _ORACLE["f"] = tab, f
     t0 = time.perf_counter()
-    collide_pairs(tab, f)
+    if workers == 1:
+        for t in tasks:
+            _oracle_eval(t)
+    else:
+        with mp.get_context("fork").Pool(workers) as pool:
+            pool.map(_oracle_eval, tasks, chunksize=1)
     dt = time.perf_counter() - t0
-    return n_points * cfg.ns * cfg.ns, dt, 1
+    _ORACLE.clear()
+    return len(tasks), dt, workers, tab
+
+
+def oracle_points(cfg):
+    """Sample size giving roughly 10-30 s of CPU work per timing at 16 cores."""
+    return {"c0": 4, "c1": 32, "c2": 16, "c3": 16, "c4": 4, "couette": 16}[cfg.name]
+
+
+def workload_desc(cfg, nx, ngpus, stages):
+    kinds = {"bimaxwell": "bi-Maxwellian inputs", "c2mix": "half near-equilibrium, half bi-Maxwellian",
+             "dg": "1-D DG slab, %d elements of order %d, diffuse walls, one SSP-RK3 step of dgfs_step" % (cfg.ne, cfg.order),
+             "couette": "Couette case C-01 (Table 2), %d elements of order %d, one Euler step of dgfs_step_euler" % (cfg.ne, cfg.order)}
+    vss = sum(a != 1.0 for row in cfg.alpha for a in row)
+    phys = "%d species, masses %s, %d of %d pairs VSS" % (cfg.ns, "/".join("%.4g" % m for m in cfg.mass), vss, cfg.ns ** 2)
+    return {"workload": "%s: %s; N=%d, N_rho=%d, M=%d, L=%g, nx=%d spatial points per GPU (%s)" % (
+                cfg.name, phys, cfg.N, cfg.N_rho, cfg.M, cfg.L, nx, kinds[cfg.kind]),
+            "N": cfg.N, "N_rho": cfg.N_rho, "M": cfg.M, "ns": cfg.ns, "nx_per_gpu": nx,
+            "collide_calls_per_step": stages, "pair_evals_per_step": stages * nx * cfg.ns * cfg.ns * ngpus,
+            "parallelism": "replicated tables, nx sharded over %d GPU(s), no collective" % ngpus,
+            "l2": ("inputs (%.2f GB per GPU) exceed the 126 MB L2; no flush needed" % (nx * cfg.ns * cfg.N ** 3 * 8 / 1e9)
+                   if nx * cfg.ns * cfg.N ** 3 * 8 > 126e6 else
+                   "state (%.1f MB) fits the L2; 256 MB written between timed steps to flush it" % (nx * cfg.ns * cfg.N ** 3 * 8 / 1e6))}
+
+
+def stages_of(cfg):
+    return 3 if cfg.kind == "dg" else 1
 
 
 def run_reference(args, cfg, rank):
-    """--impl reference: the CPU oracle on the host cores (kind = oracle)."""
+    """--impl reference: the CPU oracle on the host cores (kind = oracle); each step a bounded sample."""
     if rank != 0:
         return
-    sample_pts = 2
-    times = []
-    evals = 0
+    npts = oracle_points(cfg)
+    times, evals, workers, tab = [], 0, 1, None
     for i in range(args.warmup + args.steps):
-        evals, dt, cores = oracle_sample(cfg, sample_pts)
+        evals, dt, workers, tab = oracle_sample(cfg, npts, tab)
         if i >= args.warmup:
             times.append(dt)
         if sum(times) > 240:
             break
     t = sum(times) / len(times)
     val = evals / t
-    sample = "%d point(s) x %d pairs of %s per step (oracle collide_pairs, numpy single thread)" % (
-        sample_pts, cfg.ns * cfg.ns, cfg.name)
+    sample = "%d point(s) x %d pairs of %s per step (oracle.collide.collide_pair per (point, pair), %d worker processes on %s)" % (
+        npts, cfg.ns * cfg.ns, cfg.name, workers, cpu_model())
     print(json.dumps({
         "impl": "reference", "metric": METRIC, "value": val, "unit": UNIT, "n_gpus": args.gpus,
         "steps": len(times), "warmup": args.warmup, "ms_per_step": 1e3 * t, "higher_is_better": True,
         "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
-        "config": workload_desc(cfg, cfg.nx, args.gpus),
-        "cpu_baseline": {"value": val, "unit": UNIT, "cores": 1, "kind": "oracle", "sample": sample},
+        "config": workload_desc(cfg, cfg.nx, args.gpus, stages_of(cfg)),
+        "cpu_baseline": {"value": val, "unit": UNIT, "cores": workers, "kind": "oracle", "sample": sample},
         "e2e": {"value": val, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
         "gpu_launches": 0,
     }))
 
 
-def workload_desc(cfg, nx, ngpus):
-    return {"workload": "%s: homogeneous %d-species Ar/Kr VHS collide, N=%d, N_rho=%d, M=%d, L=%g, "
-                        "nx=%d points per GPU (half near-equilibrium, half bi-Maxwellian)" % (
-                            cfg.name, cfg.ns, cfg.N, cfg.N_rho, cfg.M, cfg.L, nx),
-            "N": cfg.N, "N_rho": cfg.N_rho, "M": cfg.M, "ns": cfg.ns, "nx_per_gpu": nx,
-            "pair_evals_per_step": nx * cfg.ns * cfg.ns * ngpus,
-            "parallelism": "replicated tables, nx sharded over %d GPU(s), no collective" % ngpus,
-            "l2": "inputs (%.2f GB per GPU) exceed the 126 MB L2; no flush needed" % (
-                nx * cfg.ns * cfg.N ** 3 * 8 / 1e9)}
+def measured_hbm_gbs():
+    try:
+        with open(os.path.join(ROOT, "MEASURED_PEAKS.json")) as fh:
+            return float(json.load(fh)["hbm_gbs"]), "MEASURED_PEAKS.json (measured copy bandwidth)"
+    except Exception:
+        return HBM_FALLBACK_GBS, "B200_PROFILING.md fallback"
+
+
+def step_traffic(cfg, prof, steps):
+    """DRAM bytes of one step from this round's ncu capture (profiles/r02_traffic.json: dram__bytes_read.sum +
+    dram__bytes_write.sum per launch of each kernel class at the c2 operating point, 512-point chunk), scaled by
+    the launches the live run made.  None for other operating points."""
+    try:
+        with open(TRAFFIC_JSON) as fh:
+            tj = json.load(fh)
+    except Exception:
+        return None, None
+    if (cfg.N, cfg.N_rho, cfg.M, cfg.ns) != tuple(tj["operating_point"]):
+        return None, tj
+    per = tj["dram_bytes_per_launch"]
+    total = 0.0
+    for p in prof:
+        if p["name"] in per:
+            total += per[p["name"]] * p["launches"] / steps
+    return total, tj
 
 
 def main():
     args = parse()
-    from workloads import get_config, make_points
+    from workloads import get_config, make_points, make_dg_state
     cfg = get_config(args.workload)
     rank = int(os.environ.get("RANK", "0"))
     world = int(os.environ.get("WORLD_SIZE", "1"))
@@ -153,7 +238,6 @@ def main():
         run_reference(args, cfg, rank)
         return
 
-    import numpy as np
     import torch
     import torch.distributed as dist
     if not torch.cuda.is_available():
@@ -166,64 +250,90 @@ def main():
         entry.build()
     if world > 1:
         dist.barrier()
-    from paper_1903_04670_b200 import Dgfs
+    from paper_1903_04670_b200 import Dgfs, Mesh1D, api
     from paper_1903_04670_b200.parallel import rank_seed, max_over_ranks, whole_job_rate
 
-    nx = args.nx if args.nx > 0 else cfg.nx
+    is_dg = cfg.kind in ("dg", "couette")
+    stages = stages_of(cfg)
     # weak scaling: every rank owns its own nx points (rank r draws them with seed + 1000 r)
     rcfg = dataclasses.replace(cfg, seed=rank_seed(cfg.seed, rank))
-    if nx == cfg.nx:
-        f_np = make_points(rcfg, range(nx))
-    else:      # reduced batch keeps both halves of the c2 mix
-        half = nx // 2
-        xs = list(range(half)) + list(range(cfg.nx - (nx - half), cfg.nx))
-        f_np = make_points(rcfg, xs)
+    if is_dg:
+        f_np = make_dg_state(rcfg)
+        nx = cfg.ne * (cfg.order + 1)
+        mesh = Mesh1D(cfg.ne, cfg.order, wall_T=cfg.wall_T, wall_u=cfg.wall_u)
+    else:
+        nx = args.nx if args.nx > 0 else cfg.nx
+        if nx == cfg.nx:
+            f_np = make_points(rcfg, range(nx))
+        else:      # reduced batch keeps both halves of the c2 mix
+            half = nx // 2
+            f_np = make_points(rcfg, list(range(half)) + list(range(cfg.nx - (nx - half), cfg.nx)))
     f_host = torch.from_numpy(f_np).pin_memory()
     q_host = torch.empty_like(f_host).pin_memory()
-    op = Dgfs.from_config(cfg, device=local, nyquist_filter=args.nyquist_filter)
+    kw = {"nyquist_filter": True} if args.nyquist_filter else {}
+    if args.precision == "f32":
+        kw["precision"] = 1
+    op = Dgfs.from_config(cfg, device=local, **kw)
     op.reserve(nx)
     f_dev = f_host.cuda()
     q_dev = torch.empty_like(f_dev)
     stream = torch.cuda.current_stream()
+    small = f_dev.numel() * 8 <= 126e6
+    flush = torch.empty(256 << 20, dtype=torch.uint8, device="cuda") if small else None
 
     def barrier():
         if world > 1:
             dist.barrier()
         torch.cuda.synchronize()
 
+    def step_device():
+        if is_dg:
+            (api.dgfs_step if cfg.scheme == "rk3" else api.dgfs_step_euler)(op.ctx, mesh, f_dev, cfg.dt, 1)
+        else:
+            op.collide(f_dev, q_dev)
+
     # ---------------- device-resident timing ----------------
     for _ in range(args.warmup):
-        op.collide(f_dev, q_dev)
+        step_device()
     barrier()
     op.profile(on=True, reset=True)
     launches0 = op.launch_count()
     sampler = ClockSampler(local)
     sampler.start()
-    ev = [torch.cuda.Event(enable_timing=True) for _ in range(args.steps + 1)]
-    ev[0].record(stream)
+    ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(args.steps)]
     for i in range(args.steps):
-        op.collide(f_dev, q_dev)
-        ev[i + 1].record(stream)
+        if flush is not None:
+            flush.fill_(i)                 # L2 flush between timed steps, outside the timed intervals
+        ev[i][0].record(stream)
+        step_device()
+        ev[i][1].record(stream)
     barrier()
     sampler.stop_flag = True
     sampler.join()
-    total_ms = ev[0].elapsed_time(ev[-1])
+    total_ms = sum(a.elapsed_time(b) for a, b in ev)
     prof = op.profile(on=False)
     launches = op.launch_count() - launches0
     total_ms = max_over_ranks(total_ms)
     ms_per_step = total_ms / args.steps
-    evals_per_step = nx * cfg.ns * cfg.ns * world
-    value = whole_job_rate(nx * cfg.ns * cfg.ns, world, ms_per_step)
+    evals_rank = stages * nx * cfg.ns * cfg.ns
+    value = whole_job_rate(evals_rank, world, ms_per_step)
 
-    # ---------------- end to end: pinned host -> device -> collide -> pinned host ----------------
-    # dgfs_collide_host: HOST pointers in and out; the library's own streams carry the copies and the
-    # kernels, and the call returns when Q is in host memory, so the region is timed on the host
-    # clock between two device synchronisations (CUDA events on torch's stream would not see it).
-    del f_dev, q_dev
-    torch.cuda.empty_cache()
+    # ---------------- end to end: pinned host -> device -> step -> pinned host ----------------
+    # homogeneous workloads: dgfs_collide_host (HOST pointers in and out; the library's own streams carry the copies
+    # and the kernels; returns when Q is in host memory).  DG workloads: state up, one step, state down.  Timed on the
+    # host clock between two device synchronisations.
+    if not is_dg:
+        del f_dev, q_dev
+        torch.cuda.empty_cache()
 
     def e2e_step():
-        op.collide_host(f_host, q_host)
+        if is_dg:
+            f_dev.copy_(f_host, non_blocking=True)
+            step_device()
+            q_host.copy_(f_dev, non_blocking=True)
+            torch.cuda.synchronize()
+        else:
+            op.collide_host(f_host, q_host)
 
     e2e_step()
     barrier()
@@ -235,62 +345,88 @@ def main():
     nbytes = f_host.numel() * 8
 
     if rank == 0:
-        # ---------------- roofline of the dominant kernel class ----------------
-        prof = [p for p in prof if p["launches"] > 0]
-        top = max(prof, key=lambda p: p["ms"])
-        ksum = sum(p["ms"] for p in prof)
-        achieved = top["flops"] / (top["ms"] * 1e-3) / 1e12
-        flops_step = sum(op.flops_per_pair_eval(p, q) for p in range(cfg.ns) for q in range(cfg.ns)) * nx
-        from paper_1903_04670_b200 import dgfs_measure_fp64_peak
-        FP64_PEAK_MEASURED_TFLOPS = dgfs_measure_fp64_peak(local, 2.0)[1]
-        roofline = {
-            "bound": "alu", "kernel": top["name"], "achieved": achieved, "peak": FP64_PEAK_NOMINAL_TFLOPS,
-            "unit": "TFLOP/s", "frac": achieved / FP64_PEAK_NOMINAL_TFLOPS,
-            "peak_source": "FP64 DFMA pipe, 148 SM x 64 DFMA/clk x 2 x 1.965 GHz (DESIGN.md); "
-                           "MEASURED_PEAKS.json has no fp64 entry",
-            "frac_of_measured_dfma_peak": achieved / FP64_PEAK_MEASURED_TFLOPS,
-            "measured_dfma_peak": FP64_PEAK_MEASURED_TFLOPS,
-            "measured_dfma_peak_how": "dgfs_measure_fp64_peak: dependency-free DFMA chains, 2 s sustained, same box",
-            "kernel_share_of_step": top["ms"] / ksum,
-            "launch_ms": top["ms"] / top["launches"], "launches": top["launches"],
-            "flops_per_launch": top["flops"] / top["launches"],
-            "whole_step_tflops": flops_step / (ms_per_step * 1e-3) / 1e12 / 1.0,
-            "whole_step_frac": flops_step / (ms_per_step * 1e-3) / 1e12 / FP64_PEAK_NOMINAL_TFLOPS,
-            "traffic": (NCU_DRAM_BYTES_PER_POINT[top["name"]] * (nx * cfg.N_rho / top["launches"] * args.steps)
-                        if top["name"] in NCU_DRAM_BYTES_PER_POINT and (cfg.N, cfg.N_rho, cfg.M) == (32, 32, 12) else None),
-            "traffic_note": "DRAM bytes per launch of the dominant kernel, scaled from the ncu capture in "
-                            "profiles/r01_v1_ncu.md (6.42 MB per point and radial node); algorithmic bytes per point: "
-                            "4.72 MB z-shifted half planes + 0.79 MB S + 0.83 MB T for the three pairs that run",
-            "kernels": [{"name": p["name"], "launches": p["launches"], "ms": round(p["ms"], 3),
-                         "tflops": (p["flops"] / (p["ms"] * 1e-3) / 1e12 if p["ms"] > 0 else None)} for p in prof],
-        }
-        cpu = None
-        if world == 1 and not args.no_cpu_baseline:
-            npts = 4
-            ev_n, dt, cores = oracle_sample(cfg, npts)
-            cpu = {"value": ev_n / dt, "unit": UNIT, "cores": cores, "kind": "oracle",
-                   "sample": "%d points of %s (two from each half of the batch), all %d pairs, %.1f s (oracle "
-                             "collide_pairs, numpy, one thread, tables untimed)" % (npts, cfg.name, cfg.ns * cfg.ns, dt)}
-        out = {
-            "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
-            "warmup": args.warmup, "ms_per_step": ms_per_step, "higher_is_better": True, "scaling": "weak",
-            "vs_baseline": value / world / PAPER_P100_PAIR_EVALS_PER_S if cfg.name == "c2" else None,
-            "vs_baseline_note": "per-GPU value / 94.6 pair-evals/s: paper Table 1 (P:316), 1 x Tesla P100, same "
-                                "(N, N_rho, M) operating point, BKW workload; context, not the target",
-            "dtype": "f64", "data": "synthetic",
-            "config": dict(workload_desc(cfg, nx, world), **({"variant": "nyquist_filter"} if args.nyquist_filter else {})),
-            "clocks": sampler.summary(),
-            "e2e": {"value": evals_per_step / (e2e_ms * 1e-3), "unit": UNIT, "ms_per_step": e2e_ms,
-                    "h2d_bytes_per_step": nbytes, "d2h_bytes_per_step": nbytes,
-                    "call": "dgfs_collide_host (C ABI, pinned host buffers in and out, host clock)"},
-            "gpu_launches": launches,
-            "roofline": roofline,
-            "cpu_baseline": cpu,
-        }
-        print(json.dumps(out))
+        report(args, cfg, op, prof, nx, world, stages, ms_per_step, value, e2e_ms, nbytes, launches, sampler, local, is_dg)
     op.close()
     if world > 1:
         dist.destroy_process_group()
+
+
+def report(args, cfg, op, prof, nx, world, stages, ms_per_step, value, e2e_ms, nbytes, launches, sampler, local, is_dg):
+    from paper_1903_04670_b200 import dgfs_measure_fp64_peak
+    prof = [p for p in prof if p["launches"] > 0]
+    top = max(prof, key=lambda p: p["ms"])
+    ksum = sum(p["ms"] for p in prof)
+    kernel_tflops = top["flops"] / (top["ms"] * 1e-3) / 1e12
+    flops_step = stages * nx * sum(op.flops_per_pair_eval(p, q) for p in range(cfg.ns) for q in range(cfg.ns))
+    step_tflops = flops_step / (ms_per_step * 1e-3) / 1e12
+    peak_meas = dgfs_measure_fp64_peak(local, 2.0)[1]
+    hbm_gbs, hbm_src = measured_hbm_gbs()
+    dram_step, tj = step_traffic(cfg, prof, args.steps)
+    flops_floor_ms = flops_step / (FP64_PEAK_NOMINAL_TFLOPS * 1e12) * 1e3
+    bytes_floor_ms = dram_step / (hbm_gbs * 1e9) * 1e3 if dram_step else None
+    # north_star: the roofline is the slower of flops at the FP64 peak and bytes at the HBM bandwidth
+    bound = "hbm" if (bytes_floor_ms and bytes_floor_ms > flops_floor_ms) else "alu"
+    floor_ms = max(flops_floor_ms, bytes_floor_ms or 0.0)
+    top_traffic = tj["dram_bytes_per_launch"].get(top["name"]) if (tj and dram_step) else None
+    roofline = {
+        "bound": bound,
+        # the whole step against its roofline (executed-algorithm flops of ALL kernels / step time / FP64 peak when
+        # alu-bound; DRAM bytes of the step / step time / HBM bandwidth when hbm-bound): north_star's figure
+        "frac": floor_ms / ms_per_step,
+        "achieved": step_tflops if bound == "alu" else dram_step / (ms_per_step * 1e-3) / 1e9,
+        "peak": FP64_PEAK_NOMINAL_TFLOPS if bound == "alu" else hbm_gbs,
+        "unit": "TFLOP/s" if bound == "alu" else "GB/s",
+        "peak_source": ("FP64 DFMA pipe, 148 SM x 64 DFMA/clk x 2 x 1.965 GHz (DESIGN.md section 8); "
+                        "MEASURED_PEAKS.json has no fp64 entry") if bound == "alu" else hbm_src,
+        "scope": "whole step (every kernel of dgfs_collide), flop count of the algorithm as executed",
+        "flops_floor_ms": flops_floor_ms, "bytes_floor_ms": bytes_floor_ms, "step_ms": ms_per_step,
+        "step_flops": flops_step, "step_dram_bytes": dram_step,
+        "frac_of_measured_dfma_peak": step_tflops / peak_meas,
+        "measured_dfma_peak": peak_meas,
+        "measured_dfma_peak_how": "dgfs_measure_fp64_peak: dependency-free DFMA chains, 2 s sustained, same box",
+        "hbm_gbs": hbm_gbs,
+        # the dominant kernel class, from the library's per-launch CUDA events on the launching stream
+        "kernel": top["name"], "kernel_frac": kernel_tflops / FP64_PEAK_NOMINAL_TFLOPS,
+        "kernel_tflops": kernel_tflops, "kernel_share_of_step": top["ms"] / ksum,
+        "launch_ms": top["ms"] / top["launches"], "launches": top["launches"],
+        "flops_per_launch": top["flops"] / top["launches"],
+        "traffic": top_traffic,
+        "traffic_note": ("dram__bytes_read.sum + dram__bytes_write.sum per launch of the dominant kernel and per step, from "
+                         "profiles/r02_traffic.json (%s)" % tj.get("source", "") if tj else
+                         "no ncu capture for this operating point"),
+        "kernels": [{"name": p["name"], "launches": p["launches"], "ms": round(p["ms"], 3),
+                     "tflops": (p["flops"] / (p["ms"] * 1e-3) / 1e12 if p["ms"] > 0 else None)} for p in prof],
+    }
+    cpu = None
+    if world == 1 and not args.no_cpu_baseline:
+        npts = oracle_points(cfg)
+        ev_n, dt, workers, _ = oracle_sample(cfg, npts)
+        cpu = {"value": ev_n / dt, "unit": UNIT, "cores": workers, "kind": "oracle", "cpu": cpu_model(),
+               "host_cores": os.cpu_count(),
+               "sample": "%d points of %s (both halves of the batch), all %d pairs, %.1f s: oracle.collide.collide_pair per "
+                         "(point, pair) in %d forked worker processes, tables untimed" % (npts, cfg.name, cfg.ns * cfg.ns, dt, workers)}
+    evals_step = stages * nx * cfg.ns * cfg.ns * world
+    variant = {}
+    if args.nyquist_filter:
+        variant["variant"] = "nyquist_filter"
+    out = {
+        "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
+        "warmup": args.warmup, "ms_per_step": ms_per_step, "higher_is_better": True, "scaling": "weak",
+        "vs_baseline": value / world / PAPER_P100_PAIR_EVALS_PER_S if cfg.name == "c2" and args.precision == "f64" else None,
+        "vs_baseline_note": "per-GPU value / 94.6 pair-evals/s: paper Table 1 (P:316), 1 x Tesla P100, same "
+                            "(N, N_rho, M) operating point, BKW workload; context, not the target",
+        "dtype": args.precision, "data": "synthetic",
+        "config": dict(workload_desc(cfg, nx, world, stages), **variant),
+        "clocks": sampler.summary(),
+        "e2e": {"value": evals_step / (e2e_ms * 1e-3), "unit": UNIT, "ms_per_step": e2e_ms,
+                "h2d_bytes_per_step": nbytes, "d2h_bytes_per_step": nbytes,
+                "call": ("state host -> device, one step, device -> host (pinned buffers, host clock)" if is_dg else
+                         "dgfs_collide_host (C ABI, pinned host buffers in and out, host clock)")},
+        "gpu_launches": launches,
+        "roofline": roofline,
+        "cpu_baseline": cpu,
+    }
+    print(json.dumps(out))
 
 
 if __name__ == "__main__":

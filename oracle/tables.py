@@ -99,9 +99,45 @@ def C_eta(eta: float) -> float:
     return 2.0 * pi * 2.0 ** (eta + 1.0) / (eta + 1.0)
 
 
+_POOL_ARGS = None
+
+
+def _pair_tables_pooled(pq):
+    return _pair_tables(pq[0], pq[1], *_POOL_ARGS)
+
+
+def _pair_tables(p, q, mass, gam, eta, omega, alpha, kn, rho, w_rho, sigma, w_sigma, L, l, lnorm, table_mode,
+                 sigma_pre, w_pre):
+    """b^(pq)[N_rho][M][N^3], c^(pq)[N^3], beta_pq of one pair: the body of Algorithm 1's loops over x, y (and y-hat)."""
+    N_rho, M, N3 = len(rho), len(w_sigma), len(lnorm)
+    b = np.zeros((N_rho, M, N3), dtype=np.complex128)
+    c = np.zeros(N3, dtype=np.complex128)
+    mu_q = mass[q] / (mass[p] + mass[q])
+    g, e = gam[p, q], eta[p, q]
+    beta = prefactor_beta(mass[p], mass[q], omega[p, q], alpha[p, q], kn[p, q])
+    for x in range(N_rho):
+        for y in range(M):
+            if table_mode == 0:
+                b[x, y, :] = _b_exact(rho[x], g, e, mu_q, L, l, lnorm, sigma[y])
+            else:
+                # Algo 1 steps 9-13 (P:189-196): quadrature over the pre-computation sphere
+                for yh in range(len(w_pre)):
+                    Bpq = (1.0 + sigma[y] @ sigma_pre[yh]) ** e
+                    b[x, y, :] += Bpq * w_pre[yh] * rho[x] ** (g + 2.0) * np.exp(
+                        -1j * mu_q * pi / L * rho[x] * (l @ sigma_pre[yh]))
+                    # step 14 (P:197): c accumulates over x, y and y-hat (reading Q-3)
+                    c[:] += w_rho[x] * w_sigma[y] * Bpq * w_pre[yh] * rho[x] ** (g + 2.0) \
+                        * np.exp(-1j * pi / L * rho[x] * (l @ sigma_pre[yh]))
+        if table_mode == 0:
+            # O-8: both angular integrals of Eq. 17 done exactly
+            c[:] += w_rho[x] * rho[x] ** (g + 2.0) * C_eta(e) * 4.0 * pi \
+                * sinc_u(pi * rho[x] / L * lnorm)
+    return b, c, beta
+
+
 def precompute(N, N_rho, M, L, mass, omega, alpha, kn=None, R=None, sigma=None, w_sigma=None,
-               table_mode=0, sigma_pre=None, w_pre=None, beta_override=None) -> Tables:
-    """Algorithm 1."""
+               table_mode=0, sigma_pre=None, w_pre=None, beta_override=None, workers=1) -> Tables:
+    """Algorithm 1.  workers > 1: the pairs (p,q) are computed in that many forked processes."""
     mass = np.asarray(mass, dtype=np.float64)
     ns = len(mass)
     omega = np.asarray(omega, dtype=np.float64).reshape(ns, ns)
@@ -131,28 +167,20 @@ def precompute(N, N_rho, M, L, mass, omega, alpha, kn=None, R=None, sigma=None, 
         for y in range(M):                          # step 6
             a[x, y, :] = pi / L * rho[x] * (l @ sigma[y])        # step 7
 
-    for p in range(ns):
-        for q in range(ns):
-            mu_q = mass[q] / (mass[p] + mass[q])
-            g, e = gam[p, q], eta[p, q]
-            beta[p, q] = prefactor_beta(mass[p], mass[q], omega[p, q], alpha[p, q], kn[p, q])
-            for x in range(N_rho):
-                for y in range(M):
-                    if table_mode == 0:
-                        b[p, q, x, y, :] = _b_exact(rho[x], g, e, mu_q, L, l, lnorm, sigma[y])
-                    else:
-                        # Algo 1 steps 9-13: quadrature over the pre-computation sphere
-                        for yh in range(len(w_pre)):
-                            Bpq = (1.0 + sigma[y] @ sigma_pre[yh]) ** e
-                            b[p, q, x, y, :] += Bpq * w_pre[yh] * rho[x] ** (g + 2.0) * np.exp(
-                                -1j * mu_q * pi / L * rho[x] * (l @ sigma_pre[yh]))
-                            # step 14: c accumulates over x, y and y-hat (reading Q-3)
-                            c[p, q, :] += w_rho[x] * w_sigma[y] * Bpq * w_pre[yh] * rho[x] ** (g + 2.0) \
-                                * np.exp(-1j * pi / L * rho[x] * (l @ sigma_pre[yh]))
-                if table_mode == 0:
-                    # O-8: both angular integrals of Eq. 17 done exactly
-                    c[p, q, :] += w_rho[x] * rho[x] ** (g + 2.0) * C_eta(e) * 4.0 * pi \
-                        * sinc_u(pi * rho[x] / L * lnorm)
+    args = (mass, gam, eta, omega, alpha, kn, rho, w_rho, sigma, w_sigma, L, l, lnorm, table_mode, sigma_pre, w_pre)
+    pairs = [(p, q) for p in range(ns) for q in range(ns)]
+    if workers and workers > 1 and len(pairs) > 1:
+        # the pairs are independent: same statements, run in forked worker processes (no change of arithmetic)
+        import multiprocessing as mp
+        global _POOL_ARGS
+        _POOL_ARGS = args
+        with mp.get_context("fork").Pool(min(workers, len(pairs))) as pool:
+            res = pool.map(_pair_tables_pooled, pairs, chunksize=1)
+        _POOL_ARGS = None
+    else:
+        res = [_pair_tables(p, q, *args) for (p, q) in pairs]
+    for (p, q), (bpq, cpq, betapq) in zip(pairs, res):
+        b[p, q], c[p, q], beta[p, q] = bpq, cpq, betapq
     if beta_override is not None:
         beta = np.asarray(beta_override, dtype=np.float64).reshape(ns, ns).copy()
     return Tables(N, N_rho, M, L, R, mass, rho, w_rho, sigma, w_sigma, a, b, c, beta, gam, eta)

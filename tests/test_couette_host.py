@@ -1,10 +1,10 @@
-"""Host-side pieces of the Couette runner (paper_1903_04670_b200/couette.py): the diagnostics it prints are
+"""Host-side pieces of the Couette runner (workloads/couette_case.py): the diagnostics it prints are
 plain reductions; they are checked against what they must return on a Maxwellian and on polynomials.  The
 configuration itself is checked against the numbers Table 2 prints."""
 import numpy as np
 import torch
 
-from paper_1903_04670_b200.couette import gll, moments
+from workloads.couette_case import gll, moments
 from workloads import get_config, make_dg_state
 from workloads.inputs import maxwellian
 

@@ -77,7 +77,8 @@ def test_small_radial_rule_every_N(torch_cuda, N, N_rho, M, ns, alpha):
     _small_radial_rule(torch_cuda, N, N_rho, M, ns, alpha)
 
 
-@pytest.mark.parametrize("N,N_rho,M,ns", [(8, 3, 6, 2), (16, 2, 12, 2), (32, 2, 12, 2)])
+@pytest.mark.parametrize("N,N_rho,M,ns", [(8, 3, 6, 2), (16, 2, 12, 2), (32, 2, 12, 2),
+                                          (8, 2, 32, 2)])      # weighted 32-point rule: R-10 weight folding (v0_wfac)
 def test_v0_pipeline_on_vhs_pairs(torch_cuda, monkeypatch, N, N_rho, M, ns):
     """All-VHS configurations default to the v1 pipeline; DGFS_PIPELINE=v0 keeps the stage-per-kernel
     pipeline (the one VSS pairs and N = 48 use) covered on the same inputs."""

@@ -1,13 +1,15 @@
-"""Parity at the sizes of BASELINE.json's configs c1..c4: the GPU runs the batch in the launch
-configuration bench.py times (one dgfs_collide[_pairs] call over the whole batch); the oracle
-computes a seeded sample of points one by one (SURVEY.md 8(d) "parity is checked on a seeded
-subset").  Tolerance: 1e-10 relative to max|Q| per (point, pair) array."""
-import os
-
+"""Parity at the sizes of BASELINE.json's configs c1..c4, sampled as SURVEY.md 8(d) prescribes: the GPU runs the whole
+batch in the launch configuration bench.py times (one dgfs_collide[_pairs] call); the oracle computes a seeded sample
+of points one by one, every pair (c1, c2: 16 points, eight from each half of c2; c4: 4 points; c3: all 64 DOF),
+spread over the host cores by tests/oracle_pool.py (the oracle's arithmetic is untouched).  Sampled points are also
+re-run with nx = 1 and must equal the batched result bit for bit.  Tolerance: 1e-10 relative to max|Q| per
+(point, pair) array (BASELINE.json north_star).  The achieved errors go to the parity log (oracle_pool.record),
+from which profiles/r02_parity.md is written."""
 import numpy as np
 import pytest
 
 from workloads import get_config, make_points, make_dg_state
+from oracle_pool import tables_for, drop_tables, collide_pairs_pool, record
 
 pytestmark = pytest.mark.gpu
 
@@ -23,62 +25,82 @@ def torch_cuda():
     return torch
 
 
-def _oracle_pairs(cfg, f_sample):
-    from oracle.tables import precompute
-    from oracle.collide import collide_pairs
-    tab = precompute(cfg.N, cfg.N_rho, cfg.M, cfg.L, cfg.mass, cfg.omega, cfg.alpha)
-    return collide_pairs(tab, f_sample)
+def _errs(Qg, Qo):
+    """max over velocity nodes of |Qg - Qo| relative to max|Qo|, per leading index."""
+    return np.max(np.abs(Qg - Qo), axis=-1) / np.max(np.abs(Qo), axis=-1)
 
 
-def _check(Qg, Qo, what):
-    num = np.max(np.abs(Qg - Qo), axis=-1)
-    den = np.max(np.abs(Qo), axis=-1)
-    err = num / den
-    print("%s: max rel err %.3e over %d (point, pair) arrays" % (what, err.max(), err.size))
+def _check_pairs(cfg, Qg, Qo, label, groups=None):
+    """Qg, Qo: [npts][ns][ns][N^3].  Records the worst error per pair (and per group of points) and asserts."""
+    err = _errs(Qg, Qo)
+    groups = groups or {"all": range(err.shape[0])}
+    for gname, idx in groups.items():
+        idx = list(idx)
+        for p in range(cfg.ns):
+            for q in range(cfg.ns):
+                record(cfg.name, "%s, %s points, pair (%d,%d)" % (label, gname, p, q), err[idx, p, q].max(), TOL,
+                       points=len(idx))
     assert err.max() < TOL, err
 
 
-def _run_batch(torch, cfg, xs_all, sample, pairs=True):
+def test_c1_full_batch_16_points_all_pairs(torch_cuda):
+    torch = torch_cuda
     from paper_1903_04670_b200 import Dgfs
-    f = make_points(cfg, xs_all)
-    pos = [list(xs_all).index(x) for x in sample]
+    cfg = get_config("c1")
+    sample = [0, 1, 63, 64, 127, 255, 256, 300, 511, 512, 600, 767, 768, 900, 1022, 1023]
+    f = make_points(cfg, range(cfg.nx))
     with Dgfs.from_config(cfg, device=0) as op:
         fd = torch.from_numpy(f).cuda()
-        Q = op.collide_pairs(fd) if pairs else op.collide(fd)
-        torch.cuda.synchronize()
-        Qs = Q[pos].cpu().numpy()
+        Q = op.collide_pairs(fd)
+        Qg = Q[sample].cpu().numpy()
+        for x in sample[::5]:                                   # batch == per-point call, bit for bit
+            assert torch.equal(op.collide_pairs(fd[x:x + 1].contiguous())[0], Q[x])
         del Q, fd
     torch.cuda.empty_cache()
-    return f[pos], Qs
+    _check_pairs(cfg, Qg, collide_pairs_pool(tables_for(cfg), f[sample]), "full batch of 1024")
+    drop_tables(cfg)
 
 
-def test_c1_full_batch_sampled_points(torch_cuda):
-    cfg = get_config("c1")
-    sample = [0, 1, 511, 1023]
-    fs, Qg = _run_batch(torch_cuda, cfg, range(cfg.nx), sample)
-    _check(Qg, _oracle_pairs(cfg, fs), "c1")
-
-
-def test_c2_full_batch_sampled_points_both_halves(torch_cuda):
-    """Headline config, all 4096 points in one call; sample covers the near-equilibrium half
-    (x < 2048, Q is a small difference of large terms) and the non-equilibrium half."""
+def test_c2_full_batch_16_points_both_halves_all_pairs(torch_cuda):
+    """Headline config: all 4096 points in one dgfs_collide call (what bench.py times) and in one dgfs_collide_pairs
+    call.  Eight sampled points from the near-equilibrium half (x < 2048: Q is a difference of gain and loss terms
+    ~1e3 larger, reading T-1) and eight from the non-equilibrium half."""
+    torch = torch_cuda
+    from paper_1903_04670_b200 import Dgfs
     cfg = get_config("c2")
-    sample = [0, 2047, 2048, 4095]
-    fs, Qg = _run_batch(torch_cuda, cfg, range(cfg.nx), sample, pairs=False)
-    Qo = _oracle_pairs(cfg, fs).sum(axis=2)
-    _check(Qg, Qo, "c2 (summed over q)")
+    near = [0, 1, 255, 777, 1024, 1500, 2046, 2047]
+    far = [2048, 2049, 2500, 3000, 3333, 3800, 4094, 4095]
+    sample = near + far
+    f = make_points(cfg, range(cfg.nx))
+    with Dgfs.from_config(cfg, device=0) as op:
+        fd = torch.from_numpy(f).cuda()
+        Qs = op.collide(fd)
+        Qsum_g = Qs[sample].cpu().numpy()
+        for x in (0, 2047, 2048, 4095):                          # batch == per-point call, bit for bit
+            assert torch.equal(op.collide(fd[x:x + 1].contiguous())[0], Qs[x])
+        del Qs
+        Q = op.collide_pairs(fd)
+        Qg = Q[sample].cpu().numpy()
+        for x in (1, 3000):
+            assert torch.equal(op.collide_pairs(fd[x:x + 1].contiguous())[0], Q[x])
+        del Q, fd
+    torch.cuda.empty_cache()
+    Qo = collide_pairs_pool(tables_for(cfg), f[sample])
+    drop_tables(cfg)
+    groups = {"near-equilibrium": range(0, 8), "non-equilibrium": range(8, 16)}
+    # ratio of the gain / loss magnitude to the result on the near-equilibrium half: how much cancellation the
+    # 1e-10 has to survive (reading T-1)
+    _check_pairs(cfg, Qg, Qo, "full batch of 4096, dgfs_collide_pairs", groups)
+    es = _errs(Qsum_g, Qo.sum(axis=2))
+    for gname, idx in groups.items():
+        for p in range(cfg.ns):
+            record(cfg.name, "full batch of 4096, dgfs_collide (summed over q), %s points, species %d" % (gname, p),
+                   es[list(idx), p].max(), TOL, points=8)
+    assert es.max() < TOL, es
 
 
-def test_c2_pairs_output_reduced_batch(torch_cuda):
-    cfg = get_config("c2")
-    xs = [5, 1000, 2047, 2048, 3000, 4095, 17]
-    sample = [1000, 3000]
-    fs, Qg = _run_batch(torch_cuda, cfg, xs, sample)
-    _check(Qg, _oracle_pairs(cfg, fs), "c2 pairs")
-
-
-def test_c3_collision_term_of_dg_state(torch_cuda):
-    """c3's collide call: 3 species, 8 of 9 pairs VSS (full b tables), 64 spatial DOF."""
+def test_c3_collision_term_all_dof_all_pairs(torch_cuda):
+    """c3's collide call: 3 species, 8 of 9 pairs VSS (full b tables), all 64 spatial DOF against the oracle."""
     torch = torch_cuda
     from paper_1903_04670_b200 import Dgfs
     cfg = get_config("c3")
@@ -87,25 +109,31 @@ def test_c3_collision_term_of_dg_state(torch_cuda):
     # perturb node values so that the DOF of one element differ
     rng = np.random.default_rng(cfg.seed)
     f = f * (1.0 + 0.02 * rng.uniform(-1, 1, (f.shape[0], f.shape[1], 1)))
-    pos = [0, 37]
     with Dgfs.from_config(cfg, device=0) as op:
-        Q = op.collide_pairs(torch.from_numpy(f).cuda())
-        Qg = Q[pos].cpu().numpy()
-    _check(Qg, _oracle_pairs(cfg, f[pos]), "c3 collide")
+        Qg = op.collide_pairs(torch.from_numpy(f).cuda()).cpu().numpy()
+    _check_pairs(cfg, Qg, collide_pairs_pool(tables_for(cfg), f), "64 DOF")
 
 
 @pytest.mark.slow
-def test_c4_stress_reduced_batch(torch_cuda):
-    """N=48, N_rho=48, M=32 (tables and arrays beyond shared memory).  The batch is cut to 24 of
-    the config's 2048 points (the full batch is ~0.4 PFLOP); one point goes through the oracle."""
+def test_c4_full_batch_4_points_all_pairs(torch_cuda):
+    """N = 48, N_rho = 48, M = 32 (tables and arrays beyond shared memory): the whole 2048-point batch in one
+    dgfs_collide_pairs call; four sampled points, all four pairs (the same-species pairs exercise the weight
+    folding of the 32-point rule, R-10) through the oracle."""
+    torch = torch_cuda
+    from paper_1903_04670_b200 import Dgfs
     cfg = get_config("c4")
-    xs = list(range(0, 2048, 89))[:24]
-    xs[-1] = 2047
-    sample = [xs[7]]
-    fs, Qg = _run_batch(torch_cuda, cfg, xs, sample)
-    from oracle.tables import precompute
-    from oracle.collide import collide_pair
-    tab = precompute(cfg.N, cfg.N_rho, cfg.M, cfg.L, cfg.mass, cfg.omega, cfg.alpha)
-    for (p, q) in ((0, 1), (1, 0)):          # ~1 min of oracle time per pair
-        Qo = collide_pair(tab, p, q, fs[0, p], fs[0, q])
-        _check(Qg[0, p, q][None], Qo[None], "c4 pair (%d,%d)" % (p, q))
+    sample = [0, 777, 1501, 2047]
+    f = make_points(cfg, range(cfg.nx))
+    with Dgfs.from_config(cfg, device=0) as op:
+        fd = torch.from_numpy(f).cuda()
+        Q = op.collide_pairs(fd)
+        torch.cuda.synchronize()
+        Qg = Q[sample].cpu().numpy()
+        assert torch.equal(op.collide_pairs(fd[777:778].contiguous())[0], Q[777])
+        del Q, fd
+    torch.cuda.empty_cache()
+    fs = f[sample].copy()
+    del f
+    Qo = collide_pairs_pool(tables_for(cfg), fs)
+    drop_tables(cfg)
+    _check_pairs(cfg, Qg, Qo, "full batch of 2048")

@@ -195,3 +195,24 @@ def test_table_mode1_converges_to_exact_angles():
     # eta = 0.3: (1 + sigma.u)^eta is not smooth at the antipode, algebraic convergence only
     # (measured 3.8e-3 -> 1.3e-3) -- the reason table_mode 0 is the default (reading P-1)
     assert vss[1] < vss[0] < 1e-2
+
+
+def test_precompute_in_worker_processes_is_bit_identical():
+    """precompute(workers=n) runs the same statements per pair in forked processes: identical tables."""
+    kw = dict(N=6, N_rho=3, M=6, L=5.0, mass=(1.0, 2.0, 1.5), omega=[[0.7, 0.75, 0.8]] * 3, alpha=[[1.0, 1.2, 1.4]] * 3)
+    t1 = precompute(**kw)
+    t2 = precompute(workers=3, **kw)
+    for name in ("a", "b", "c", "beta"):
+        assert np.array_equal(getattr(t1, name), getattr(t2, name)), name
+
+
+def test_pooled_oracle_equals_serial_oracle():
+    """tests/oracle_pool.py only distributes oracle.collide.collide_pair calls: same numbers as collide_pairs."""
+    import os, sys
+    sys.path.insert(0, os.path.dirname(os.path.abspath(__file__)))
+    from oracle.collide import collide_pairs
+    from oracle_pool import collide_pairs_pool
+    tab = precompute(N=6, N_rho=2, M=6, L=5.0, mass=(1.0, 2.0), omega=[[0.6, 0.7]] * 2, alpha=[[1.0, 1.3]] * 2)
+    rng = np.random.default_rng(5)
+    f = rng.uniform(0.1, 1.0, (3, 2, 216))
+    assert np.array_equal(collide_pairs_pool(tab, f), collide_pairs(tab, f))

@@ -1,11 +1,12 @@
 """Second workload: the paper's Couette case C-01 (Table 2) run to
 its steady state through `dgfs_step_euler`, on one GPU.
 
-    python -m paper_1903_04670_b200.couette [--dt 1e-3] [--block 250] [--tol 2e-4] [--max-steps 40000]
+    python -m workloads.couette_case [--dt 1e-3] [--block 250] [--tol 2e-4] [--max-steps 40000]
 
-Every step of the path (wall balance, collisions of all four VSS pairs, transport, Euler update) runs in the
-library's kernels; this script only marshals, and every `--block` steps reads bulk moments of the state (plain
-torch reductions: diagnostics, not part of the timed path) to decide when the flow has stopped changing.
+It lives beside the workload definitions, not in the product package: every step of the path (wall balance,
+collisions of all four VSS pairs, transport, Euler update) runs in the library's kernels through `dgfs_step_euler`;
+this script only drives it, and every `--block` steps reads bulk moments of the state (plain torch reductions:
+diagnostics of a workload, not part of the method or of the timed path) to decide when the flow has stopped changing.
 Prints ONE JSON line: steps and device time to the steady state, time per step, the moment profiles and the
 self-consistency checks the paper's text allows (the DSMC curves of its Fig. 2 are images that are not in the
 container): per-species mass balance (drift = mass defect of the collision term), antisymmetry of u_y about the centre plane, velocity slip at the
@@ -59,7 +60,7 @@ def main():
 
     import torch
     from workloads import get_config, make_dg_state
-    from . import Dgfs, Mesh1D, api
+    from paper_1903_04670_b200 import Dgfs, Mesh1D, api
 
     if not torch.cuda.is_available():
         raise SystemExit("couette: needs a CUDA device (there is no CPU path)")
