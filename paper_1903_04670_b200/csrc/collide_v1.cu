@@ -284,6 +284,33 @@ __device__ __forceinline__ void cp_async_wait_all() { asm volatile("cp.async.wai
 template <int PENDING>
 __device__ __forceinline__ void cp_async_wait_pending() { asm volatile("cp.async.wait_group %0;\n" ::"n"(PENDING) : "memory"); }
 
+// Bulk asynchronous copy global -> shared by the TMA unit (cp.async.bulk; SASS UBLKCP): ONE thread issues a copy of
+// a contiguous run (16-byte aligned, a multiple of 16 bytes) and the bytes are counted on an mbarrier in shared
+// memory; the consumers wait on the barrier's phase parity.  No per-thread address arithmetic, no registers in flight.
+__device__ __forceinline__ unsigned smem_u32(const void* p) { return (unsigned)__cvta_generic_to_shared(p); }
+__device__ __forceinline__ void mbar_init(unsigned long long* bar, unsigned count) {
+  asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;\n" ::"r"(smem_u32(bar)), "r"(count));
+}
+__device__ __forceinline__ void mbar_expect_tx(unsigned long long* bar, unsigned bytes) {
+  asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;\n" ::"r"(smem_u32(bar)), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void mbar_wait(unsigned long long* bar, unsigned parity) {
+  asm volatile(
+      "{\n"
+      ".reg .pred p;\n"
+      "WAIT_%=:\n"
+      "mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n"
+      "@p bra DONE_%=;\n"
+      "bra WAIT_%=;\n"
+      "DONE_%=:\n"
+      "}\n" ::"r"(smem_u32(bar)), "r"(parity) : "memory");
+}
+__device__ __forceinline__ void tma_bulk_g2s(void* smem, const void* gmem, unsigned bytes, unsigned long long* bar) {
+  asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];\n" ::"r"(smem_u32(smem)),
+               "l"(gmem), "r"(bytes), "r"(smem_u32(bar)) : "memory");
+}
+__device__ __forceinline__ void fence_mbar_init() { asm volatile("fence.mbarrier_init.release.cluster;\n" ::: "memory"); }
+
 // Inverse z pass of h_z f^ for the z jobs k0 .. k0 + nk - 1 of point blockIdx.z that shift species blockIdx.y;
 // thread per (lx, m) pencil.  The block's 128 pencils of the half-packed spectrum are read ONCE into shared memory
 // (every job of a species starts from the same spectrum: 8 jobs per species and radial node at c2) and each job
@@ -564,7 +591,7 @@ __global__ void __launch_bounds__(32 * NW) k_nyq2(V1Tables t, DevTables tab, con
       cplx* out = nyq + ((size_t)item * tab.M + s) * NL::STRIDE;
       if (which == 0) {
 #pragma unroll
-        for (int j = 0; j < N; ++j) out[NL::UZ + j * N + ln] = X[j];
+        for (int j = 0; j < N; ++j) out[NL::UZ + (j * 2 + (ln & 1)) * H + (ln >> 1)] = X[j];
       } else if (which == 1) {
         const double sb = (ln & 1) ? -1.0 : 1.0;
 #pragma unroll
@@ -574,7 +601,7 @@ __global__ void __launch_bounds__(32 * NW) k_nyq2(V1Tables t, DevTables tab, con
         }
       } else {
 #pragma unroll
-        for (int j = 0; j < N; ++j) out[NL::UY + j * N + ln] = X[j];
+        for (int j = 0; j < N; ++j) out[NL::UY + j * N + (ln ^ uy_swz(j))] = X[j];
       }
     }
     s = sn; scale = scale_next;
@@ -740,9 +767,9 @@ __global__ void __launch_bounds__(32 * W) k_xy_full(V1Tables t, DevTables tab, G
       cp_async16(&buf[JS::VXP + ln], nq + NL::VXP + ln);
       if (ln == 0) cp_async16(&buf[JS::VZP], nq + NL::VZP + cz);
 #pragma unroll
-      for (int j = 0; j < N; ++j) cp_async16(&buf[FS::UZ + j * N + ln], nq + NL::UZ + j * N + ln);
+      for (int j = 0; j < N; ++j) cp_async16(&buf[FS::UZ + j * N + ln], nq + NL::UZ + (j * 2 + (ln & 1)) * H + (ln >> 1));
       cp_async16(&buf[FS::UX + ln], nq + NL::UXP + ln * N + cz);
-      cp_async16(&buf[FS::UY + ln], nq + NL::UY + ln * N + cz);
+      cp_async16(&buf[FS::UY + ln], nq + NL::UY + ln * N + (cz ^ uy_swz(ln)));
     }
     cp_async_commit();
   };
@@ -866,141 +893,136 @@ __global__ void __launch_bounds__(256) k_zfwd_full(DevTables tab, V1Tables t, co
 }
 
 // S(c) = -sum_s Re W_s(c) Im W_s(c),  W_s(c) = (-1)^cx ux'_s(cy,cz) + (-1)^cy uy_s(cx,cz) + (-1)^cz uz_s(cx,cy)
-// (W = a_i + i b_i, file header).  This kernel is bound by the L2 -> SM traffic of its tables (150 KB per
-// (item, s) if every byte is fetched once, for 5 FP64 instructions per node).  A block of 256 threads covers 8 cz
-// planes and fetches the uz plane once; two blocks per SM (four-stage ring, 99 KB each at N = 32) overlap one
-// block's pipeline fill and its store of S with the other's arithmetic, which is worth more than the halved uz
-// traffic of 16-plane blocks that fill the SM alone (measured: 102 against 107 ms per step of c2).  Thread = 2 x 2 tile of (cx, cy): every table element
-// serves several nodes and all signs are compile-time constants.  The tables of one s (uz plane, rows of
-// ux' and uy) are staged in shared memory by cp.async, a ring of four stages over s; uz and uy are stored
-// de-interleaved by the parity of cx so that the pair loads are conflict-free.
+// (W = a_i + i b_i, file header).  Five FP64 instructions per node and sphere point against three tables of N^2
+// complex values each: the kernel is bound by how its tables reach the SM, not by arithmetic.  A block of 256 threads
+// covers a slab of 8 cy rows of one item, all (cx, cz): in the layouts k_nyq2 writes (first index = the transform's
+// register index, second = its lane) the slab's rows of ux'[cy][cz] and uz[cy][cx] and the whole plane uy[cx][cz] are
+// three CONTIGUOUS runs, so one thread stages the tables of a sphere point with three bulk copies of the TMA unit
+// (cp.async.bulk, completion counted on an mbarrier; a ring of four stages over s).  Round 1 staged them with
+// 16-byte cp.async and its per-element address arithmetic took 60 % of the kernel's issue slots (profiles/r02_wterm.md).
+// Thread = 2 x 2 tile of (cx, cz) over the slab's 8 rows: every table element serves several nodes and all signs are
+// compile-time constants.  Bank conflicts: uz is stored de-interleaved by the parity of cx, uy with its cz index
+// XOR-swizzled by (cx / 2) mod 8 (v1_tables.h), so that the 8 lanes of a 128-bit wavefront read 8 different banks.
 template <int N>
 struct WtermSmem {
-  static constexpr int CZG = 8, NH = 1, CZB = CZG * NH, THREADS = 256 * NH;
-  static constexpr int RS = N + 1;                  // row stride of V and U: consecutive planes land in different banks
-  static constexpr int Z = 0;                       // [cy][parity][H]
-  static constexpr int V = N * N;                   // [i][parity][H], rows padded to RS
-  static constexpr int U = N * N + CZB * RS;        // [i][cy], rows padded to RS
-  static constexpr int WORDS = N * N + 2 * CZB * RS;
-  static constexpr int COPIES = N * N + 2 * CZB * N;   // elements staged per s
-  static constexpr int STAGES = 4;                     // ring depth (two blocks per SM: 8 stages in flight per SM)
+  static constexpr int CYB = 8, THREADS = 256;
+  static constexpr int Y = 0;                       // [cx][cz ^ swz(cx)]      the uy plane
+  static constexpr int Z = N * N;                   // [i][parity][H]          uz rows of the slab
+  static constexpr int U = N * N + CYB * N;         // [i][cz]                 ux' rows of the slab
+  static constexpr int WORDS = N * N + 2 * CYB * N;
+  static constexpr int STAGES = 4;                  // ring depth (two blocks per SM: 8 stages in flight per SM)
 };
-// Arithmetic of one s for the thread's 2 x 2 x 8 nodes.  MASK bit d set: the field of axis d (ux', uy, uz) is
-// identically zero for this sphere point (V1Tables::smask) and is neither staged nor read.
+
+// Arithmetic of one s for the thread's 2 x 2 x 8 nodes (cx = 2 tx + a, cz = 2 tz + b, cy = cy0 + i).  MASK bit d set:
+// the field of axis d (ux', uy, uz) is identically zero for this sphere point (V1Tables::smask), neither staged nor read.
 template <int N, int MASK>
-__device__ __forceinline__ void wterm_planes(const cplx* __restrict__ b_, int half, int tx, int ty, double (&acc)[8][2][2]) {
+__device__ __forceinline__ void wterm_rows(const cplx* __restrict__ b_, int tx, int tz, double (&acc)[8][2][2]) {
   typedef WtermSmem<N> WS;
-  constexpr int H = N / 2, CZG = WS::CZG;
+  constexpr int H = N / 2, CYB = WS::CYB;
   constexpr bool HU = !(MASK & 1), HV = !(MASK & 2), HZ = !(MASK & 4);
   const cplx zero = make_double2(0.0, 0.0);
-  cplx z[2][2];
+  cplx y[2][2];                                     // uy(cx = 2 tx + a, cz = 2 tz + b)
 #pragma unroll
   for (int b = 0; b < 2; ++b)
 #pragma unroll
-    for (int a = 0; a < 2; ++a) z[b][a] = HZ ? b_[WS::Z + ((2 * ty + b) * 2 + a) * H + tx] : zero;
-  // software pipeline over the planes: the loads of plane i + 1 are in flight during the arithmetic of plane i
-  const cplx* ub = b_ + WS::U + (half * CZG) * WS::RS + 2 * ty;
-  const cplx* vb = b_ + WS::V + (half * CZG) * WS::RS + tx;
-  cplx un[2] = {HU ? ub[0] : zero, HU ? ub[1] : zero}, vn[2] = {HV ? vb[0] : zero, HV ? vb[H] : zero};
+    for (int a = 0; a < 2; ++a) y[b][a] = HV ? b_[WS::Y + (2 * tx + a) * N + ((2 * tz + b) ^ uy_swz(2 * tx + a))] : zero;
+  // software pipeline over the rows: the loads of row i + 1 are in flight during the arithmetic of row i
+  const cplx* ub = b_ + WS::U + 2 * tz;             // ux'(cy0 + i, cz = 2 tz + b): the same for all lanes of a tz
+  const cplx* zb = b_ + WS::Z + tx;                 // uz(cy0 + i, cx = 2 tx + a) at [i][a][tx]
+  cplx un[2] = {HU ? ub[0] : zero, HU ? ub[1] : zero}, zn[2] = {HZ ? zb[0] : zero, HZ ? zb[H] : zero};
 #pragma unroll
-  for (int i = 0; i < CZG; ++i) {
-    const cplx u[2] = {un[0], un[1]}, v[2] = {vn[0], vn[1]};
-    if (i + 1 < CZG) {
-      if (HU) { un[0] = ub[(i + 1) * WS::RS]; un[1] = ub[(i + 1) * WS::RS + 1]; }
-      if (HV) { vn[0] = vb[(i + 1) * WS::RS]; vn[1] = vb[(i + 1) * WS::RS + H]; }
+  for (int i = 0; i < CYB; ++i) {
+    const cplx u[2] = {un[0], un[1]}, z[2] = {zn[0], zn[1]};
+    if (i + 1 < CYB) {
+      if (HU) { un[0] = ub[(i + 1) * N]; un[1] = ub[(i + 1) * N + 1]; }
+      if (HZ) { zn[0] = zb[(i + 1) * N]; zn[1] = zb[(i + 1) * N + H]; }
     }
 #pragma unroll
     for (int b = 0; b < 2; ++b)
 #pragma unroll
       for (int a = 0; a < 2; ++a) {
-        // signs: the tile starts at even cx, cy; plane groups start at even cz
+        // signs: the tile starts at even cx, cz; slabs start at even cy
         double wx = 0.0, wy = 0.0;
         if (HU) { wx = a ? -u[b].x : u[b].x; wy = a ? -u[b].y : u[b].y; }
-        if (HV) { wx += b ? -v[a].x : v[a].x; wy += b ? -v[a].y : v[a].y; }
-        if (HZ) { wx += (i & 1) ? -z[b][a].x : z[b][a].x; wy += (i & 1) ? -z[b][a].y : z[b][a].y; }
+        if (HV) { wx += (i & 1) ? -y[b][a].x : y[b][a].x; wy += (i & 1) ? -y[b][a].y : y[b][a].y; }
+        if (HZ) { wx += b ? -z[a].x : z[a].x; wy += b ? -z[a].y : z[a].y; }
         acc[i][b][a] = fma(wx, wy, acc[i][b][a]);
       }
   }
 }
 
 template <int N>
-__global__ void __launch_bounds__(WtermSmem<N>::THREADS, 2 / WtermSmem<N>::NH) k_wterm(const cplx* __restrict__ nyq, int M, double* __restrict__ S, const unsigned char* __restrict__ full, int npairs,
+__global__ void __launch_bounds__(WtermSmem<N>::THREADS, 2) k_wterm(const cplx* __restrict__ nyq, int M, double* __restrict__ S, const unsigned char* __restrict__ full, int npairs,
         const unsigned char* __restrict__ smask, const unsigned char* __restrict__ sskip, const int* __restrict__ tsrc) {
-  constexpr int H = N / 2, N2 = N * N, N3 = N2 * N;
+  constexpr int N2 = N * N, N3 = N2 * N, H = N / 2;
   typedef NyqLayout<N> NL;
   typedef WtermSmem<N> WS;
-  constexpr int CZG = WS::CZG, CZB = WS::CZB, NT = WS::THREADS, NS = WS::STAGES;
+  constexpr int CYB = WS::CYB, NT = WS::THREADS, NS = WS::STAGES;
   extern __shared__ cplx sm[];
   // pairs with a full b table take k_xy_full, transposed pairs reuse the other's S_r (uniform per block)
   if (full[blockIdx.y % npairs] || tsrc[blockIdx.y % npairs] != (int)(blockIdx.y % npairs)) return;
-  const int half = threadIdx.x / 256, tt = threadIdx.x % 256;
-  const int tx = tt % 16, ty = tt / 16;
-  const bool act = tx < H && ty < H;
-  const int cz0 = blockIdx.x * CZB;
+  const int tx = threadIdx.x % 16, tz = threadIdx.x / 16;
+  const bool act = tx < H && tz < H;
+  const int cy0 = blockIdx.x * CYB;
   const cplx* nbase = nyq + (size_t)blockIdx.y * M * NL::STRIDE;
   const unsigned char* skip = sskip + (size_t)(blockIdx.y % npairs) * M;
   // which fields each sphere point has (7: none, or the point is not run for this pair, R-10), once per block in
   // shared memory: the loop below then never waits for a global load before it can issue or branch
   __shared__ unsigned char mk_s[256];
+  __shared__ unsigned long long bar[NS];             // one "stage is full" barrier per ring slot
   for (int i = threadIdx.x; i < M && i < 256; i += NT) mk_s[i] = skip[i] ? 7 : smask[i];
+  if (threadIdx.x == 0) {
+    for (int k = 0; k < NS; ++k) mbar_init(&bar[k], 1);
+    fence_mbar_init();
+  }
   __syncthreads();
   auto mk = [&](int s) -> int { return s < 256 ? (int)mk_s[s] : (skip[s] ? 7 : (int)smask[s]); };
   auto next_a = [&](int s) { while (s < M && mk(s) == 7) ++s; return s; };      // next point with something to add
+  // the tables of sphere point s into ring slot `slot` (thread 0): three contiguous runs; vanishing fields are not staged
   auto issue = [&](int s, int slot) {
     cplx* dst = sm + (size_t)slot * WS::WORDS;
     const cplx* nq = nbase + (size_t)s * NL::STRIDE;
-    const int mask = mk(s);                          // vanishing fields are not staged
-    for (int e = threadIdx.x; e < WS::COPIES; e += NT) {
-      if (e < N2) {
-        const int cy = e / N, cx = e % N;
-        if (!(mask & 4)) cp_async16(&dst[WS::Z + (cy * 2 + (cx & 1)) * H + (cx >> 1)], nq + NL::UZ + e);
-      } else if (e < N2 + CZB * N) {
-        const int cx = (e - N2) / CZB, i = (e - N2) % CZB;
-        if (!(mask & 2)) cp_async16(&dst[WS::V + i * WS::RS + (cx & 1) * H + (cx >> 1)], nq + NL::UY + cx * N + cz0 + i);
-      } else {
-        const int cy = (e - N2 - CZB * N) / CZB, i = (e - N2 - CZB * N) % CZB;
-        if (!(mask & 1)) cp_async16(&dst[WS::U + i * WS::RS + cy], nq + NL::UXP + cy * N + cz0 + i);
-      }
-    }
-    cp_async_commit();
+    const int mask = mk(s);
+    const unsigned bu = (mask & 1) ? 0u : (unsigned)(CYB * N * sizeof(cplx));
+    const unsigned by = (mask & 2) ? 0u : (unsigned)(N2 * sizeof(cplx));
+    const unsigned bz = (mask & 4) ? 0u : (unsigned)(CYB * N * sizeof(cplx));
+    mbar_expect_tx(&bar[slot], bu + by + bz);
+    if (by) tma_bulk_g2s(dst + WS::Y, nq + NL::UY, by, &bar[slot]);
+    if (bz) tma_bulk_g2s(dst + WS::Z, nq + NL::UZ + (size_t)cy0 * N, bz, &bar[slot]);
+    if (bu) tma_bulk_g2s(dst + WS::U, nq + NL::UXP + (size_t)cy0 * N, bu, &bar[slot]);
   };
-  double acc[CZG][2][2];                      // [cz][cy][cx]
+  double acc[CYB][2][2];                      // [cy][cz][cx]
 #pragma unroll
-  for (int i = 0; i < CZG; ++i) acc[i][0][0] = acc[i][0][1] = acc[i][1][0] = acc[i][1][1] = 0.0;
-  // ring of NS stages over the points that are run: job j uses stage j % NS; groups 0 .. j + NS - 2 are committed
-  // when job j waits for group j (empty groups keep the count uniform at the end)
+  for (int i = 0; i < CYB; ++i) acc[i][0][0] = acc[i][0][1] = acc[i][1][0] = acc[i][1][1] = 0.0;
+  // ring of NS slots over the points that are run: job j uses slot j % NS; thread 0 keeps NS - 1 jobs in flight
   int s_issue = next_a(0), j_issue = 0;
-#pragma unroll
-  for (int k = 0; k < NS - 1; ++k) {
-    if (s_issue < M) { issue(s_issue, j_issue % NS); s_issue = next_a(s_issue + 1); } else cp_async_commit();
-    ++j_issue;
+  if (threadIdx.x == 0) {
+    for (int k = 0; k < NS - 1 && s_issue < M; ++k) { issue(s_issue, j_issue % NS); s_issue = next_a(s_issue + 1); ++j_issue; }
   }
   for (int s = next_a(0), j = 0; s < M; s = next_a(s + 1), ++j) {
-    cp_async_wait_pending<NS - 2>();
-    __syncthreads();
-    if (s_issue < M) { issue(s_issue, j_issue % NS); s_issue = next_a(s_issue + 1); } else cp_async_commit();
-    ++j_issue;
+    mbar_wait(&bar[j % NS], (unsigned)((j / NS) & 1));       // the bulk copies of job j have landed
+    __syncthreads();                                          // everyone is done with job j - 1: its slot is free
+    if (threadIdx.x == 0 && s_issue < M) { issue(s_issue, j_issue % NS); s_issue = next_a(s_issue + 1); ++j_issue; }
     if (!act) continue;
     const cplx* b_ = sm + (size_t)(j % NS) * WS::WORDS;
     switch (mk(s)) {                                 // uniform over the block
-      case 0: wterm_planes<N, 0>(b_, half, tx, ty, acc); break;
-      case 1: wterm_planes<N, 1>(b_, half, tx, ty, acc); break;
-      case 2: wterm_planes<N, 2>(b_, half, tx, ty, acc); break;
-      case 3: wterm_planes<N, 3>(b_, half, tx, ty, acc); break;
-      case 4: wterm_planes<N, 4>(b_, half, tx, ty, acc); break;
-      case 5: wterm_planes<N, 5>(b_, half, tx, ty, acc); break;
-      case 6: wterm_planes<N, 6>(b_, half, tx, ty, acc); break;
+      case 0: wterm_rows<N, 0>(b_, tx, tz, acc); break;
+      case 1: wterm_rows<N, 1>(b_, tx, tz, acc); break;
+      case 2: wterm_rows<N, 2>(b_, tx, tz, acc); break;
+      case 3: wterm_rows<N, 3>(b_, tx, tz, acc); break;
+      case 4: wterm_rows<N, 4>(b_, tx, tz, acc); break;
+      case 5: wterm_rows<N, 5>(b_, tx, tz, acc); break;
+      case 6: wterm_rows<N, 6>(b_, tx, tz, acc); break;
       default: break;
     }
   }
   if (!act) return;
-  double* o = S + (size_t)blockIdx.y * N3 + (size_t)(cz0 + half * CZG) * N2 + (2 * ty) * N + 2 * tx;
+  double* o = S + (size_t)blockIdx.y * N3 + (size_t)(2 * tz) * N2 + (size_t)cy0 * N + 2 * tx;
 #pragma unroll
-  for (int i = 0; i < CZG; ++i)
+  for (int i = 0; i < CYB; ++i)
 #pragma unroll
-    for (int b = 0; b < 2; ++b) {
-      *reinterpret_cast<double2*>(o + (size_t)i * N2 + b * N) = make_double2(-acc[i][b][0], -acc[i][b][1]);
-    }
+    for (int b = 0; b < 2; ++b)
+      *reinterpret_cast<double2*>(o + (size_t)b * N2 + i * N) = make_double2(-acc[i][b][0], -acc[i][b][1]);
 }
 
 // Forward z pass and steps 7-8 for a group of nr radial nodes r0 .. r0+nr-1:
@@ -1376,7 +1398,7 @@ static int collide_v1_impl(dgfs_ctx* c, const double* f, double* out, int nx, bo
         k_nyq2<N, 2><<<dim3(3, items), 64, smem_nyq, sa>>>(c->v1, c->tab, fhh, nyqy, nyqb[b], r); }
       if (nvhs > 0)
         { ProfScope ps(c->prof, sa, "k_wterm", nb * run_vhs * fl.wterm);
-          k_wterm<N><<<dim3(N / WtermSmem<N>::CZB, items), WtermSmem<N>::THREADS, smem_wt, sa>>>(nyqb[b], c->M, Sb[b], c->tab.full, np, c->v1.smask, c->v1.sskip, c->v1.tsrc); }
+          k_wterm<N><<<dim3(N / WtermSmem<N>::CYB, items), WtermSmem<N>::THREADS, smem_wt, sa>>>(nyqb[b], c->M, Sb[b], c->tab.full, np, c->v1.smask, c->v1.sskip, c->v1.tsrc); }
       }
       record(c->ev_prep[b], sa);
       // ---- plane jobs of radial node r (caller's stream)

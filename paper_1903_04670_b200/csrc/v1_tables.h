@@ -32,6 +32,9 @@ struct V1Tables {
                              //      the Nyquist field of that axis (ux', uy, uz for d = x, y, z) vanishes identically
 };
 
+// swizzle of the cz index of uy within its row (NyqLayout::UY)
+__host__ __device__ __forceinline__ int uy_swz(int cx) { return (cx >> 1) & 7; }
+
 // per (item, s) block of Nyquist-plane fields written by k_nyq, in units of cplx
 template <int N>
 struct NyqLayout {
@@ -40,8 +43,8 @@ struct NyqLayout {
   static constexpr int VZP = 2 * N;        // [N]     packed, (H,H) element correction per cz
   static constexpr int VT = 3 * N;         // [1]     packed, s_x s_y s_z f^(H,H,H)
   static constexpr int UXP = 4 * N;        // [cy][cz]
-  static constexpr int UY = 4 * N + N * N; // [cx][cz]
-  static constexpr int UZ = 4 * N + 2 * N * N;   // [cy][cx]
+  static constexpr int UY = 4 * N + N * N; // [cx][cz ^ ((cx / 2) mod 8)]: cz XOR-swizzled within its row (uy_swz), conflict-free plane reads in k_wterm
+  static constexpr int UZ = 4 * N + 2 * N * N;   // [cy][cx & 1][cx / 2]: de-interleaved by the parity of cx, the shared-memory image k_wterm reads
   static constexpr int STRIDE = 4 * N + 3 * N * N;
 };
 
