@@ -69,6 +69,13 @@ typedef struct dgfs_params {
                               c_d' of (-1)^{c_d'} f.  A different discrete operator:
                               every shifted field is then exactly real, so the Nyquist-field kernels of
                               the N <= 32 pipeline are not run.                                    */
+  int precision;           /* 0 (default): every step in fp64 (tolerance 1e-10 of max|Q| against the oracle).
+                              1: the shifted fields, their transforms in x and y, the product and the sum over
+                              sphere points (steps 4-6 of Algorithm 2: 3/4 of the work) run in fp32 on
+                              single-precision copies of the z-shifted spectra and phase factors; step 1, the z
+                              shifts, the forward z pass, steps 7-10 and the Nyquist-plane terms stay fp64.  Errors of
+                              ~1e-6 of the GAIN term: within 1e-4 of max|Q| away from equilibrium, not near it
+                              (DESIGN.md section 8e).  VHS pairs, table_mode 0, N <= 32 only: DGFS_ENOSUP otherwise. */
 } dgfs_params;
 
 /* Algorithm 1: quadratures, truncation radius (Eq. 9), prefactors (Eq. 6) and the
@@ -118,6 +125,12 @@ int dgfs_get_quadrature(const dgfs_ctx *c, double *R, double *rho, double *w_rho
  * NULL. The internal device tables are factored/compressed; this call expands them with the
  * library's own kernels. */
 int dgfs_get_tables(dgfs_ctx *c, int p, int q, double *a, double *b, double *cc);
+
+/* Device bytes held by the full kernel-mode tables b^(pq)_rs(k) of the pairs that need one (VSS, table_mode 1).  With
+ * table_mode 0 these are stored once per orbit of the sphere rule under sign flips and the x <-> z swap, on the extended grid
+ * [-N/2, N/2]^3 (b_rs(k) depends on k through |k| and k . sigma_s only, Eq. 16): [N_rho][orbits][(N+1)^3] complex
+ * instead of the paper's [N_rho][M][N^3].  Environment DGFS_BTABLE=full keeps the paper's layout. */
+size_t dgfs_table_bytes(const dgfs_ctx *c);
 
 /* FLOP count of one pair evaluation as executed (SURVEY 8(d) / DESIGN.md "Roofline"), for the
  * benchmark's roofline line. */

@@ -19,7 +19,7 @@ ABI_SYMBOLS = (
     "dgfs_workspace_bytes", "dgfs_reserve", "dgfs_get_quadrature", "dgfs_get_tables",
     "dgfs_flops_per_pair_eval", "dgfs_step", "dgfs_step_euler", "dgfs_advect_rhs",
     "dgfs_launch_count", "dgfs_profile_enable", "dgfs_profile_count", "dgfs_profile_get",
-    "dgfs_profile_reset", "dgfs_collide_host", "dgfs_measure_fp64_peak",
+    "dgfs_profile_reset", "dgfs_collide_host", "dgfs_measure_fp64_peak", "dgfs_table_bytes",
 )
 
 DGFS_OK, DGFS_EINVAL, DGFS_ECUDA, DGFS_ENOMEM, DGFS_ENOSUP = 0, -1, -2, -3, -4
@@ -40,7 +40,7 @@ class _Params(C.Structure):
         ("prefactor", _dp), ("N", C.c_int), ("N_rho", C.c_int), ("M", C.c_int),
         ("L", C.c_double), ("R", C.c_double), ("sigma", _dp), ("w_sigma", _dp),
         ("table_mode", C.c_int), ("M_pre", C.c_int), ("sigma_pre", _dp), ("w_pre", _dp),
-        ("device", C.c_int), ("nyquist_filter", C.c_int),
+        ("device", C.c_int), ("nyquist_filter", C.c_int), ("precision", C.c_int),
     ]
 
 
@@ -97,6 +97,8 @@ def load_library():
     lib.dgfs_measure_fp64_peak.restype = ip
     lib.dgfs_workspace_bytes.argtypes = [vp, ip]
     lib.dgfs_workspace_bytes.restype = C.c_size_t
+    lib.dgfs_table_bytes.argtypes = [vp]
+    lib.dgfs_table_bytes.restype = C.c_size_t
     lib.dgfs_reserve.argtypes = [vp, ip]
     lib.dgfs_reserve.restype = ip
     lib.dgfs_get_quadrature.argtypes = [vp, _dp, _dp, _dp, _dp, _dp, _dp]
@@ -152,7 +154,7 @@ def dgfs_last_error(ctx=None):
 
 
 def dgfs_create(mass, omega, alpha, N, N_rho, M, L, kn=None, prefactor=None, R=0.0, sigma=None,
-                w_sigma=None, table_mode=0, sigma_pre=None, w_pre=None, device=0, nyquist_filter=False):
+                w_sigma=None, table_mode=0, sigma_pre=None, w_pre=None, device=0, nyquist_filter=False, precision=0):
     """Algorithm 1 on the device.  Returns the opaque context handle."""
     lib = load_library()
     ns = len(np.asarray(mass).reshape(-1))
@@ -172,6 +174,7 @@ def dgfs_create(mass, omega, alpha, N, N_rho, M, L, kn=None, prefactor=None, R=0
     p.M_pre = 0 if w_pre is None else len(np.asarray(w_pre).reshape(-1))
     p.device = int(device)
     p.nyquist_filter = int(bool(nyquist_filter))
+    p.precision = int(precision)
     out = C.c_void_p()
     rc = lib.dgfs_create(C.byref(p), C.byref(out))
     _check(None, rc)
@@ -237,6 +240,10 @@ def dgfs_workspace_bytes(ctx, nx):
 
 def dgfs_reserve(ctx, nx):
     _check(ctx, load_library().dgfs_reserve(ctx, int(nx)))
+
+
+def dgfs_table_bytes(ctx):
+    return int(load_library().dgfs_table_bytes(ctx))
 
 
 def dgfs_flops_per_pair_eval(ctx, p, q):
@@ -382,3 +389,6 @@ class Dgfs:
 
     def workspace_bytes(self, nx):
         return dgfs_workspace_bytes(self.ctx, nx)
+
+    def table_bytes(self):
+        return dgfs_table_bytes(self.ctx)

@@ -231,10 +231,15 @@ int build_tables_v1(dgfs_ctx* c) {
   if ((rc = upload(c, &c->d_v1_hz, hz, "upload z factors"))) return rc;
   if ((rc = upload(c, &c->d_v1_szv, szv, "upload z scalars"))) return rc;
   if ((rc = upload(c, &c->d_v1_hxy, hxy, "upload x,y factors"))) return rc;
+  if (c->precision == 1) {
+    std::vector<cplxf> hxyf(hxy.size());
+    for (size_t i = 0; i < hxy.size(); ++i) hxyf[i] = make_float2((float)hxy[i].x, (float)hxy[i].y);
+    if ((rc = upload(c, &c->d_v1_hxyf, hxyf, "upload x,y factors (fp32)"))) return rc;
+  }
   if ((rc = upload(c, &c->d_v1_sxy, sxy, "upload x,y scalars"))) return rc;
   V1Tables& t = c->v1;
   t.nz = nz; t.zsp = c->d_v1_zsp; t.zmap = c->d_v1_zmap; t.hz = c->d_v1_hz; t.szv = c->d_v1_szv;
-  t.hxy = c->d_v1_hxy; t.sxy = c->d_v1_sxy; t.smask = c->d_v1_smask; t.sskip = c->d_v1_sskip; t.tsrc = c->d_v1_tsrc; t.fsrc_s = c->d_v1_fsrc_s; t.fscale = c->d_v1_fscale; t.anti = c->d_v1_anti; t.tpartner = c->d_v1_tpartner;
+  t.hxy = c->d_v1_hxy; t.hxyf = c->d_v1_hxyf; t.sxy = c->d_v1_sxy; t.smask = c->d_v1_smask; t.sskip = c->d_v1_sskip; t.tsrc = c->d_v1_tsrc; t.fsrc_s = c->d_v1_fsrc_s; t.fscale = c->d_v1_fscale; t.anti = c->d_v1_anti; t.tpartner = c->d_v1_tpartner;
   t.jobs = c->d_v1_jobs; t.njobs = c->d_v1_njobs;
   return DGFS_OK;
 }
@@ -242,7 +247,7 @@ int build_tables_v1(dgfs_ctx* c) {
 void free_tables_v1(dgfs_ctx* c) {
   cudaFree(c->d_v1_zsp); cudaFree(c->d_v1_zmap); cudaFree(c->d_v1_hz); cudaFree(c->d_v1_szv);
   cudaFree(c->d_v1_hxy); cudaFree(c->d_v1_sxy); cudaFree(c->d_v1_smask); cudaFree(c->d_v1_sskip); cudaFree(c->d_v1_tsrc); cudaFree(c->d_v1_fsrc_s); cudaFree(c->d_v1_fscale); cudaFree(c->d_v1_anti); cudaFree(c->d_v1_tpartner);
-  cudaFree(c->d_v1_jobs); cudaFree(c->d_v1_njobs);
+  cudaFree(c->d_v1_jobs); cudaFree(c->d_v1_njobs); cudaFree(c->d_v1_hxyf);
 }
 
 // ---------------------------------------------------------------- device code -------------------
@@ -279,6 +284,13 @@ __device__ __forceinline__ void cp_async16(void* smem, const void* gmem) {
   const unsigned sa = (unsigned)__cvta_generic_to_shared(smem);
   asm volatile("cp.async.cg.shared.global [%0], [%1], 16;\n" ::"r"(sa), "l"(gmem));
 }
+__device__ __forceinline__ void cp_async8(void* smem, const void* gmem) {
+  const unsigned sa = (unsigned)__cvta_generic_to_shared(smem);
+  asm volatile("cp.async.ca.shared.global [%0], [%1], 8;\n" ::"r"(sa), "l"(gmem));
+}
+__device__ __forceinline__ void cp_async_el(cplx* smem, const cplx* gmem) { cp_async16(smem, gmem); }
+__device__ __forceinline__ void cp_async_el(cplxf* smem, const cplxf* gmem) { cp_async8(smem, gmem); }
+template <class C> __device__ __forceinline__ C cvt(cplx v) { return mkc<C>((typename real_of<C>::type)v.x, (typename real_of<C>::type)v.y); }
 __device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;\n" ::); }
 __device__ __forceinline__ void cp_async_wait_all() { asm volatile("cp.async.wait_group 0;\n" ::: "memory"); }
 template <int PENDING>
@@ -317,8 +329,8 @@ __device__ __forceinline__ void fence_mbar_init() { asm volatile("fence.mbarrier
 // multiplies, transforms in registers and stores its own array.
 // in: fhh[xl][species][lz][lx][m];  out: Gz[xl][k - kbase][cz][lx][m], kstride arrays per point (the jobs that depend
 // on the radial node and the sigma_z = 0 jobs, which do not, live in separate buffers: GzView below).
-template <int N>
-__global__ void __launch_bounds__(128, 3) k_zshift(V1Tables t, int ns, const cplx* __restrict__ fhh, cplx* __restrict__ Gz, int r, int k0, int nk,
+template <int N, class CO>
+__global__ void __launch_bounds__(128, 3) k_zshift(V1Tables t, int ns, const cplx* __restrict__ fhh, CO* __restrict__ Gz, int r, int k0, int nk,
                                                    int kbase, int kstride) {
   constexpr int H = N / 2, NP = N * H;
   extern __shared__ cplx sm[];                       // [lz][128]
@@ -343,22 +355,24 @@ __global__ void __launch_bounds__(128, 3) k_zshift(V1Tables t, int ns, const cpl
 #pragma unroll
     for (int i = 0; i < N; ++i) v[i] = cmul(sm[i * 128 + threadIdx.x], __ldg(&hz[i]));
     fft_reg<N, +1>(v);
-    cplx* dst = Gz + ((size_t)xl * kstride + (k - kbase)) * (size_t)(N * NP) + pid;
+    CO* dst = Gz + ((size_t)xl * kstride + (k - kbase)) * (size_t)(N * NP) + pid;      // CO = float2: precision 1
 #pragma unroll
-    for (int i = 0; i < N; ++i) dst[(size_t)i * NP] = v[i];
+    for (int i = 0; i < N; ++i) dst[(size_t)i * NP] = cvt<CO>(v[i]);
   }
 }
 
 // Where the z-shifted arrays of a chunk live: jobs 0 .. nzr-1 depend on the radial node (double-buffered, one buffer
 // per radial node in flight), jobs nzr .. nz-1 (sigma_z = 0) are written once per chunk.
-struct GzView {
-  const cplx* r;             // [xl][nzr][cz][lx][m]
-  const cplx* z0;            // [xl][nz - nzr][cz][lx][m]
+template <class C>
+struct GzViewT {
+  const C* r;                // [xl][nzr][cz][lx][m]
+  const C* z0;               // [xl][nz - nzr][cz][lx][m]
   int nzr, nz0;
-  __device__ __forceinline__ const cplx* job(int xl, int k, size_t arr) const {
+  __device__ __forceinline__ const C* job(int xl, int k, size_t arr) const {
     return k < nzr ? r + ((size_t)xl * nzr + k) * arr : z0 + ((size_t)xl * nz0 + (k - nzr)) * arr;
   }
 };
+typedef GzViewT<cplx> GzView;
 
 // Per-warp shared memory of a plane job: the N x (N+1) tile (input columns, then the transposition) and
 // the job's small tables.
@@ -438,12 +452,13 @@ __global__ void __launch_bounds__(128) k_nyq1d(V1Tables t, DevTables tab, const 
 
 // Pass 1 of a plane job (lane = (side, m), column m of the Hermitian half): multiply by the factor along
 // the pass-1 index, inverse transform in registers, factor of the lane's own column, back into the tile.
-template <int N, bool CORR>
-__device__ __forceinline__ void job_pass1(cplx* buf, int ln, int side, int m, double szs, double scale,
-                                          bool unit_i = false, bool real_m = false) {
+template <int N, bool CORR, class C>
+__device__ __forceinline__ void job_pass1(C* buf, int ln, int side, int m, typename real_of<C>::type szs,
+                                          typename real_of<C>::type scale, C c1, bool unit_i = false, bool real_m = false) {
   typedef JobSmem<N> JS;
+  typedef typename real_of<C>::type R;
   constexpr int H = N / 2, P = JS::P;
-  cplx v[N];
+  C v[N];
   if (unit_i) {
     // theta = 0 along the pass-1 axis: the factor is the same real number for every index; the caller has
     // folded it into `scale` (warp-uniform branch)
@@ -453,49 +468,49 @@ __device__ __forceinline__ void job_pass1(cplx* buf, int ln, int side, int m, do
 #pragma unroll
     for (int i = 0; i < N; ++i) v[i] = cmul(buf[i * P + ln], buf[JS::HI + side * JS::TS + i]);
   }
-  if (CORR) {
-    const cplx c1 = buf[JS::VYH + ln];
-    v[H].x = fma(-szs, c1.x, v[H].x);
-    v[H].y = fma(-szs, c1.y, v[H].y);
+  if (CORR) {            // c1: the x-Nyquist row correction of this lane's column (NyqLayout::VYH)
+    v[H].x = fma_(-szs, c1.x, v[H].x);
+    v[H].y = fma_(-szs, c1.y, v[H].y);
   }
   fft_reg<N, +1>(v);
   // complex h[m] for m >= 1; for the packed lane m = 0 the real h[0], h[H] scale Re (column 0) and
   // Im (column H) separately
-  const cplx hy0 = buf[JS::HM + side * JS::TS + m];
-  const double hyH = buf[JS::HM + side * JS::TS + H].x;
-  const double ya = scale * hy0.x, yb = (m == 0) ? 0.0 : -scale * hy0.y, yc = (m == 0) ? 0.0 : scale * hy0.y,
-               yd = (m == 0) ? scale * hyH : scale * hy0.x;
+  const C hy0 = buf[JS::HM + side * JS::TS + m];
+  const R hyH = buf[JS::HM + side * JS::TS + H].x;
+  const R ya = scale * hy0.x, yb = (m == 0) ? (R)0 : -scale * hy0.y, yc = (m == 0) ? (R)0 : scale * hy0.y,
+          yd = (m == 0) ? scale * hyH : scale * hy0.x;
   if (real_m) {
     // theta = 0 along the pass-2 axis: every h[m] is the same real number (yb = yc = 0)
 #pragma unroll
-    for (int i = 0; i < N; ++i) buf[i * P + ln] = make_double2(v[i].x * ya, v[i].y * yd);
+    for (int i = 0; i < N; ++i) buf[i * P + ln] = mkc<C>(v[i].x * ya, v[i].y * yd);
   } else {
 #pragma unroll
     for (int i = 0; i < N; ++i)
-      buf[i * P + ln] = make_double2(fma(v[i].x, ya, v[i].y * yb), fma(v[i].x, yc, v[i].y * yd));
+      buf[i * P + ln] = mkc<C>(fma_(v[i].x, ya, v[i].y * yb), fma_(v[i].x, yc, v[i].y * yd));
   }
 }
 
 // Input of pass 2 (lane = pass-1 output index): the N packed columns X = Y_A + i Y_B, the mirror half by
-// conjugation (Y_A, Y_B are Hermitian along the pass-2 index).
-template <int N, bool CORR>
-__device__ __forceinline__ void job_pass2_in(const cplx* buf, int ln, double szs, double sxb, cplx (&X)[N]) {
+// conjugation (Y_A, Y_B are Hermitian along the pass-2 index).  vx, vz: the y-Nyquist column and (H,H) element
+// corrections of this lane / plane (NyqLayout::VXP, VZP).
+template <int N, bool CORR, class C>
+__device__ __forceinline__ void job_pass2_in(const C* buf, int ln, typename real_of<C>::type szs,
+                                             typename real_of<C>::type sxb, C vx, C vz, C (&X)[N]) {
   typedef JobSmem<N> JS;
   constexpr int H = N / 2, P = JS::P;
-  const cplx* row = buf + ln * P;
-  const cplx a0 = row[0], b0 = row[H];
-  X[0] = make_double2(a0.x, b0.x);
-  X[H] = make_double2(a0.y, b0.y);
+  const C* row = buf + ln * P;
+  const C a0 = row[0], b0 = row[H];
+  X[0] = mkc<C>(a0.x, b0.x);
+  X[H] = mkc<C>(a0.y, b0.y);
   if (CORR) {
-    const cplx vx = buf[JS::VXP + ln], vz = buf[JS::VZP];
     X[H].x -= szs * vx.x + sxb * vz.x;
     X[H].y -= szs * vx.y + sxb * vz.y;
   }
 #pragma unroll
   for (int mm = 1; mm < H; ++mm) {
-    const cplx ya = row[mm], yb = row[H + mm];
-    X[mm] = make_double2(ya.x - yb.y, ya.y + yb.x);
-    X[N - mm] = make_double2(ya.x + yb.y, yb.x - ya.y);
+    const C ya = row[mm], yb = row[H + mm];
+    X[mm] = mkc<C>(ya.x - yb.y, ya.y + yb.x);
+    X[N - mm] = mkc<C>(ya.x + yb.y, yb.x - ya.y);
   }
 }
 
@@ -579,10 +594,10 @@ __global__ void __launch_bounds__(32 * NW) k_nyq2(V1Tables t, DevTables tab, con
     cp_async_wait_all();
     __syncwarp();
     cplx X[N];
-    if (act) job_pass1<N, false>(buf, ln, side, m, 0.0, scale);
+    if (act) job_pass1<N, false>(buf, ln, side, m, 0.0, scale, make_double2(0.0, 0.0));
     __syncwarp();
     cplx vt = make_double2(0.0, 0.0);
-    if (act) { job_pass2_in<N, false>(buf, ln, 0.0, 0.0, X); vt = buf[JS::VZP]; }
+    if (act) { job_pass2_in<N, false>(buf, ln, 0.0, 0.0, make_double2(0.0, 0.0), make_double2(0.0, 0.0), X); vt = buf[JS::VZP]; }
     __syncwarp();
     const double scale_next = (sn < tab.M) ? scale_of(sn) : 0.0;
     if (sn < tab.M) issue(sn);
@@ -617,92 +632,108 @@ __global__ void __launch_bounds__(32 * NW) k_nyq2(V1Tables t, DevTables tab, con
 //   pass 2: lane = cx rebuilds the N packed columns X[ly] = Y_A + i Y_B (mirror half by conjugation), inverse
 //           y pass: Z = a_r + i b_r;  acc[cy] += Re Z Im Z
 // in: S[item][cz][cy][cx] = -sum_s Re W Im W (k_wterm);  out: T[item][cz][kx][ky <= H] = fft_xy of S_r(., ., cz).
-template <int N, int W>
-__global__ void __launch_bounds__(32 * W) __maxnreg__(W == 2 ? 200 : 255) k_xy(V1Tables t, DevTables tab, GzView Gz,
-                                               const cplx* __restrict__ nyq, const double* __restrict__ S,
+// C = double2: Algorithm 2 in fp64.  C = float2 (dgfs_params::precision = 1): the same job on single-precision copies
+// of the z-shifted arrays and factor tables; the Nyquist corrections and S are read in double and converted, T is
+// written in double (the forward z pass and everything after it stay fp64).
+template <int N, int W, class C>
+__global__ void __launch_bounds__(32 * W) __maxnreg__(sizeof(C) == 8 ? 128 : (W == 2 ? 200 : 255)) k_xy(V1Tables t, DevTables tab, GzViewT<C> Gz,
+                                               const C* __restrict__ hxy, const cplx* __restrict__ nyq, const double* __restrict__ S,
                                                cplx* __restrict__ T, int r) {
   constexpr int H = N / 2, NH = N * H, N2 = N * N;
+  constexpr bool F32 = sizeof(C) == sizeof(float2);
+  typedef typename real_of<C>::type R;
   typedef NyqLayout<N> NL;
   typedef JobSmem<N> JS;
   constexpr int P = JS::P;
   static_assert(N <= 32, "one lane per pencil");
-  extern __shared__ cplx sm[];
+  extern __shared__ __align__(16) unsigned char sm_raw[];
+  C* sm = reinterpret_cast<C*>(sm_raw);
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
   const int cz = blockIdx.x * W + warp, item = blockIdx.y;
   const int pair = item % tab.npairs, xl = item / tab.npairs;
   if (cz >= N || tab.full[pair] || t.tsrc[pair] != pair) return;      // R-11: (q,p) uses the buffer of (p,q)
-  cplx* buf = sm + (size_t)warp * JS::WORDS;
+  C* buf = sm + (size_t)warp * JS::WORDS;
   const bool act = lane < N;
   const int ln = act ? lane : 0;
   const int side = ln / H, m = ln % H;
-  const double szs = (cz & 1) ? -1.0 : 1.0;
-  const double sxb = (ln & 1) ? -1.0 : 1.0;
+  const R szs = (cz & 1) ? (R)-1 : (R)1;
+  const R sxb = (ln & 1) ? (R)-1 : (R)1;
   const size_t goff = (size_t)cz * NH + m;
-  const cplx* hbase = t.hxy + (((size_t)pair * tab.N_rho + r) * tab.M) * 4 * N;
+  const C* hbase = hxy + (((size_t)pair * tab.N_rho + r) * tab.M) * 4 * N;
   const cplx* nbase = nyq + (size_t)item * tab.M * NL::STRIDE;
   // job = {s, z job of side A, z job of side B, smask[s]} (V1Tables::jobs): the entry of the next job is fetched a
   // whole job ahead, so no look-up sits between the end of one job and the prefetch of the next
   const int4* jl = t.jobs + (size_t)pair * tab.M;
   const int nj = t.njobs[pair];
+  cplx n1 = make_double2(0.0, 0.0), n2 = n1, n3 = n1;       // F32: Nyquist corrections of the job in flight (registers)
   auto issue = [&](int4 jb) {
     if (act) {
-      const cplx* g = Gz.job(xl, side ? jb.z : jb.y, (size_t)(N * NH)) + goff;
+      const C* g = Gz.job(xl, side ? jb.z : jb.y, (size_t)(N * NH)) + goff;
 #pragma unroll
-      for (int i = 0; i < N; ++i) cp_async16(&buf[i * P + ln], g + i * H);
-      const cplx* hx = hbase + (size_t)jb.x * 4 * N;       // [side][x|y][N]
-      cp_async16(&buf[JS::HI + ln], hx + ln);               // h_x side A
-      cp_async16(&buf[JS::HI + JS::TS + ln], hx + 2 * N + ln);   // h_x side B
-      cp_async16(&buf[JS::HM + ln], hx + N + ln);           // h_y side A
-      cp_async16(&buf[JS::HM + JS::TS + ln], hx + 3 * N + ln);   // h_y side B
+      for (int i = 0; i < N; ++i) cp_async_el(&buf[i * P + ln], g + i * H);
+      const C* hx = hbase + (size_t)jb.x * 4 * N;          // [side][x|y][N]
+      cp_async_el(&buf[JS::HI + ln], hx + ln);               // h_x side A
+      cp_async_el(&buf[JS::HI + JS::TS + ln], hx + 2 * N + ln);   // h_x side B
+      cp_async_el(&buf[JS::HM + ln], hx + N + ln);           // h_y side A
+      cp_async_el(&buf[JS::HM + JS::TS + ln], hx + 3 * N + ln);   // h_y side B
       const cplx* nq = nbase + (size_t)jb.x * NL::STRIDE;
-      cp_async16(&buf[JS::VYH + ln], nq + NL::VYH + ln);
-      cp_async16(&buf[JS::VXP + ln], nq + NL::VXP + ln);
-      if (ln == 0) cp_async16(&buf[JS::VZP], nq + NL::VZP + cz);
+      if (F32) {
+        n1 = __ldg(nq + NL::VYH + ln); n2 = __ldg(nq + NL::VXP + ln); n3 = __ldg(nq + NL::VZP + cz);
+      } else {
+        cplx* bd = reinterpret_cast<cplx*>(buf);
+        cp_async16(&bd[JS::VYH + ln], nq + NL::VYH + ln);
+        cp_async16(&bd[JS::VXP + ln], nq + NL::VXP + ln);
+        if (ln == 0) cp_async16(&bd[JS::VZP], nq + NL::VZP + cz);
+      }
     }
     cp_async_commit();
   };
   int mask = 0;
   if (nj > 0) { const int4 j0 = __ldg(&jl[0]); issue(j0); mask = j0.w; }
   // start from the Nyquist-field product written by k_wterm
-  double acc[N];
+  R acc[N];
   {
     const double* w0 = S + ((size_t)item * N + cz) * N2 + ln;
 #pragma unroll
-    for (int j = 0; j < N; ++j) acc[j] = w0[j * N];
+    for (int j = 0; j < N; ++j) acc[j] = (R)w0[j * N];
   }
   for (int j = 0; j < nj; ++j) {
     const int4 jn = __ldg(&jl[j + 1 < nj ? j + 1 : j]);          // used after pass 1: its latency hides behind it
     cp_async_wait_all();
     __syncwarp();
-    cplx X[N];
+    C X[N];
     if (act) {
       // sigma_x = 0: h_x is the constant w_s / N (side A) or 1 / N; sigma_y = 0: h_y is the constant 1 / N
       const bool ux_ = (mask & 1) != 0, ry_ = (mask & 2) != 0;
-      job_pass1<N, true>(buf, ln, side, m, szs, ux_ ? buf[JS::HI + side * JS::TS].x : 1.0, ux_, ry_);
+      const C c1 = F32 ? cvt<C>(n1) : buf[JS::VYH + ln];
+      job_pass1<N, true>(buf, ln, side, m, szs, ux_ ? buf[JS::HI + side * JS::TS].x : (R)1, c1, ux_, ry_);
     }
     __syncwarp();
-    if (act) job_pass2_in<N, true>(buf, ln, szs, sxb, X);
+    if (act) {
+      const C c2 = F32 ? cvt<C>(n2) : buf[JS::VXP + ln], c3 = F32 ? cvt<C>(n3) : buf[JS::VZP];
+      job_pass2_in<N, true>(buf, ln, szs, sxb, c2, c3, X);
+    }
     __syncwarp();
     if (j + 1 < nj) issue(jn);               // the tile is free: the next job's data arrives during pass 2
     if (act) {
       fft_reg<N, +1>(X);
 #pragma unroll
-      for (int jj = 0; jj < N; ++jj) acc[jj] = fma(X[jj].x, X[jj].y, acc[jj]);
+      for (int jj = 0; jj < N; ++jj) acc[jj] = fma_(X[jj].x, X[jj].y, acc[jj]);
     }
     mask = jn.w;
   }
   // forward y and x passes of the real plane S_r(., ., cz) (steps 6-7, after R-1)
   if (act) {
-    cplx v[N];
+    C v[N];
 #pragma unroll
-    for (int j = 0; j < N; ++j) v[j] = make_double2(acc[j], 0.0);
+    for (int j = 0; j < N; ++j) v[j] = mkc<C>(acc[j], (R)0);
     fft_reg<N, -1>(v);
 #pragma unroll
     for (int j = 0; j < N; ++j) buf[j * P + ln] = v[j];          // [ky][cx]
   }
   __syncwarp();
   if (act) {
-    cplx v[N];
+    C v[N];
 #pragma unroll
     for (int i = 0; i < N; ++i) v[i] = buf[ln * P + i];          // lane = ky
     fft_reg<N, -1>(v);
@@ -710,7 +741,7 @@ __global__ void __launch_bounds__(32 * W) __maxnreg__(W == 2 ? 200 : 255) k_xy(V
     if (ln <= H) {
       cplx* o = T + ((size_t)item * N + cz) * (size_t)(N * (H + 1)) + ln;
 #pragma unroll
-      for (int k = 0; k < N; ++k) o[k * (H + 1)] = v[k];         // [cz][kx][ky <= H]
+      for (int k = 0; k < N; ++k) o[k * (H + 1)] = make_double2((double)v[k].x, (double)v[k].y);         // [cz][kx][ky <= H]
     }
   }
 }
@@ -786,11 +817,11 @@ __global__ void __launch_bounds__(32 * W) k_xy_full(V1Tables t, DevTables tab, G
       // sigma_x = 0: h_x is the constant w_s / N (side A) or 1 / N; sigma_y = 0: h_y is the constant 1 / N
       const int mk = t.smask[s];
       const bool ux_ = (mk & 1) != 0, ry_ = (mk & 2) != 0;
-      job_pass1<N, true>(buf, ln, side, m, szs, ux_ ? buf[JS::HI + side * JS::TS].x : 1.0, ux_, ry_);
+      job_pass1<N, true>(buf, ln, side, m, szs, ux_ ? buf[JS::HI + side * JS::TS].x : 1.0, buf[JS::VYH + ln], ux_, ry_);
     }
     __syncwarp();
     if (act) {
-      job_pass2_in<N, true>(buf, ln, szs, sxb, X);
+      job_pass2_in<N, true>(buf, ln, szs, sxb, buf[JS::VXP + ln], buf[JS::VZP], X);
       fft_reg<N, +1>(X);                                   // Z = a_r + i b_r, lane = cx, index = cy
       const cplx uyv = buf[FS::UY + ln];
 #pragma unroll
@@ -844,6 +875,7 @@ __global__ void __launch_bounds__(256) k_zfwd_full(DevTables tab, V1Tables t, co
   if (pid >= N2 || !tab.full[pair] || t.tsrc[pair] != pair) return;
   const int M = tab.M;
   const int partner = t.tpartner[pair];                 // pair that reads this one's products, or -1
+  const int kxs = sfreq(pid / N, N), kys = sfreq(pid % N, N);
   const unsigned char* skip = t.sskip + (size_t)pair * M;
   const double scale = tab.w_rho[r];
   cplx acc[H], acc2[H];
@@ -862,20 +894,22 @@ __global__ void __launch_bounds__(256) k_zfwd_full(DevTables tab, V1Tables t, co
     }
     fft_reg<H, -1>(u);
     const int sa = t.anti[s];
-    const cplx* bf = tab.bfull[pair] + ((size_t)r * M + s) * N3 + pid;
     // same-species pair: s also stands for its antipode
     const bool twin = sa >= 0 && skip[sa] && t.fsrc_s[(size_t)pair * M + sa] == s;
-    const cplx* bt = twin ? tab.bfull[pair] + ((size_t)r * M + sa) * N3 + pid : nullptr;
     const double ft = twin ? t.fscale[(size_t)pair * M + sa] : 0.0;
-    const cplx* bp = (partner >= 0) ? tab.bfull[partner] + ((size_t)r * M + sa) * N3 + pid : nullptr;
     const double fp = (partner >= 0) ? t.fscale[(size_t)partner * M + sa] : 0.0;
+    const bool sym = tab.bsym != 0;
+    const BSweep b1 = bfull_sweep(tab, pair, r, s, kxs, kys);
+    const BSweep b2 = bfull_sweep(tab, pair, r, twin ? sa : s, kxs, kys);
+    const BSweep b3 = bfull_sweep(tab, partner >= 0 ? partner : pair, r, partner >= 0 ? sa : s, kxs, kys);
 #pragma unroll
     for (int k = 0; k < H; ++k) {
-      const size_t o = (size_t)(2 * k + par) * N2;
-      cplx b = bf[o];
-      if (twin) { const cplx b2 = bt[o]; b.x = fma(ft, b2.x, b.x); b.y = fma(ft, b2.y, b.y); }
+      const int iz = 2 * k + par, kzs = iz - (iz >= H ? N : 0);
+      const long zi = sym ? kzs : iz;
+      cplx b = b1.p[zi * b1.sz];
+      if (twin) { const cplx bb = b2.p[zi * b2.sz]; b.x = fma(ft, bb.x, b.x); b.y = fma(ft, bb.y, b.y); }
       acc[k] = cfma(b, u[k], acc[k]);
-      if (partner >= 0) { const cplx b3 = bp[o]; acc2[k] = cfma(make_double2(fp * b3.x, fp * b3.y), u[k], acc2[k]); }
+      if (partner >= 0) { const cplx b3v = b3.p[zi * b3.sz]; acc2[k] = cfma(make_double2(fp * b3v.x, fp * b3v.y), u[k], acc2[k]); }
     }
   }
   cplx* dst = QG + (size_t)item * qstride + pid;
@@ -1158,7 +1192,8 @@ PlanV1 plan_v1(const dgfs_ctx* c, int nx) {
   const size_t items = (size_t)nbx * c->npairs;
   const size_t nyq_stride = 4 * N + 3 * N * N;
   const size_t nzr = c->v1_nz - c->v1_nz0;
-  size_t gz = (size_t)nbx * nzr * (arr / 2), g2 = items * 2 * arr;
+  const size_t gel = c->precision == 1 ? 2 : 1;              // precision 1: z-shifted arrays in float2
+  size_t gz = (size_t)nbx * nzr * (arr / 2) / gel, g2 = items * 2 * arr;
   size_t off = 0;
   auto take = [&](size_t bytes) { size_t o = off; off += (bytes + 255) & ~(size_t)255; return o; };
   pl.off_fhat = take((size_t)nbx * c->ns * arr);
@@ -1170,7 +1205,7 @@ PlanV1 plan_v1(const dgfs_ctx* c, int nx) {
   pl.off_qg = take(items * pl.qstride * sizeof(cplx));
   pl.off_gzr[0] = take(gz > g2 ? gz : g2);               // also the scratch of step 10
   pl.off_gzr[1] = pl.nbuf > 1 ? take(gz) : pl.off_gzr[0];
-  pl.off_gz0 = take((size_t)nbx * c->v1_nz0 * (arr / 2));
+  pl.off_gz0 = take((size_t)nbx * c->v1_nz0 * (arr / 2) / gel);
   pl.nyq_bytes = items * c->M * nyq_stride * sizeof(cplx);
   pl.off_nyq[0] = take(pl.nyq_bytes);
   pl.off_nyq[1] = pl.nbuf > 1 ? take(pl.nyq_bytes) : pl.off_nyq[0];
@@ -1293,6 +1328,7 @@ static int collide_v1_impl(dgfs_ctx* c, const double* f, double* out, int nx, bo
   int rc = ensure_workspace(c, pl.total, st);
   if (rc) return rc;
   const bool ov = c->v1_overlap != 0;
+  const bool f32 = c->precision == 1;
   cudaStream_t sa = ov ? c->aux : st, sz = ov ? c->aux2 : st;
   auto wait = [&](cudaStream_t s, cudaEvent_t e) { if (ov) cudaStreamWaitEvent(s, e, 0); };
   auto record = [&](cudaEvent_t e, cudaStream_t s) { if (ov) cudaEventRecord(e, s); };
@@ -1336,12 +1372,14 @@ static int collide_v1_impl(dgfs_ctx* c, const double* f, double* out, int nx, bo
     cudaFuncSetAttribute(k_plane_fwd<N, W, 0>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_plane);
     cudaFuncSetAttribute(k_plane_fwd<N, W, 1>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_plane);
     cudaFuncSetAttribute(k_final_xy_h<N>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_final);
-    cudaFuncSetAttribute(k_xy<N, W>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_xy);
-    cudaFuncSetAttribute(k_xy<N, 2>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_xy / 2);
+    cudaFuncSetAttribute(k_xy<N, W, cplx>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_xy);
+    cudaFuncSetAttribute(k_xy<N, W, cplxf>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_xy / 2);
+    cudaFuncSetAttribute(k_xy<N, 2, cplx>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_xy / 2);
     cudaFuncSetAttribute(k_xy_full<N, W>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_xyf);
     cudaFuncSetAttribute(k_wterm<N>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_wt);
     cudaFuncSetAttribute(k_nyq2<N, 2>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_nyq);
-    cudaFuncSetAttribute(k_zshift<N>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_zs);
+    cudaFuncSetAttribute(k_zshift<N, cplx>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_zs);
+    cudaFuncSetAttribute(k_zshift<N, cplxf>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_zs);
     cudaFuncSetAttribute(k_zfwd_acc<N, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_zacc);
     cudaFuncSetAttribute(k_zfwd_acc<N, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_zacc);
     c->v1_attr_done = true;
@@ -1381,7 +1419,8 @@ static int collide_v1_impl(dgfs_ctx* c, const double* f, double* out, int nx, bo
     if (nvhs > 0) wait(sz, c->ev_head);
     if (nz0 > 0) {     // the unshifted arrays (sigma_z = 0), the same for every radial node
       ProfScope ps(c->prof, sa, "k_zshift", items * fl.zshift * nz0 / (nzr > 0 ? nzr : 1));
-      k_zshift<N><<<dim3(hpen_blocks, ns, nb), 128, smem_zs, sa>>>(c->v1, ns, fhh, Gz0, 0, nzr, nz0, nzr, nz0);
+      if (f32) k_zshift<N, cplxf><<<dim3(hpen_blocks, ns, nb), 128, smem_zs, sa>>>(c->v1, ns, fhh, (cplxf*)Gz0, 0, nzr, nz0, nzr, nz0);
+      else k_zshift<N, cplx><<<dim3(hpen_blocks, ns, nb), 128, smem_zs, sa>>>(c->v1, ns, fhh, Gz0, 0, nzr, nz0, nzr, nz0);
     }
     int ngroups = 0;
     for (int r = 0; r < c->N_rho; ++r) {
@@ -1390,7 +1429,8 @@ static int collide_v1_impl(dgfs_ctx* c, const double* f, double* out, int nx, bo
       if (r >= 2) wait(sa, c->ev_xy[b]);                     // the plane jobs of r - 2 have read buffer b
       if (nzr > 0)
       { ProfScope ps(c->prof, sa, "k_zshift", items * fl.zshift);
-        k_zshift<N><<<dim3(hpen_blocks, ns, nb), 128, smem_zs, sa>>>(c->v1, ns, fhh, GzR[b], r, 0, nzr, 0, nzr); }
+        if (f32) k_zshift<N, cplxf><<<dim3(hpen_blocks, ns, nb), 128, smem_zs, sa>>>(c->v1, ns, fhh, (cplxf*)GzR[b], r, 0, nzr, 0, nzr);
+        else k_zshift<N, cplx><<<dim3(hpen_blocks, ns, nb), 128, smem_zs, sa>>>(c->v1, ns, fhh, GzR[b], r, 0, nzr, 0, nzr); }
       if (!c->nyq_filter) {
       { ProfScope ps(c->prof, sa, "k_nyq1d", nb * run_all * c->M * 16.0 * N2);
         k_nyq1d<N><<<(items * c->M + 3) / 4, 128, 0, sa>>>(c->v1, c->tab, fhat, nyqb[b], r, items * c->M); }
@@ -1408,10 +1448,13 @@ static int collide_v1_impl(dgfs_ctx* c, const double* f, double* out, int nx, bo
         const int g = r / RG, slot = r % pl.tslots;
         if (r % RG == 0 && g >= 2) wait(st, c->ev_acc[g & 1]);       // the forward z pass of group g - 2 has read these slots
         { ProfScope ps(c->prof, st, "k_xy", nb * (run_vhs * (fl.xy - fwd_xy) + nrun_vhs * fwd_xy));
-          if (c->v1_xyw == 2)       // DGFS_V1_XYW=2: blocks of two warps, five per SM (ten warps at <= 204 registers)
-            k_xy<N, 2><<<dim3((N + 1) / 2, items), 64, smem_xy / 2, st>>>(c->v1, c->tab, gv, nyqb[b], Sb[b], T + (size_t)slot * slot_stride, r);
+          if (f32) {                // dgfs_params::precision = 1
+            const GzViewT<cplxf> gvf{(const cplxf*)GzR[b], (const cplxf*)Gz0, nzr, nz0};
+            k_xy<N, W, cplxf><<<dim3((N + W - 1) / W, items), 32 * W, smem_xy / 2, st>>>(c->v1, c->tab, gvf, c->v1.hxyf, nyqb[b], Sb[b], T + (size_t)slot * slot_stride, r);
+          } else if (c->v1_xyw == 2)       // DGFS_V1_XYW=2: blocks of two warps, five per SM (ten warps at <= 200 registers)
+            k_xy<N, 2, cplx><<<dim3((N + 1) / 2, items), 64, smem_xy / 2, st>>>(c->v1, c->tab, gv, c->v1.hxy, nyqb[b], Sb[b], T + (size_t)slot * slot_stride, r);
           else
-            k_xy<N, W><<<dim3((N + W - 1) / W, items), 32 * W, smem_xy, st>>>(c->v1, c->tab, gv, nyqb[b], Sb[b], T + (size_t)slot * slot_stride, r); }
+            k_xy<N, W, cplx><<<dim3((N + W - 1) / W, items), 32 * W, smem_xy, st>>>(c->v1, c->tab, gv, c->v1.hxy, nyqb[b], Sb[b], T + (size_t)slot * slot_stride, r); }
       }
       if (nfull > 0) {
         { ProfScope ps(c->prof, st, "k_xy_full", nb * (run_all - run_vhs) * fl.xy_full);

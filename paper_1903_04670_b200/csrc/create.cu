@@ -162,67 +162,91 @@ __global__ void k_closs0(cplx* out, int ns, int N, int N_rho, double L, const do
 // a_n = (2n+1)/2 I_n, I_0 = 2^{eta+1}/(eta+1), I_{n+1} = I_n (eta - n)/(eta + n + 2).
 // j_n by Miller's backward recurrence normalised with sum (2n+1) j_n^2 = 1 and the sign of j_0 / j_1.
 #define DGFS_NSER 224
+// F of the comment above times rho^{gamma+2}: one mode (kx, ky, kz) (signed frequencies), one sphere point sigma.
+__device__ cplx b_series(int kx, int ky, int kz, const double* sigma3, double mu_q, double rho_r, double L, double gam,
+                         double eta) {
+  const double pi = 3.14159265358979323846;
+  double ln = sqrt((double)(kx * kx + ky * ky + kz * kz));
+  double z = mu_q * (pi * rho_r / L) * ln;
+  double pref = 4.0 * pi * pow(rho_r, gam + 2.0);
+  double I0 = exp2(eta + 1.0) / (eta + 1.0);
+  if (ln == 0.0) return make_double2(pref * 0.5 * I0, 0.0);
+  double kappa = (kx * sigma3[0] + ky * sigma3[1] + kz * sigma3[2]) / ln;
+  kappa = fmin(1.0, fmax(-1.0, kappa));
+  // spherical Bessel j_0..j_nmax(z)
+  int nmax = (int)(z + 12.0 * cbrt(z + 1.0) + 20.0);
+  if (nmax > DGFS_NSER - 1) nmax = DGFS_NSER - 1;
+  double jn[DGFS_NSER];
+  if (z < 1e-3) {            // series j_n ~ z^n/(2n+1)!! (1 - z^2/(2(2n+3)))
+    double tterm = 1.0;
+    for (int n = 0; n <= nmax; ++n) { jn[n] = tterm * (1.0 - z * z / (2.0 * (2 * n + 3))); tterm *= z / (2 * n + 3); }
+  } else {
+    int nstart = nmax + 40;
+    double fp1 = 0.0, f = 1e-120, norm = 0.0;
+    for (int n = nstart; n >= 0; --n) {
+      // j_{n-1} = (2n+1)/z j_n - j_{n+1}
+      if (n <= nmax) jn[n] = f;
+      norm += (2 * n + 1) * f * f;
+      double fm1 = (2 * n + 1) / z * f - fp1;
+      fp1 = f; f = fm1;
+      if (fabs(f) > 1e120) {   // rescale so that f^2 in the norm cannot overflow
+        f *= 1e-120; fp1 *= 1e-120; norm *= 1e-240;
+        for (int m = n; m <= nmax; ++m) jn[m] *= 1e-120;
+      }
+    }
+    double scale = rsqrt(norm);
+    // fix the sign with whichever of j_0 = sin z / z, j_1 = sin z / z^2 - cos z / z is larger in magnitude
+    double sn, cs; sincos(z, &sn, &cs);
+    double j0 = sn / z, j1 = sn / (z * z) - cs / z;
+    if (fabs(j0) >= fabs(j1)) { if ((jn[0] * scale > 0) != (j0 > 0)) scale = -scale; }
+    else { if ((jn[1] * scale > 0) != (j1 > 0)) scale = -scale; }
+    for (int n = 0; n <= nmax; ++n) jn[n] *= scale;
+  }
+  double re = 0.0, im = 0.0;
+  double In = I0, Pm1 = 0.0, Pn = 1.0;     // P_{n-1}, P_n at kappa
+  for (int n = 0; n <= nmax; ++n) {
+    double term = 0.5 * (2 * n + 1) * In * jn[n] * Pn;
+    switch (n & 3) {            // (-i)^n
+      case 0: re += term; break;
+      case 1: im -= term; break;
+      case 2: re -= term; break;
+      default: im += term; break;
+    }
+    double Pp1 = ((2 * n + 1) * kappa * Pn - n * Pm1) / (n + 1);
+    Pm1 = Pn; Pn = Pp1;
+    In *= (eta - n) / (eta + n + 2.0);
+  }
+  return make_double2(pref * re, pref * im);
+}
+
+// out[r][s][N^3] (SPEC layout): every sphere point of the rule in full
 __global__ void k_bfull_series(cplx* out, int p, int q, int N, int N_rho, int M, double L, const double* mass,
                                double gam, double eta, const double* rho, const double* sigma) {
   const int N3 = N * N * N;
   const long total = (long)N_rho * M * N3;
-  const double pi = 3.14159265358979323846;
   const double mu_q = mass[q] / (mass[p] + mass[q]);
   for (long i = blockIdx.x * (long)blockDim.x + threadIdx.x; i < total; i += (long)gridDim.x * blockDim.x) {
     int idx = i % N3; long t = i / N3;
     int s = t % M, r = t / M;
     int kx, ky, kz; spec_freq(idx, N, kx, ky, kz);
-    double ln = sqrt((double)(kx * kx + ky * ky + kz * kz));
-    double z = mu_q * (pi * rho[r] / L) * ln;
-    double pref = 4.0 * pi * pow(rho[r], gam + 2.0);
-    double I0 = exp2(eta + 1.0) / (eta + 1.0);
-    if (ln == 0.0) { out[i] = make_double2(pref * 0.5 * I0, 0.0); continue; }
-    double kappa = (kx * sigma[s * 3] + ky * sigma[s * 3 + 1] + kz * sigma[s * 3 + 2]) / ln;
-    kappa = fmin(1.0, fmax(-1.0, kappa));
-    // spherical Bessel j_0..j_nmax(z)
-    int nmax = (int)(z + 12.0 * cbrt(z + 1.0) + 20.0);
-    if (nmax > DGFS_NSER - 1) nmax = DGFS_NSER - 1;
-    double jn[DGFS_NSER];
-    if (z < 1e-3) {            // series j_n ~ z^n/(2n+1)!! (1 - z^2/(2(2n+3)))
-      double tterm = 1.0;
-      for (int n = 0; n <= nmax; ++n) { jn[n] = tterm * (1.0 - z * z / (2.0 * (2 * n + 3))); tterm *= z / (2 * n + 3); }
-    } else {
-      int nstart = nmax + 40;
-      double fp1 = 0.0, f = 1e-120, norm = 0.0;
-      for (int n = nstart; n >= 0; --n) {
-        // j_{n-1} = (2n+1)/z j_n - j_{n+1}
-        if (n <= nmax) jn[n] = f;
-        norm += (2 * n + 1) * f * f;
-        double fm1 = (2 * n + 1) / z * f - fp1;
-        fp1 = f; f = fm1;
-        if (fabs(f) > 1e120) {   // rescale so that f^2 in the norm cannot overflow
-          f *= 1e-120; fp1 *= 1e-120; norm *= 1e-240;
-          for (int m = n; m <= nmax; ++m) jn[m] *= 1e-120;
-        }
-      }
-      double scale = rsqrt(norm);
-      // fix the sign with whichever of j_0 = sin z / z, j_1 = sin z / z^2 - cos z / z is larger in magnitude
-      double sn, cs; sincos(z, &sn, &cs);
-      double j0 = sn / z, j1 = sn / (z * z) - cs / z;
-      if (fabs(j0) >= fabs(j1)) { if ((jn[0] * scale > 0) != (j0 > 0)) scale = -scale; }
-      else { if ((jn[1] * scale > 0) != (j1 > 0)) scale = -scale; }
-      for (int n = 0; n <= nmax; ++n) jn[n] *= scale;
-    }
-    double re = 0.0, im = 0.0;
-    double In = I0, Pm1 = 0.0, Pn = 1.0;     // P_{n-1}, P_n at kappa
-    for (int n = 0; n <= nmax; ++n) {
-      double term = 0.5 * (2 * n + 1) * In * jn[n] * Pn;
-      switch (n & 3) {            // (-i)^n
-        case 0: re += term; break;
-        case 1: im -= term; break;
-        case 2: re -= term; break;
-        default: im += term; break;
-      }
-      double Pp1 = ((2 * n + 1) * kappa * Pn - n * Pm1) / (n + 1);
-      Pm1 = Pn; Pn = Pp1;
-      In *= (eta - n) / (eta + n + 2.0);
-    }
-    out[i] = make_double2(pref * re, pref * im);
+    out[i] = b_series(kx, ky, kz, sigma + 3 * s, mu_q, rho[r], L, gam, eta);
+  }
+}
+
+// Symmetry-compressed b (DevTables::bsym): out[r][u][(N+1)^3] for the nref reference sphere points refs[u] only, on the
+// EXTENDED frequency grid [-N/2, N/2]^3 ([kz][kx][ky], ky fastest): b_rs(k) depends on k through |k| and k . sigma_s,
+// so for sigma_s = G sigma_u (G a signed permutation of the axes) b_rs(k) = b_ru(G^T k), and G^T maps the grid
+// [-N/2, N/2) into the extended one (the Nyquist index -N/2 may change sign).
+__global__ void k_bsym_series(cplx* out, int p, int q, int N, int N_rho, int nref, const int* refs, double L,
+                              const double* mass, double gam, double eta, const double* rho, const double* sigma) {
+  const int E = N + 1, H = N / 2, E3 = E * E * E;
+  const long total = (long)N_rho * nref * E3;
+  const double mu_q = mass[q] / (mass[p] + mass[q]);
+  for (long i = blockIdx.x * (long)blockDim.x + threadIdx.x; i < total; i += (long)gridDim.x * blockDim.x) {
+    int idx = i % E3; long t = i / E3;
+    int u = t % nref, r = t / nref;
+    int ky = idx % E - H, kx = (idx / E) % E - H, kz = idx / (E * E) - H;
+    out[i] = b_series(kx, ky, kz, sigma + 3 * refs[u], mu_q, rho[r], L, gam, eta);
   }
 }
 
@@ -293,7 +317,7 @@ __global__ void k_expand_b(cplx* b, int pair, DevTables tab) {
     int z = i % N3; long t = i / N3; int s = t % tab.M, r = t / tab.M;
     int iz = z % N, iy = (z / N) % N, ix = z / (N * N);
     if (tab.full[pair]) {
-      b[i] = tab.bfull[pair][((size_t)r * tab.M + s) * N3 + ((size_t)iz * N + ix) * N + iy];
+      b[i] = bfull_at(tab, pair, r, s, signed_freq(ix, N), signed_freq(iy, N), signed_freq(iz, N));
     } else {
       int kx = signed_freq(ix, N), ky = signed_freq(iy, N), kz = signed_freq(iz, N);
       b[i] = make_double2(tab.bvhs[((size_t)pair * tab.N_rho + r) * tab.K2n + kx * kx + ky * ky + kz * kz], 0.0);
@@ -381,13 +405,62 @@ int build_tables(dgfs_ctx* c) {
   if (c->table_mode == 0)
     k_closs0<<<blocks((long)np * N3), TB>>>(c->d_closs, ns, N, Nr, c->L, d_gam, d_eta, c->d_rho, c->d_w_rho);
 
+  // Full tables (VSS pairs, table_mode 1).  table_mode 0: b_rs(k) depends on k through |k| and k . sigma_s only, so
+  // sphere points that are signed axis permutations of one another share one table on the extended grid (bfull_at in
+  // ctx.h).  DGFS_BTABLE=full keeps [r][s][N^3] (the paper's layout).
+  c->bsym = 0; c->nref = 0; c->bref.clear(); c->bmap.assign(M, make_int4(0, 0, 0, 0));
+  if (c->any_full && c->table_mode == 0) {
+    const char* bt = getenv("DGFS_BTABLE");
+    const int E = N + 1, H = N / 2;
+    const int S3[3] = {E, 1, E * E};                                   // stride of the x, y, z index ([kz][kx][ky])
+    // only the permutations that keep y in place: the consumers' lanes run along ky, and with ky mapped to another
+    // axis of the reference table every lane of a load would touch its own 128-byte line (measured on config c3:
+    // k_zfwd_full 3.2x slower with the full group of 48, whose one orbit would store the icosahedron 12x smaller)
+    static const int perms[2][3] = {{0, 1, 2}, {2, 1, 0}};
+    for (int s2 = 0; s2 < M; ++s2) {
+      bool found = false;
+      for (int u = 0; u < (int)c->bref.size() && !found; ++u) {
+        const double* su = &c->sigma[3 * c->bref[u]];
+        for (int pi_ = 0; pi_ < 2 && !found; ++pi_) {
+          int eps[3]; bool ok = true;
+          for (int d = 0; d < 3 && ok; ++d) {                          // sigma_s[d] = eps_d sigma_u[perm(d)]
+            const double a = c->sigma[3 * s2 + d], b = su[perms[pi_][d]];
+            if (fabs(a - b) <= 1e-15) eps[d] = 1;
+            else if (fabs(a + b) <= 1e-15) eps[d] = -1;
+            else ok = false;
+          }
+          if (!ok) continue;
+          // k . sigma_s = k' . sigma_u with k'_{perm(d)} = eps_d k_d
+          c->bmap[s2] = make_int4(u * E * E * E + H * (E * E + E + 1), eps[0] * S3[perms[pi_][0]],
+                                  eps[1] * S3[perms[pi_][1]], eps[2] * S3[perms[pi_][2]]);
+          found = true;
+        }
+      }
+      if (!found) {
+        c->bmap[s2] = make_int4((int)c->bref.size() * E * E * E + H * (E * E + E + 1), S3[0], S3[1], S3[2]);
+        c->bref.push_back(s2);
+      }
+    }
+    c->nref = (int)c->bref.size();
+    c->bsym = !(bt && std::string(bt) == "full") && (size_t)c->nref * E * E * E < (size_t)M * N3;
+    if (c->bsym) {
+      if ((rc = dev_upload(c, &c->d_bref, c->bref.data(), c->bref.size(), "upload reference points"))) return rc;
+      if ((rc = dev_upload(c, &c->d_bmap, c->bmap.data(), c->bmap.size(), "upload table maps"))) return rc;
+    }
+  }
   c->h_bfull.assign(np, nullptr);
+  c->table_bytes = 0;
   for (int pair = 0; pair < np; ++pair) {
     int p = pair / ns, q = pair % ns;
     if (c->full[pair]) {
-      size_t n = (size_t)Nr * M * N3;
+      const size_t E3 = (size_t)(N + 1) * (N + 1) * (N + 1);
+      size_t n = c->bsym ? (size_t)Nr * c->nref * E3 : (size_t)Nr * M * N3;
       if ((rc = check_cuda(c, cudaMalloc((void**)&c->h_bfull[pair], n * sizeof(cplx)), "alloc full b table"))) return rc;
-      if (c->table_mode == 0)
+      c->table_bytes += n * sizeof(cplx);
+      if (c->bsym)
+        k_bsym_series<<<blocks(n), 128>>>(c->h_bfull[pair], p, q, N, Nr, c->nref, c->d_bref, c->L, d_mass, c->gam[pair],
+                                          c->eta[pair], c->d_rho, c->d_sigma);
+      else if (c->table_mode == 0)
         k_bfull_series<<<blocks(n), 128>>>(c->h_bfull[pair], p, q, N, Nr, M, c->L, d_mass, c->gam[pair], c->eta[pair],
                                            c->d_rho, c->d_sigma);
       else
@@ -407,6 +480,7 @@ int build_tables(dgfs_ctx* c) {
   t.ns = ns; t.npairs = np; t.N = N; t.N3 = N3; t.N_rho = Nr; t.M = M; t.K2n = c->K2n;
   t.phase = c->d_phase; t.bvhs = c->d_bvhs; t.bfull = c->d_bfull; t.closs = c->d_closs;
   t.w_rho = c->d_w_rho; t.beta = c->d_beta; t.full = c->d_full; t.sskip = c->d_v0_sskip; t.tsrc = c->d_v0_tsrc;
+  t.bsym = c->bsym; t.nref = c->nref; t.bmap = c->d_bmap;
   return DGFS_OK;
 }
 
@@ -432,6 +506,7 @@ extern "C" int dgfs_create(const dgfs_params* P, dgfs_ctx** out) {
   if ((P->sigma == nullptr) != (P->w_sigma == nullptr))
     return set_error(nullptr, DGFS_EINVAL, "dgfs_create: sigma and w_sigma must both be given or both be NULL");
   if (P->table_mode != 0 && P->table_mode != 1) return set_error(nullptr, DGFS_EINVAL, "dgfs_create: table_mode must be 0 or 1");
+  if (P->precision != 0 && P->precision != 1) return set_error(nullptr, DGFS_EINVAL, "dgfs_create: precision must be 0 (fp64) or 1 (fp32 inner loop)");
   if (P->table_mode == 1 && (P->M_pre < 1 || !P->sigma_pre || !P->w_pre))
     return set_error(nullptr, DGFS_EINVAL, "dgfs_create: table_mode 1 needs M_pre >= 1, sigma_pre and w_pre");
   const int ns = P->ns, np = ns * ns;
@@ -468,6 +543,7 @@ extern "C" int dgfs_create(const dgfs_params* P, dgfs_ctx** out) {
   c->device = P->device; c->ns = ns; c->npairs = np; c->N = N; c->N3 = N * N * N; c->N_rho = P->N_rho; c->M = P->M;
   c->L = P->L; c->table_mode = P->table_mode;
   c->nyq_filter = P->nyquist_filter != 0;
+  c->precision = P->precision;
   c->K2n = 3 * (N / 2) * (N / 2) + 1;
   c->mass.assign(P->mass, P->mass + ns);
   c->omega.assign(P->omega, P->omega + np);
@@ -509,6 +585,11 @@ extern "C" int dgfs_create(const dgfs_params* P, dgfs_ctx** out) {
   // stage-per-kernel pipeline (N = 48 always runs it; the parity tests cover both)
   const char* pipe = getenv("DGFS_PIPELINE");
   c->use_v1 = N <= 32 && !(pipe && std::string(pipe) == "v0");
+  if (c->precision == 1 && (!c->use_v1 || c->any_full)) {
+    g_create_error = "dgfs_create: precision 1 is implemented for VHS pairs (alpha = 1, table_mode 0) with N <= 32 on the default pipeline";
+    dgfs_destroy(c);
+    return DGFS_ENOSUP;
+  }
   if (c->use_v1) {
     const char* ch = getenv("DGFS_V1_CHUNK");
     if (ch && atoi(ch) > 0) c->v1_chunk = atoi(ch);
@@ -531,7 +612,7 @@ extern "C" void dgfs_destroy(dgfs_ctx* c) {
   cudaSetDevice(c->device);
   cudaFree(c->d_phase); cudaFree(c->d_bvhs); cudaFree(c->d_closs); cudaFree(c->d_w_rho); cudaFree(c->d_beta);
   cudaFree(c->d_rho); cudaFree(c->d_sigma); cudaFree(c->d_full); cudaFree(c->d_bfull);
-  cudaFree(c->d_v0_sskip); cudaFree(c->d_v0_tsrc); cudaFree(c->d_v0_wfac);
+  cudaFree(c->d_v0_sskip); cudaFree(c->d_v0_tsrc); cudaFree(c->d_v0_wfac); cudaFree(c->d_bref); cudaFree(c->d_bmap);
   for (auto p : c->h_bfull) cudaFree(p);
   cudaFree(c->ws); cudaFree(c->dg_ws);
   free_tables_v1(c);
@@ -546,6 +627,8 @@ extern "C" void dgfs_destroy(dgfs_ctx* c) {
   for (auto e : c->prof.pool) cudaEventDestroy(e);
   delete c;
 }
+
+extern "C" size_t dgfs_table_bytes(const dgfs_ctx* c) { return c ? c->table_bytes : 0; }
 
 extern "C" int dgfs_get_quadrature(const dgfs_ctx* c, double* R, double* rho, double* w_rho, double* sigma,
                                    double* w_sigma, double* beta) {

@@ -22,7 +22,9 @@ struct DevTables {
   // b^(pq)_r(|k|^2) for pairs whose b does not depend on s (VHS, table_mode 0; Eq. 16)
   const double* bvhs;           // [pair][r][K2n]
   // full b^(pq)_rs(k) in SPEC layout for the other pairs (VSS or table_mode 1), else nullptr
-  const cplx* const* bfull;     // [pair] -> [r][s][N3]
+  const cplx* const* bfull;     // [pair] -> [r][s][N3], or (bsym) [r][nref][(N+1)^3]: see bfull_at below
+  int bsym, nref;               // symmetry-compressed full tables: reference sphere points only, extended grid
+  const int4* bmap;             // [s] {offset, stride of kx, of ky, of kz} into the reference tables (signed frequencies)
   const cplx* closs;            // [pair][N3]  c^(pq)(k), SPEC layout (Eq. 17)
   const double* w_rho;          // [N_rho]
   const double* beta;           // [pair]      beta_pq (Eq. 6)
@@ -31,6 +33,36 @@ struct DevTables {
   const unsigned char* sskip;   // [pair][s]
   const int* tsrc;              // [pair]
 };
+
+// b^(pq)_rs(k) of a pair with a full table, at SIGNED frequencies (kx, ky, kz) in [-N/2, N/2).
+// bsym: b_rs(k) = F_r(|k|, k . sigma_s) (Eq. 16), so for sigma_s = G sigma_u with G a signed permutation of the
+// axes, b_rs(k) = b_ru(G^T k): only the reference points u are stored, on the extended grid [-N/2, N/2]^3 (G^T may flip
+// the sign of the Nyquist index), and the index of G^T k is linear in (kx, ky, kz): bmap[s].  G ranges over the sign
+// flips and the x <-> z swap (ky stays the fastest index, loads stay coalesced): 3 tables for the 12 points of the
+// icosahedron, 7 for the 32-point rule: 2.7 GB -> 0.63 GB per pair at (48, 48, 32).
+// Written without branches (both index forms are a few integer operations; the load is unconditional).
+__device__ __forceinline__ size_t bfull_index(const DevTables& tab, int r, int s, int kx, int ky, int kz) {
+  const int N = tab.N;
+  const int4 m = tab.bsym ? tab.bmap[s] : make_int4(0, 0, 0, 0);
+  const size_t E = N + 1;
+  const int ix = kx < 0 ? kx + N : kx, iy = ky < 0 ? ky + N : ky, iz = kz < 0 ? kz + N : kz;
+  const size_t isym = (size_t)r * tab.nref * (E * E * E) + (size_t)(m.x + kx * m.y + ky * m.z + kz * m.w);
+  const size_t ifull = ((size_t)r * tab.M + s) * tab.N3 + ((size_t)iz * N + ix) * N + iy;
+  return tab.bsym ? isym : ifull;
+}
+__device__ __forceinline__ cplx bfull_at(const DevTables& tab, int pair, int r, int s, int kx, int ky, int kz) {
+  return tab.bfull[pair][bfull_index(tab, r, s, kx, ky, kz)];
+}
+// The same for a sweep over kz at fixed (kx, ky): pointer to the element of kz = 0 and the stride (in elements) per
+// unit of the index zi = kz (signed, bsym) or iz = kz mod N (full layout).
+struct BSweep { const cplx* p; long sz; };
+__device__ __forceinline__ BSweep bfull_sweep(const DevTables& tab, int pair, int r, int s, int kx, int ky) {
+  const int4 m = tab.bsym ? tab.bmap[s] : make_int4(0, 0, 0, 0);
+  BSweep b;
+  b.p = tab.bfull[pair] + bfull_index(tab, r, s, kx, ky, 0);
+  b.sz = tab.bsym ? (long)m.w : (long)tab.N * tab.N;
+  return b;
+}
 
 }  // namespace dgfs
 
@@ -86,6 +118,7 @@ struct dgfs_ctx {
   double L = 0, R = 0;
   int table_mode = 0;
   bool nyq_filter = false;               // dgfs_params::nyquist_filter
+  int precision = 0;                     // dgfs_params::precision
   bool any_full = false;
   std::vector<double> mass, omega, alpha, kn, beta, gam, eta, rho, w_rho, sigma, w_sigma;
   std::vector<double> sigma_pre, w_pre;
@@ -95,6 +128,12 @@ struct dgfs_ctx {
   dgfs::cplx* d_phase = nullptr;
   double* d_bvhs = nullptr;
   std::vector<dgfs::cplx*> h_bfull;      // device pointers, one per pair (or nullptr)
+  int bsym = 0, nref = 0;                // symmetry-compressed full tables (DevTables::bsym)
+  std::vector<int> bref;                 // [nref] sphere point each reference table belongs to
+  std::vector<int4> bmap;                // [M]
+  int* d_bref = nullptr;
+  int4* d_bmap = nullptr;
+  size_t table_bytes = 0;                // device bytes of the b tables (reported by dgfs_table_bytes)
   dgfs::cplx** d_bfull = nullptr;
   dgfs::cplx* d_closs = nullptr;
   double* d_w_rho = nullptr;
@@ -123,6 +162,7 @@ struct dgfs_ctx {
   int *d_v1_zsp = nullptr, *d_v1_zmap = nullptr, *d_v1_tsrc = nullptr, *d_v1_fsrc_s = nullptr, *d_v1_anti = nullptr, *d_v1_tpartner = nullptr;
   double* d_v1_fscale = nullptr;
   dgfs::cplx *d_v1_hz = nullptr, *d_v1_hxy = nullptr;
+  dgfs::cplxf* d_v1_hxyf = nullptr;      // precision 1: single-precision copy of the x, y factors
   double *d_v1_szv = nullptr, *d_v1_sxy = nullptr;
   std::vector<unsigned char> v1_smask, v1_sskip;
   unsigned char *d_v1_smask = nullptr, *d_v1_sskip = nullptr;

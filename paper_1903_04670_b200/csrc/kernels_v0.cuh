@@ -88,7 +88,6 @@ __global__ void __launch_bounds__(32 * W) k_plane_fwd(DevTables tab, const cplx*
     const int sitem = (MODE == 1 && !full) ? item - pair + tab.tsrc[pair] : item;
     const cplx* in = T + ((size_t)sitem * Tslices + sl) * N3 + (size_t)kz * N2;
     const double* bv = tab.bvhs + ((size_t)pair * tab.N_rho + r) * tab.K2n;
-    const cplx* bf = (MODE == 1 && full) ? tab.bfull[pair] + ((size_t)r * tab.M + sl) * N3 + (size_t)kz * N2 : nullptr;
     warp_plane_fft<N, -1>(
         buf, lane, [&](int cy, int cx) { return in[cy * N + cx]; }, [](cplx x, int) { return x; },
         [&](int kx, int ky, cplx val) {
@@ -98,7 +97,7 @@ __global__ void __launch_bounds__(32 * W) k_plane_fwd(DevTables tab, const cplx*
           } else {
             cplx acc = o[idx];
             if (full) {
-              cplx b = bf[idx];
+              cplx b = bfull_at(tab, pair, r, sl, sfreq(kx, N), sfreq(ky, N), kzs);
               acc.x += scale * (b.x * val.x - b.y * val.y);
               acc.y += scale * (b.x * val.y + b.y * val.x);
             } else {

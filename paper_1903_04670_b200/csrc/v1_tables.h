@@ -18,6 +18,7 @@ struct V1Tables {
   const cplx* hz;            // [r][nz][N]           Hermitian-preserving z factor (1/N folded)
   const double* szv;         // [r][nz]              anti-Hermitian z scalar (1/N folded)
   const cplx* hxy;           // [pair][r][s][side][2][N]   x factors then y factors
+  const cplxf* hxyf;         // the same in single precision (dgfs_params::precision = 1), else nullptr
   const double* sxy;         // [pair][r][s][side][2]      anti-Hermitian x, y scalars
   const int* tsrc;           // [pair]  pair whose S_r (buffer T) this pair uses: itself, or its transpose (q,p) -> (p,q) (R-11)
   const int* anti;           // [s]     antipode of sphere point s, or -1

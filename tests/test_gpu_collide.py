@@ -354,3 +354,92 @@ def test_fp64_peak_probe_is_plausible(torch_cuda):
     from paper_1903_04670_b200 import dgfs_measure_fp64_peak
     burst, sustained = dgfs_measure_fp64_peak(0, 0.2)
     assert 5.0 < sustained <= burst < 60.0
+
+
+# ------------------------------------------------------------------ symmetry-compressed full b tables
+@pytest.mark.parametrize("N,M,pipeline", [(8, 12, "v1"), (8, 32, "v1"), (16, 12, "v0"), (24, 12, "v1")])
+def test_full_b_tables_stored_per_orbit_of_the_sphere_rule(torch_cuda, monkeypatch, N, M, pipeline):
+    """b_rs(k) of a VSS pair depends on k through |k| and k . sigma_s only (Eq. 16), so the
+    library stores one table per orbit of the sphere rule under the signed axis permutations that keep y in place
+    (icosahedron: 3 of 12, 32-point rule: 7 of 32) on the extended grid.  Same table values as the oracle's _b_exact (1e-13), same Q as the
+    paper's layout [N_rho][M][N^3] (DGFS_BTABLE=full) and as the oracle (1e-10), a fraction of the bytes."""
+    torch = torch_cuda
+    from oracle.collide import collide_pairs
+    if pipeline == "v0":
+        monkeypatch.setenv("DGFS_PIPELINE", "v0")
+    from oracle.quadrature import sphere_rule
+    cfg = _rand_cfg("t", 2, N, 2, M, (1.2, 1.45), (0.6, 0.8), (1.0, 2.0), seed=21)
+    f = make_points(cfg, range(2))
+    sig, wsig = sphere_rule(M)          # the same sphere points in the same order on both sides (inputs, not results)
+    tab = _oracle_tables(cfg, sigma=sig, w_sigma=wsig)
+    Qo = collide_pairs(tab, f)
+    res = {}
+    for mode in ("sym", "full"):
+        monkeypatch.setenv("DGFS_BTABLE", mode)
+        with _gpu_op(cfg, sigma=sig, w_sigma=wsig) as op:
+            Q = op.collide_pairs(torch.from_numpy(f).cuda()).cpu().numpy()
+            b01 = op.tables(0, 1)[1]
+            res[mode] = (Q, b01, op.table_bytes())
+        assert _pair_errs(Q, Qo).max() < TOL, mode
+        assert np.max(np.abs(b01 - tab.b[0, 1])) < 1e-13 * np.max(np.abs(tab.b[0, 1])), mode
+    orbits = {12: 3, 32: 7}[M]        # orbits under sign flips and the x <-> z swap (the ky index stays the fastest)
+    assert res["full"][2] == 4 * cfg.N_rho * M * N ** 3 * 16
+    assert res["sym"][2] == 4 * cfg.N_rho * orbits * (N + 1) ** 3 * 16
+    assert _pair_errs(res["sym"][0], res["full"][0]).max() < 1e-12
+
+
+def test_full_b_tables_of_a_rule_without_symmetry_stay_in_full(torch_cuda):
+    """A rotated sphere rule has no two points related by a signed axis permutation: nothing to share."""
+    torch = torch_cuda
+    from oracle.quadrature import sphere_rule
+    from oracle.collide import collide_pairs
+    sig, w = sphere_rule(12)
+    th = 0.3
+    Rz = np.array([[np.cos(th), -np.sin(th), 0], [np.sin(th), np.cos(th), 0], [0, 0, 1.0]])
+    Rx = np.array([[1.0, 0, 0], [0, np.cos(0.7), -np.sin(0.7)], [0, np.sin(0.7), np.cos(0.7)]])
+    sig = sig @ (Rz @ Rx).T
+    sig /= np.linalg.norm(sig, axis=1)[:, None]
+    cfg = _rand_cfg("t", 2, 8, 2, 12, (1.3, 1.3), (0.6, 0.8), (1.0, 2.0), seed=22)
+    f = make_points(cfg, range(2))
+    Qo = collide_pairs(_oracle_tables(cfg, sigma=sig, w_sigma=w), f)
+    with _gpu_op(cfg, sigma=sig, w_sigma=w) as op:
+        Q = op.collide_pairs(torch.from_numpy(f).cuda()).cpu().numpy()
+        assert op.table_bytes() >= 4 * cfg.N_rho * 6 * 8 ** 3 * 16      # antipodes may still pair up, nothing more
+    assert _pair_errs(Q, Qo).max() < TOL
+
+
+# ------------------------------------------------------------------ dgfs_params.precision = 1 (fp32 inner loop)
+@pytest.mark.parametrize("N,N_rho,M", [(8, 4, 6), (16, 3, 12), (24, 3, 12), (32, 3, 12), (32, 2, 32)])
+def test_precision_1_within_1e_4_on_non_equilibrium_inputs(torch_cuda, N, N_rho, M):
+    """SURVEY 8(f) item 1 / north_star "1e-4 if an fp32 mode is offered": steps 4-6 of Algorithm 2 in fp32, the rest in
+    fp64, against the SAME fp64 oracle at 1e-4 of max|Q| per (point, pair) array on bi-Maxwellian inputs."""
+    torch = torch_cuda
+    from oracle.collide import collide_pairs
+    from oracle_pool import record
+    cfg = _rand_cfg("t", 2, N, N_rho, M, (1.0, 1.0), (0.6, 0.8), (1.0, 2.0), seed=31)
+    f = make_points(cfg, range(3))
+    Qo = collide_pairs(_oracle_tables(cfg), f)
+    with _gpu_op(cfg, precision=1) as op:
+        fd = torch.from_numpy(f).cuda()
+        Qg = op.collide_pairs(fd).cpu().numpy()
+        Qs = op.collide(fd).cpu().numpy()
+    err = _pair_errs(Qg, Qo).max()
+    record("fp32", "N=%d N_rho=%d M=%d, bi-Maxwellian inputs, all pairs" % (N, N_rho, M), err, 1e-4)
+    assert err < 1e-4
+    Qos = Qo.sum(axis=2)
+    assert (np.max(np.abs(Qs - Qos), axis=-1) / np.max(np.abs(Qos), axis=-1)).max() < 1e-4
+
+
+def test_precision_1_is_refused_where_it_is_not_implemented(torch_cuda):
+    from paper_1903_04670_b200 import api
+    vss = _rand_cfg("t", 2, 8, 2, 6, (1.0, 1.3), (0.6, 0.8), (1.0, 2.0), seed=1)
+    with pytest.raises(api.DgfsError) as e:
+        _gpu_op(vss, precision=1)
+    assert e.value.code == api.DGFS_ENOSUP
+    big = _rand_cfg("t", 2, 48, 1, 6, (1.0, 1.0), (0.6, 0.8), (1.0, 2.0), seed=1)
+    with pytest.raises(api.DgfsError) as e:
+        _gpu_op(big, precision=1)
+    assert e.value.code == api.DGFS_ENOSUP
+    with pytest.raises(api.DgfsError) as e:
+        _gpu_op(vss, precision=2)
+    assert e.value.code == api.DGFS_EINVAL
