@@ -330,7 +330,7 @@ __device__ __forceinline__ void fence_mbar_init() { asm volatile("fence.mbarrier
 // in: fhh[xl][species][lz][lx][m];  out: Gz[xl][k - kbase][cz][lx][m], kstride arrays per point (the jobs that depend
 // on the radial node and the sigma_z = 0 jobs, which do not, live in separate buffers: GzView below).
 template <int N, class CO>
-__global__ void __launch_bounds__(128, 3) k_zshift(V1Tables t, int ns, const cplx* __restrict__ fhh, CO* __restrict__ Gz, int r, int k0, int nk,
+__global__ void __launch_bounds__(128, N > 32 ? 2 : 3) k_zshift(V1Tables t, int ns, const cplx* __restrict__ fhh, CO* __restrict__ Gz, int r, int k0, int nk,
                                                    int kbase, int kstride) {
   constexpr int H = N / 2, NP = N * H;
   extern __shared__ cplx sm[];                       // [lz][128]
@@ -939,12 +939,12 @@ __global__ void __launch_bounds__(256) k_zfwd_full(DevTables tab, V1Tables t, co
 // XOR-swizzled by (cx / 2) mod 8 (v1_tables.h), so that the 8 lanes of a 128-bit wavefront read 8 different banks.
 template <int N>
 struct WtermSmem {
-  static constexpr int CYB = 8, THREADS = 256;
+  static constexpr int CYB = 8, THREADS = (N / 2) * (N / 2);    // thread = 2 x 2 tile of (cx, cz)
   static constexpr int Y = 0;                       // [cx][cz ^ swz(cx)]      the uy plane
   static constexpr int Z = N * N;                   // [i][parity][H]          uz rows of the slab
   static constexpr int U = N * N + CYB * N;         // [i][cz]                 ux' rows of the slab
   static constexpr int WORDS = N * N + 2 * CYB * N;
-  static constexpr int STAGES = 4;                  // ring depth (two blocks per SM: 8 stages in flight per SM)
+  static constexpr int STAGES = N > 32 ? 2 : 4;     // ring depth (N = 32: two blocks per SM, 8 stages in flight per SM)
 };
 
 // Arithmetic of one s for the thread's 2 x 2 x 8 nodes (cx = 2 tx + a, cz = 2 tz + b, cy = cy0 + i).  MASK bit d set:
@@ -986,7 +986,7 @@ __device__ __forceinline__ void wterm_rows(const cplx* __restrict__ b_, int tx, 
 }
 
 template <int N>
-__global__ void __launch_bounds__(WtermSmem<N>::THREADS, 2) k_wterm(const cplx* __restrict__ nyq, int M, double* __restrict__ S, const unsigned char* __restrict__ full, int npairs,
+__global__ void __launch_bounds__(WtermSmem<N>::THREADS, N > 32 ? 1 : 2) k_wterm(const cplx* __restrict__ nyq, int M, double* __restrict__ S, const unsigned char* __restrict__ full, int npairs,
         const unsigned char* __restrict__ smask, const unsigned char* __restrict__ sskip, const int* __restrict__ tsrc) {
   constexpr int N2 = N * N, N3 = N2 * N, H = N / 2;
   typedef NyqLayout<N> NL;
@@ -995,8 +995,8 @@ __global__ void __launch_bounds__(WtermSmem<N>::THREADS, 2) k_wterm(const cplx* 
   extern __shared__ cplx sm[];
   // pairs with a full b table take k_xy_full, transposed pairs reuse the other's S_r (uniform per block)
   if (full[blockIdx.y % npairs] || tsrc[blockIdx.y % npairs] != (int)(blockIdx.y % npairs)) return;
-  const int tx = threadIdx.x % 16, tz = threadIdx.x / 16;
-  const bool act = tx < H && tz < H;
+  const int tx = threadIdx.x % H, tz = threadIdx.x / H;
+  const bool act = true;
   const int cy0 = blockIdx.x * CYB;
   const cplx* nbase = nyq + (size_t)blockIdx.y * M * NL::STRIDE;
   const unsigned char* skip = sskip + (size_t)(blockIdx.y % npairs) * M;
@@ -1172,6 +1172,10 @@ __global__ void __launch_bounds__(64) k_final_xy_h(DevTables tab, const cplx* __
       },
       [](cplx x, int) { return x; }, [&](int cy, int cx, cplx val) { o[cy * N + cx] = val; });
 }
+
+}  // namespace dgfs
+#include "collide_v1_wide.cuh"
+namespace dgfs {
 
 // ---------------------------------------------------------------- host orchestration ------------
 namespace {
@@ -1368,16 +1372,22 @@ static int collide_v1_impl(dgfs_ctx* c, const double* f, double* out, int nx, bo
   const size_t smem_nyq = sizeof(cplx) * (size_t)2 * JobSmem<N>::WORDS;
   const size_t smem_zacc = sizeof(cplx) * (size_t)ZaccSmem<N>::STAGES * ZaccSmem<N>::WORDS;
   const size_t smem_zs = sizeof(cplx) * (size_t)N * 128;
+  const size_t smem_wide = sizeof(cplx) * (size_t)JobSmem<N>::WORDS;      // one job per block of 64 threads (N > 32)
   if (!c->v1_attr_done) {                 // per context, hence per device
     cudaFuncSetAttribute(k_plane_fwd<N, W, 0>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_plane);
     cudaFuncSetAttribute(k_plane_fwd<N, W, 1>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_plane);
     cudaFuncSetAttribute(k_final_xy_h<N>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_final);
-    cudaFuncSetAttribute(k_xy<N, W, cplx>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_xy);
-    cudaFuncSetAttribute(k_xy<N, W, cplxf>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_xy / 2);
-    cudaFuncSetAttribute(k_xy<N, 2, cplx>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_xy / 2);
-    cudaFuncSetAttribute(k_xy_full<N, W>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_xyf);
+    if constexpr (N <= 32) {
+      cudaFuncSetAttribute(k_xy<N, W, cplx>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_xy);
+      cudaFuncSetAttribute(k_xy<N, W, cplxf>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_xy / 2);
+      cudaFuncSetAttribute(k_xy<N, 2, cplx>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_xy / 2);
+      cudaFuncSetAttribute(k_xy_full<N, W>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_xyf);
+      cudaFuncSetAttribute(k_nyq2<N, 2>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_nyq);
+    } else {
+      cudaFuncSetAttribute(k_xy_wide<N>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)(2 * smem_wide));
+      cudaFuncSetAttribute(k_nyq2_wide<N>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_wide);
+    }
     cudaFuncSetAttribute(k_wterm<N>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_wt);
-    cudaFuncSetAttribute(k_nyq2<N, 2>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_nyq);
     cudaFuncSetAttribute(k_zshift<N, cplx>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_zs);
     cudaFuncSetAttribute(k_zshift<N, cplxf>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_zs);
     cudaFuncSetAttribute(k_zfwd_acc<N, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_zacc);
@@ -1435,7 +1445,8 @@ static int collide_v1_impl(dgfs_ctx* c, const double* f, double* out, int nx, bo
       { ProfScope ps(c->prof, sa, "k_nyq1d", nb * run_all * c->M * 16.0 * N2);
         k_nyq1d<N><<<(items * c->M + 3) / 4, 128, 0, sa>>>(c->v1, c->tab, fhat, nyqb[b], r, items * c->M); }
       { ProfScope ps(c->prof, sa, "k_nyq2", nb * run_all * (fl.nyq - c->M * 16.0 * N2));
-        k_nyq2<N, 2><<<dim3(3, items), 64, smem_nyq, sa>>>(c->v1, c->tab, fhh, nyqy, nyqb[b], r); }
+        if constexpr (N <= 32) k_nyq2<N, 2><<<dim3(3, items), 64, smem_nyq, sa>>>(c->v1, c->tab, fhh, nyqy, nyqb[b], r);
+        else k_nyq2_wide<N><<<dim3(3, items), 64, smem_wide, sa>>>(c->v1, c->tab, fhh, nyqy, nyqb[b], r); }
       if (nvhs > 0)
         { ProfScope ps(c->prof, sa, "k_wterm", nb * run_vhs * fl.wterm);
           k_wterm<N><<<dim3(N / WtermSmem<N>::CYB, items), WtermSmem<N>::THREADS, smem_wt, sa>>>(nyqb[b], c->M, Sb[b], c->tab.full, np, c->v1.smask, c->v1.sskip, c->v1.tsrc); }
@@ -1448,7 +1459,9 @@ static int collide_v1_impl(dgfs_ctx* c, const double* f, double* out, int nx, bo
         const int g = r / RG, slot = r % pl.tslots;
         if (r % RG == 0 && g >= 2) wait(st, c->ev_acc[g & 1]);       // the forward z pass of group g - 2 has read these slots
         { ProfScope ps(c->prof, st, "k_xy", nb * (run_vhs * (fl.xy - fwd_xy) + nrun_vhs * fwd_xy));
-          if (f32) {                // dgfs_params::precision = 1
+          if constexpr (N > 32) {
+            k_xy_wide<N><<<dim3(N / 2, items), 2 * N, 2 * smem_wide, st>>>(c->v1, c->tab, gv, c->v1.hxy, nyqb[b], Sb[b], T + (size_t)slot * slot_stride, r);
+          } else if (f32) {         // dgfs_params::precision = 1
             const GzViewT<cplxf> gvf{(const cplxf*)GzR[b], (const cplxf*)Gz0, nzr, nz0};
             k_xy<N, W, cplxf><<<dim3((N + W - 1) / W, items), 32 * W, smem_xy / 2, st>>>(c->v1, c->tab, gvf, c->v1.hxyf, nyqb[b], Sb[b], T + (size_t)slot * slot_stride, r);
           } else if (c->v1_xyw == 2)       // DGFS_V1_XYW=2: blocks of two warps, five per SM (ten warps at <= 200 registers)
@@ -1456,7 +1469,7 @@ static int collide_v1_impl(dgfs_ctx* c, const double* f, double* out, int nx, bo
           else
             k_xy<N, W, cplx><<<dim3((N + W - 1) / W, items), 32 * W, smem_xy, st>>>(c->v1, c->tab, gv, c->v1.hxy, nyqb[b], Sb[b], T + (size_t)slot * slot_stride, r); }
       }
-      if (nfull > 0) {
+      if constexpr (N <= 32) if (nfull > 0) {
         { ProfScope ps(c->prof, st, "k_xy_full", nb * (run_all - run_vhs) * fl.xy_full);
           k_xy_full<N, W><<<dim3((N + W - 1) / W, items), 32 * W, smem_xyf, st>>>(c->v1, c->tab, gv, nyqb[b], Tf, r); }
         { ProfScope ps(c->prof, st, "k_zfwd_full", nb * nfull * fl.acc_full);
@@ -1497,6 +1510,7 @@ int run_collide_v1(dgfs_ctx* c, const double* f, double* out, int nx, bool pairs
     case 16: return collide_v1_impl<16>(c, f, out, nx, pairs_out, st);
     case 24: return collide_v1_impl<24>(c, f, out, nx, pairs_out, st);
     case 32: return collide_v1_impl<32>(c, f, out, nx, pairs_out, st);
+    case 48: return collide_v1_impl<48>(c, f, out, nx, pairs_out, st);      // VHS pairs only (collide_v1_wide.cuh)
   }
   return set_error(c, DGFS_ENOSUP, "v1 pipeline: unsupported N");
 }

@@ -581,17 +581,18 @@ extern "C" int dgfs_create(const dgfs_params* P, dgfs_ctx** out) {
   c->scratch_budget = (size_t)(env ? atol(env) : 3072) << 20;
   int rc = build_tables(c);
   if (rc != DGFS_OK) { g_create_error = c->err; dgfs_destroy(c); return rc; }
-  // pipeline choice: v1 (collide_v1.cu) needs one lane per pencil (N <= 32); DGFS_PIPELINE=v0 forces the
-  // stage-per-kernel pipeline (N = 48 always runs it; the parity tests cover both)
+  // DGFS_PIPELINE=v0 forces the stage-per-kernel pipeline (the parity tests cover both)
   const char* pipe = getenv("DGFS_PIPELINE");
-  c->use_v1 = N <= 32 && !(pipe && std::string(pipe) == "v0");
-  if (c->precision == 1 && (!c->use_v1 || c->any_full)) {
+  // pipeline choice: v1 (collide_v1.cu): N <= 32, or N = 48 when no pair needs a full b table (collide_v1_wide.cuh)
+  c->use_v1 = (N <= 32 || !c->any_full) && !(pipe && std::string(pipe) == "v0");
+  if (c->precision == 1 && (!c->use_v1 || c->any_full || N > 32)) {
     g_create_error = "dgfs_create: precision 1 is implemented for VHS pairs (alpha = 1, table_mode 0) with N <= 32 on the default pipeline";
     dgfs_destroy(c);
     return DGFS_ENOSUP;
   }
   if (c->use_v1) {
     const char* ch = getenv("DGFS_V1_CHUNK");
+    if (N > 32) c->v1_chunk = 256;                  // 1.7 MB arrays: half the points per launch group for the same workspace
     if (ch && atoi(ch) > 0) c->v1_chunk = atoi(ch);
     const char* rg = getenv("DGFS_V1_RGROUP");
     if (rg && atoi(rg) > 0) c->v1_rgroup = atoi(rg);

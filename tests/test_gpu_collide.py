@@ -78,7 +78,8 @@ def test_small_radial_rule_every_N(torch_cuda, N, N_rho, M, ns, alpha):
 
 
 @pytest.mark.parametrize("N,N_rho,M,ns", [(8, 3, 6, 2), (16, 2, 12, 2), (32, 2, 12, 2),
-                                          (8, 2, 32, 2)])      # weighted 32-point rule: R-10 weight folding (v0_wfac)
+                                          (8, 2, 32, 2),       # weighted 32-point rule: R-10 weight folding (v0_wfac)
+                                          (48, 1, 12, 2)])     # N = 48 on the stage-per-kernel pipeline (VSS pairs use it)
 def test_v0_pipeline_on_vhs_pairs(torch_cuda, monkeypatch, N, N_rho, M, ns):
     """All-VHS configurations default to the v1 pipeline; DGFS_PIPELINE=v0 keeps the stage-per-kernel
     pipeline (the one VSS pairs and N = 48 use) covered on the same inputs."""
@@ -92,6 +93,8 @@ def test_v0_pipeline_on_vhs_pairs(torch_cuda, monkeypatch, N, N_rho, M, ns):
     (16, 2, 32, 1, 0.3),       # single species: sides A and B share their z shifts
     (32, 2, 6, 2, 0.3),        # octahedron: sigma with two zero components
     (32, 1, 32, 1, 0.3),       # more uz planes than k_wterm keeps resident in shared memory
+    (48, 2, 12, 2, 0.3),       # N = 48: the 64-thread plane job with split transforms (collide_v1_wide.cuh)
+    (48, 1, 32, 2, 0.3),       # ... with the weighted 32-point rule of config c4
 ])
 def test_v1_nyquist_terms(torch_cuda, N, N_rho, M, ns, noise):
     _small_radial_rule(torch_cuda, N, N_rho, M, ns, (1.0,) * ns, noise=noise)
