@@ -37,7 +37,7 @@ def parse():
     ap.add_argument("--steps", type=int, default=3)
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
-    ap.add_argument("--workload", default="c2", choices=["c0", "c1", "c2", "c3", "c4", "couette"])
+    ap.add_argument("--workload", default="c2", choices=["c0", "c1", "c2", "c3", "c4", "couette", "c4vss", "c2half"])
     ap.add_argument("--nx", type=int, default=0, help="override the batch size (debugging only; reported)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--precision", default="f64", choices=["f64", "f32"],
@@ -150,7 +150,7 @@ def oracle_sample(cfg, n_points, tab=None):
 
 def oracle_points(cfg):
     """Sample size giving roughly 10-30 s of CPU work per timing at 16 cores."""
-    return {"c0": 4, "c1": 32, "c2": 16, "c3": 16, "c4": 4, "couette": 16}[cfg.name]
+    return {"c0": 4, "c1": 32, "c2": 16, "c3": 16, "c4": 4, "couette": 16, "c4vss": 4, "c2half": 16}[cfg.name]
 
 
 def workload_desc(cfg, nx, ngpus, stages):

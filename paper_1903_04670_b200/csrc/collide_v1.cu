@@ -635,8 +635,11 @@ __global__ void __launch_bounds__(32 * NW) k_nyq2(V1Tables t, DevTables tab, con
 // C = double2: Algorithm 2 in fp64.  C = float2 (dgfs_params::precision = 1): the same job on single-precision copies
 // of the z-shifted arrays and factor tables; the Nyquist corrections and S are read in double and converted, T is
 // written in double (the forward z pass and everything after it stay fp64).
-template <int N, int W, class C>
-__global__ void __launch_bounds__(32 * W) __maxnreg__(sizeof(C) == 8 ? 128 : (W == 2 ? 200 : 255)) k_xy(V1Tables t, DevTables tab, GzViewT<C> Gz,
+// PACK (N < 32, e.g. N = 24): the W jobs of a block are dealt out N lanes each over its N W threads (W = 4, N = 24:
+// three full warps run four planes) instead of one job per warp with 32 - N lanes idle; the jobs of a block then walk
+// their common job list in step, with block barriers in place of warp barriers.
+template <int N, int W, class C, bool PACK = false>
+__global__ void __launch_bounds__(PACK ? N * W : 32 * W) __maxnreg__(sizeof(C) == 8 ? 128 : (W == 2 ? 200 : 255)) k_xy(V1Tables t, DevTables tab, GzViewT<C> Gz,
                                                const C* __restrict__ hxy, const cplx* __restrict__ nyq, const double* __restrict__ S,
                                                cplx* __restrict__ T, int r) {
   constexpr int H = N / 2, NH = N * H, N2 = N * N;
@@ -648,13 +651,15 @@ __global__ void __launch_bounds__(32 * W) __maxnreg__(sizeof(C) == 8 ? 128 : (W 
   static_assert(N <= 32, "one lane per pencil");
   extern __shared__ __align__(16) unsigned char sm_raw[];
   C* sm = reinterpret_cast<C*>(sm_raw);
-  const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+  const int warp = PACK ? threadIdx.x / N : threadIdx.x >> 5, lane = PACK ? threadIdx.x % N : threadIdx.x & 31;
   const int cz = blockIdx.x * W + warp, item = blockIdx.y;
   const int pair = item % tab.npairs, xl = item / tab.npairs;
+  static_assert(!PACK || N % W == 0, "PACK: every block runs W planes");
   if (cz >= N || tab.full[pair] || t.tsrc[pair] != pair) return;      // R-11: (q,p) uses the buffer of (p,q)
   C* buf = sm + (size_t)warp * JS::WORDS;
   const bool act = lane < N;
   const int ln = act ? lane : 0;
+  auto sync = [&]() { if (PACK) __syncthreads(); else __syncwarp(); };
   const int side = ln / H, m = ln % H;
   const R szs = (cz & 1) ? (R)-1 : (R)1;
   const R sxb = (ln & 1) ? (R)-1 : (R)1;
@@ -700,7 +705,7 @@ __global__ void __launch_bounds__(32 * W) __maxnreg__(sizeof(C) == 8 ? 128 : (W 
   for (int j = 0; j < nj; ++j) {
     const int4 jn = __ldg(&jl[j + 1 < nj ? j + 1 : j]);          // used after pass 1: its latency hides behind it
     cp_async_wait_all();
-    __syncwarp();
+    sync();
     C X[N];
     if (act) {
       // sigma_x = 0: h_x is the constant w_s / N (side A) or 1 / N; sigma_y = 0: h_y is the constant 1 / N
@@ -708,12 +713,12 @@ __global__ void __launch_bounds__(32 * W) __maxnreg__(sizeof(C) == 8 ? 128 : (W 
       const C c1 = F32 ? cvt<C>(n1) : buf[JS::VYH + ln];
       job_pass1<N, true>(buf, ln, side, m, szs, ux_ ? buf[JS::HI + side * JS::TS].x : (R)1, c1, ux_, ry_);
     }
-    __syncwarp();
+    sync();
     if (act) {
       const C c2 = F32 ? cvt<C>(n2) : buf[JS::VXP + ln], c3 = F32 ? cvt<C>(n3) : buf[JS::VZP];
       job_pass2_in<N, true>(buf, ln, szs, sxb, c2, c3, X);
     }
-    __syncwarp();
+    sync();
     if (j + 1 < nj) issue(jn);               // the tile is free: the next job's data arrives during pass 2
     if (act) {
       fft_reg<N, +1>(X);
@@ -731,7 +736,7 @@ __global__ void __launch_bounds__(32 * W) __maxnreg__(sizeof(C) == 8 ? 128 : (W 
 #pragma unroll
     for (int j = 0; j < N; ++j) buf[j * P + ln] = v[j];          // [ky][cx]
   }
-  __syncwarp();
+  sync();
   if (act) {
     C v[N];
 #pragma unroll
@@ -1291,6 +1296,8 @@ int init_streams_v1(dgfs_ctx* c) {
   // shared memory of an SM on its own), same step time; at equal priority only the tails overlap, 1 % faster.
   // Off by default: one stream, per-kernel event times that add up.
   c->v1_overlap = (ov && atoi(ov) != 0);
+  const char* pk = getenv("DGFS_V1_PACK");
+  c->v1_pack = (pk && atoi(pk) != 0);      // measured at c1 (N = 24): 119.5 against 113.2 ms of k_xy per 3 steps, off by default
   const char* xw = getenv("DGFS_V1_XYW");
   c->v1_xyw = (xw && atoi(xw) == 2) ? 2 : 4;
   if (!c->v1_overlap) return DGFS_OK;
@@ -1381,6 +1388,10 @@ static int collide_v1_impl(dgfs_ctx* c, const double* f, double* out, int nx, bo
       cudaFuncSetAttribute(k_xy<N, W, cplx>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_xy);
       cudaFuncSetAttribute(k_xy<N, W, cplxf>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_xy / 2);
       cudaFuncSetAttribute(k_xy<N, 2, cplx>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_xy / 2);
+      if constexpr (N < 32) {
+        cudaFuncSetAttribute(k_xy<N, W, cplx, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_xy);
+        cudaFuncSetAttribute(k_xy<N, W, cplxf, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_xy / 2);
+      }
       cudaFuncSetAttribute(k_xy_full<N, W>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_xyf);
       cudaFuncSetAttribute(k_nyq2<N, 2>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_nyq);
     } else {
@@ -1461,6 +1472,14 @@ static int collide_v1_impl(dgfs_ctx* c, const double* f, double* out, int nx, bo
         { ProfScope ps(c->prof, st, "k_xy", nb * (run_vhs * (fl.xy - fwd_xy) + nrun_vhs * fwd_xy));
           if constexpr (N > 32) {
             k_xy_wide<N><<<dim3(N / 2, items), 2 * N, 2 * smem_wide, st>>>(c->v1, c->tab, gv, c->v1.hxy, nyqb[b], Sb[b], T + (size_t)slot * slot_stride, r);
+          } else if (N < 32 && c->v1_pack) {          // N lanes per job: W planes on N W threads (k_xy, PACK)
+            if constexpr (N < 32) {
+              if (f32) {
+                const GzViewT<cplxf> gvf{(const cplxf*)GzR[b], (const cplxf*)Gz0, nzr, nz0};
+                k_xy<N, W, cplxf, true><<<dim3(N / W, items), N * W, smem_xy / 2, st>>>(c->v1, c->tab, gvf, c->v1.hxyf, nyqb[b], Sb[b], T + (size_t)slot * slot_stride, r);
+              } else
+                k_xy<N, W, cplx, true><<<dim3(N / W, items), N * W, smem_xy, st>>>(c->v1, c->tab, gv, c->v1.hxy, nyqb[b], Sb[b], T + (size_t)slot * slot_stride, r);
+            }
           } else if (f32) {         // dgfs_params::precision = 1
             const GzViewT<cplxf> gvf{(const cplxf*)GzR[b], (const cplxf*)Gz0, nzr, nz0};
             k_xy<N, W, cplxf><<<dim3((N + W - 1) / W, items), 32 * W, smem_xy / 2, st>>>(c->v1, c->tab, gvf, c->v1.hxyf, nyqb[b], Sb[b], T + (size_t)slot * slot_stride, r);

@@ -171,6 +171,7 @@ struct dgfs_ctx {
   // r + 1 (z shifts, Nyquist fields, their product term; bound by memory and latency) run on `aux`, a
   // high-priority stream of the library, while the plane jobs of radial node r (bound by the FP64 pipe) run on
   // the caller's stream; double-buffered intermediates, ordered by these events
+  int v1_pack = 0;                       // DGFS_V1_PACK=1, N < 32: plane jobs dealt out N lanes each instead of one per warp
   int v1_xyw = 4;                        // warps per k_xy block (DGFS_V1_XYW)
   int v1_overlap = 0;                    // DGFS_V1_OVERLAP=1: three streams (default: everything on the caller's stream)
   cudaStream_t aux = nullptr, aux2 = nullptr;

@@ -77,6 +77,13 @@ CONFIGS = {
                       density=(1.0, 8.009e20 / 1.680e21),
                       wall_u=((0.0, -50.0 / 337.2, 0.0), (0.0, 50.0 / 337.2, 0.0)),
                       kn=((0.793, 0.803), (0.555, 0.606)), scheme="euler"),
+    # Two extra operating points for bench lines (not BASELINE.json configurations):
+    # c4 with VSS scattering (every pair needs a full table b_rs(k): 2.7 GB per pair in the paper's layout),
+    # and c2 at the radial resolution the paper recommends as sufficient, N_rho = N/2.
+    "c4vss": Config("c4vss", 190304676, (1.0, 4.0), _full(0.5, 2), ((1.2, 1.3), (1.3, 1.4)),
+                    N=48, L=7.0, N_rho=48, M=32, nx=64, kind="bimaxwell"),
+    "c2half": Config("c2half", 190304672, (1.0, _KR / _AR), ((0.81, 0.805), (0.805, 0.80)), _full(1.0, 2),
+                     N=32, L=6.0, N_rho=16, M=12, nx=4096, kind="c2mix"),
 }
 
 
