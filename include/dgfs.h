@@ -155,6 +155,14 @@ int dgfs_profile_reset(dgfs_ctx *c);
  * either may be NULL.  Synchronous; needs no context. */
 int dgfs_measure_fp64_peak(int device, double seconds, double *tflops_burst, double *tflops_sustained);
 
+/* Evidence for the transform kernels' design (BASELINE.json north_star: "shared-memory radix stages ... or per-axis DFT as
+ * a dense contraction on FP64 tensor cores where N makes that the faster choice"): complex 1-D DFTs of length N
+ * (8, 16, 24, 32 or 48) per second on `device`, on chip (registers / shared memory only inside the timed loop), by
+ * method 0 = the register FFT every pass of the pipeline uses, method 1 = the same DFT as a real (2N x 2N) matrix
+ * product on the FP64 tensor path (mma.sync.m8n8k4.f64).  *rel_err: one transform of each method against the direct
+ * sum evaluated on the host, relative to the largest output.  Host outputs; synchronous; needs no context. */
+int dgfs_measure_dft(int device, int N, int method, double seconds, double *dfts_per_second, double *rel_err);
+
 /* 1-D mesh for dgfs_step: ne uniform elements on [x0, x1], nodal DG of polynomial degree
  * `order` on K = order+1 Gauss-Lobatto-Legendre nodes, purely diffuse walls at both ends
  * (Table 2; readings DG-1, DG-2). */

@@ -19,7 +19,7 @@ ABI_SYMBOLS = (
     "dgfs_workspace_bytes", "dgfs_reserve", "dgfs_get_quadrature", "dgfs_get_tables",
     "dgfs_flops_per_pair_eval", "dgfs_step", "dgfs_step_euler", "dgfs_advect_rhs",
     "dgfs_launch_count", "dgfs_profile_enable", "dgfs_profile_count", "dgfs_profile_get",
-    "dgfs_profile_reset", "dgfs_collide_host", "dgfs_measure_fp64_peak", "dgfs_table_bytes",
+    "dgfs_profile_reset", "dgfs_collide_host", "dgfs_measure_fp64_peak", "dgfs_table_bytes", "dgfs_measure_dft",
 )
 
 DGFS_OK, DGFS_EINVAL, DGFS_ECUDA, DGFS_ENOMEM, DGFS_ENOSUP = 0, -1, -2, -3, -4
@@ -97,6 +97,8 @@ def load_library():
     lib.dgfs_measure_fp64_peak.restype = ip
     lib.dgfs_workspace_bytes.argtypes = [vp, ip]
     lib.dgfs_workspace_bytes.restype = C.c_size_t
+    lib.dgfs_measure_dft.argtypes = [ip, ip, ip, C.c_double, _dp, _dp]
+    lib.dgfs_measure_dft.restype = ip
     lib.dgfs_table_bytes.argtypes = [vp]
     lib.dgfs_table_bytes.restype = C.c_size_t
     lib.dgfs_reserve.argtypes = [vp, ip]
@@ -240,6 +242,13 @@ def dgfs_workspace_bytes(ctx, nx):
 
 def dgfs_reserve(ctx, nx):
     _check(ctx, load_library().dgfs_reserve(ctx, int(nx)))
+
+
+def dgfs_measure_dft(device, N, method, seconds=0.5):
+    """(complex DFTs of length N per second, relative error of one transform): method 0 register FFT, 1 FP64 MMA."""
+    rate, err = C.c_double(), C.c_double()
+    _check(None, load_library().dgfs_measure_dft(int(device), int(N), int(method), float(seconds), C.byref(rate), C.byref(err)))
+    return rate.value, err.value
 
 
 def dgfs_table_bytes(ctx):

@@ -1,6 +1,6 @@
 // collide.cu -- dgfs_collide / dgfs_collide_pairs: Algorithm 2 of PAPER.md on sm_100a.
-// This file holds the C ABI entry points and the stage-per-kernel (v0) pipeline, which serves pairs with a
-// full b table (VSS, table_mode 1) and N = 48; all-VHS configurations with N <= 32 run collide_v1.cu.
+// This file holds the C ABI entry points and the stage-per-kernel (v0) pipeline, which serves N = 48 configurations
+// with full-table pairs (VSS, table_mode 1) and DGFS_PIPELINE=v0; everything else runs collide_v1.cu.
 //
 // Per pair (p,q), spatial point x, radial node r, sphere point s (steps 2-8):
 //   A = ifft3(e^{+i mu_q a_rs} f^_p),  B = ifft3(e^{-i mu_p a_rs} f^_q),  QG += w_r w_s b_rs fft3(A.B),

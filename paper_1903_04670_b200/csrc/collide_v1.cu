@@ -570,6 +570,8 @@ __global__ void __launch_bounds__(32 * NW) k_nyq2(V1Tables t, DevTables tab, con
   };
   // fields of an axis with sigma_{s,d} = 0 vanish identically (v1_tables.h): run no job; zeros are stored only for
   // pairs with a full table (k_xy_full reads all three fields; k_wterm skips the masked ones)
+  // pairs with a full table: the fields go to k_xy_full in their natural layout [j][lane] (and zeros are stored for the
+  // fields that vanish); the other pairs' fields go to k_wterm, de-interleaved / swizzled for its bulk copies
   const bool store_zeros = tab.full[pair] != 0;
   const int zbit = (which == 0) ? 4 : (which == 1 ? 1 : 2);
   const int ooff = (which == 0) ? NL::UZ : (which == 1 ? NL::UXP : NL::UY);
@@ -606,7 +608,7 @@ __global__ void __launch_bounds__(32 * NW) k_nyq2(V1Tables t, DevTables tab, con
       cplx* out = nyq + ((size_t)item * tab.M + s) * NL::STRIDE;
       if (which == 0) {
 #pragma unroll
-        for (int j = 0; j < N; ++j) out[NL::UZ + (j * 2 + (ln & 1)) * H + (ln >> 1)] = X[j];
+        for (int j = 0; j < N; ++j) out[NL::UZ + (store_zeros ? j * N + ln : (j * 2 + (ln & 1)) * H + (ln >> 1))] = X[j];
       } else if (which == 1) {
         const double sb = (ln & 1) ? -1.0 : 1.0;
 #pragma unroll
@@ -616,7 +618,7 @@ __global__ void __launch_bounds__(32 * NW) k_nyq2(V1Tables t, DevTables tab, con
         }
       } else {
 #pragma unroll
-        for (int j = 0; j < N; ++j) out[NL::UY + j * N + (ln ^ uy_swz(j))] = X[j];
+        for (int j = 0; j < N; ++j) out[NL::UY + j * N + (store_zeros ? ln : (ln ^ uy_swz(j)))] = X[j];
       }
     }
     s = sn; scale = scale_next;
@@ -803,9 +805,9 @@ __global__ void __launch_bounds__(32 * W) k_xy_full(V1Tables t, DevTables tab, G
       cp_async16(&buf[JS::VXP + ln], nq + NL::VXP + ln);
       if (ln == 0) cp_async16(&buf[JS::VZP], nq + NL::VZP + cz);
 #pragma unroll
-      for (int j = 0; j < N; ++j) cp_async16(&buf[FS::UZ + j * N + ln], nq + NL::UZ + (j * 2 + (ln & 1)) * H + (ln >> 1));
+      for (int j = 0; j < N; ++j) cp_async16(&buf[FS::UZ + j * N + ln], nq + NL::UZ + j * N + ln);
       cp_async16(&buf[FS::UX + ln], nq + NL::UXP + ln * N + cz);
-      cp_async16(&buf[FS::UY + ln], nq + NL::UY + ln * N + (cz ^ uy_swz(ln)));
+      cp_async16(&buf[FS::UY + ln], nq + NL::UY + ln * N + cz);
     }
     cp_async_commit();
   };

@@ -36,7 +36,8 @@ struct V1Tables {
 // swizzle of the cz index of uy within its row (NyqLayout::UY)
 __host__ __device__ __forceinline__ int uy_swz(int cx) { return (cx >> 1) & 7; }
 
-// per (item, s) block of Nyquist-plane fields written by k_nyq, in units of cplx
+// per (item, s) block of Nyquist-plane fields written by k_nyq.  UY and UZ as commented for the pairs whose fields go to
+// k_wterm; for pairs with a full table (k_xy_full) they are plain [cx][cz] and [cy][cx], in units of cplx
 template <int N>
 struct NyqLayout {
   static constexpr int VYH = 0;            // [N]     lane format, x-Nyquist row correction (no y factor)

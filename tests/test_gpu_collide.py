@@ -446,3 +446,18 @@ def test_precision_1_is_refused_where_it_is_not_implemented(torch_cuda):
     with pytest.raises(api.DgfsError) as e:
         _gpu_op(vss, precision=2)
     assert e.value.code == api.DGFS_EINVAL
+
+
+@pytest.mark.parametrize("N", [8, 24, 48])
+def test_dft_probe_both_methods_compute_the_dft(torch_cuda, N):
+    """dgfs_measure_dft (the FFT-vs-tensor-core evidence of DESIGN.md section 8): each method's transform of the probe
+    input equals the direct sum (evaluated on the host inside the library) to round-off, and a rate comes back."""
+    from oracle_pool import record
+    from paper_1903_04670_b200 import dgfs_measure_dft
+    rates = []
+    for method in (0, 1):
+        rate, err = dgfs_measure_dft(0, N, method, 0.2)
+        assert err < 1e-12 and rate > 0, (method, rate, err)
+        rates.append(rate)
+    record("dft-probe", "N=%d: register FFT %.3e DFT/s, FP64 mma.sync m8n8k4 %.3e DFT/s, ratio" % (N, rates[0], rates[1]),
+           rates[0] / rates[1], 1.0)
