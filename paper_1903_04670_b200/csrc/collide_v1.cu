@@ -873,7 +873,7 @@ __global__ void __launch_bounds__(32 * W) k_xy_full(V1Tables t, DevTables tab, G
 // with f = fscale of the target (ratio of sphere weights).  Thread pair per pencil as in k_zfwd_acc; the sums
 // over s stay in registers.  b is read in SPEC layout [r][s][kz][kx][ky].
 template <int N, bool FIRST>
-__global__ void __launch_bounds__(256) k_zfwd_full(DevTables tab, V1Tables t, const cplx* __restrict__ Tf,
+__global__ void __launch_bounds__(256, N <= 24 ? 2 : 1) k_zfwd_full(DevTables tab, V1Tables t, const cplx* __restrict__ Tf,
                                                    cplx* __restrict__ QG, size_t qstride, int r) {
   constexpr int H = N / 2, N2 = N * N, N3 = N2 * N;
   const int par = threadIdx.x >> 7;

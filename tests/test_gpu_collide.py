@@ -461,3 +461,40 @@ def test_dft_probe_both_methods_compute_the_dft(torch_cuda, N):
         rates.append(rate)
     record("dft-probe", "N=%d: register FFT %.3e DFT/s, FP64 mma.sync m8n8k4 %.3e DFT/s, ratio" % (N, rates[0], rates[1]),
            rates[0] / rates[1], 1.0)
+
+
+def test_calls_on_two_streams_of_one_context_do_not_race(torch_cuda):
+    """The workspace belongs to one call at a time: a call on another stream, issued without any host or stream
+    synchronisation, waits for the previous call's last launch (include/dgfs.h: calls on one context are ordered)."""
+    torch = torch_cuda
+    cfg = _rand_cfg("t", 2, 16, 3, 12, (1.0, 1.0), (0.6, 0.8), (1.0, 2.0), seed=41)
+    fa = torch.from_numpy(make_points(cfg, range(24))).cuda()
+    fb = torch.from_numpy(make_points(cfg, range(24, 48))).cuda()
+    with _gpu_op(cfg) as op:
+        Qa0, Qb0 = op.collide(fa).clone(), op.collide(fb).clone()
+        torch.cuda.synchronize()
+        sa, sb = torch.cuda.Stream(), torch.cuda.Stream()
+        Qa, Qb = torch.empty_like(fa), torch.empty_like(fb)
+        for _ in range(3):
+            with torch.cuda.stream(sa):
+                op.collide(fa, Qa)
+            with torch.cuda.stream(sb):
+                op.collide(fb, Qb)
+        torch.cuda.synchronize()
+        assert torch.equal(Qa, Qa0) and torch.equal(Qb, Qb0)
+
+
+def test_two_contexts_on_two_devices(torch_cuda):
+    """Kernel attributes (dynamic shared memory opt-in) are set per context, i.e. per device."""
+    torch = torch_cuda
+    if torch.cuda.device_count() < 2:
+        pytest.skip("needs two GPUs")
+    cfg = get_config("c0")
+    f = make_points(cfg, range(cfg.nx))
+    outs = []
+    for dev in (0, 1):
+        with torch.cuda.device(dev):
+            from paper_1903_04670_b200 import Dgfs
+            with Dgfs.from_config(cfg, device=dev) as op:
+                outs.append(op.collide(torch.from_numpy(f).cuda(dev)).cpu())
+    assert torch.equal(outs[0], outs[1])
