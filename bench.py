@@ -379,7 +379,9 @@ def report(args, cfg, op, prof, nx, world, stages, ms_per_step, value, e2e_ms, n
         "achieved": step_tflops, "peak": FP64_PEAK_NOMINAL_TFLOPS, "unit": "TFLOP/s",
         "peak_source": "FP64 DFMA pipe, 148 SM x 64 DFMA/clk x 2 x 1.965 GHz (DESIGN.md section 8); "
                        "MEASURED_PEAKS.json has no fp64 entry",
-        "scope": "whole step (every kernel of the call), flop count of the algorithm as executed",
+        "scope": "whole step (every kernel of the call), flop count of the algorithm as executed"
+                 + ("; precision f32: the plane jobs run on the FP32 pipe (twice the lanes), so this fraction of the FP64 peak is "
+                    "for comparison with the fp64 line only, not a roofline fraction" if args.precision == "f32" else ""),
         "flops_floor_ms": flops_floor_ms, "algorithmic_bytes_floor_ms": alg_bytes_floor_ms, "step_ms": ms_per_step,
         "step_flops": flops_step, "algorithmic_bytes": alg_bytes,
         "step_dram_bytes": dram_step, "step_dram_floor_ms": dram_floor_ms,

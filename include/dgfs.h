@@ -20,6 +20,11 @@
  *     documented "host" are ordinary host pointers; the library never takes ownership of either;
  *   - `stream` is the caller's cudaStream_t passed as void* (NULL = legacy default stream);
  *     dgfs_collide* / dgfs_step enqueue work on it and return without synchronising;
+ *   - the workspace of a context belongs to one call at a time: every call first waits, on its own stream, for the
+ *     last launch of the previous call on that context, whichever stream that was issued on, so calls on different
+ *     streams are safe and serialised; when a batch needs a larger workspace it is re-allocated in stream order
+ *     (cudaFreeAsync / cudaMallocAsync on `stream`, no device-wide synchronisation) -- not possible while `stream`
+ *     is being captured into a CUDA graph: call dgfs_reserve first;
  *   - every int-returning call returns DGFS_OK (0) or a negative DGFS_E* code, validates its
  *     arguments before any launch, and records a message readable with dgfs_last_error();
  *   - there is no CPU fallback: without a CUDA device dgfs_create fails with DGFS_ECUDA.

@@ -195,11 +195,12 @@ static int dg_setup(dgfs_ctx* c, const dgfs_mesh1d* mesh, const char* who, DgOps
   build_ops(mesh->order, ops);
   const size_t N3 = c->N3, state = (size_t)mesh->ne * ops->K * c->ns * N3;
   const size_t need = (3 * state + 2 * (size_t)c->ns * N3 + 2 * c->ns + c->ns + 64) * sizeof(double);
-  if (need > c->dg_ws_bytes) {
-    cudaDeviceSynchronize();
-    cudaFree(c->dg_ws); c->dg_ws = nullptr; c->dg_ws_bytes = 0;
-    int rc = check_cuda(c, cudaMalloc(&c->dg_ws, need), "DG workspace allocation");
-    if (rc) return rc;
+  if (need > c->dg_ws_bytes) {       // ordered on the caller's stream, like the collision workspace (collide.cu)
+    if (c->ev_last_set) cudaStreamWaitEvent(st, c->ev_last, 0);
+    if (c->dg_ws) cudaFreeAsync(c->dg_ws, st);
+    c->dg_ws = nullptr; c->dg_ws_bytes = 0;
+    int rc = check_cuda(c, cudaMallocAsync(&c->dg_ws, need, st), "DG workspace allocation");
+    if (rc) { c->dg_ws = nullptr; return rc; }
     c->dg_ws_bytes = need;
   }
   double* w = (double*)c->dg_ws;
