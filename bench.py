@@ -292,11 +292,10 @@ def main():
         else:
             op.collide(f_dev, q_dev)
 
-    # ---------------- device-resident timing ----------------
+    # ---------------- device-resident timing (per-launch profiling OFF: nothing but the step is in the region) ------
     for _ in range(args.warmup):
         step_device()
     barrier()
-    op.profile(on=True, reset=True)
     launches0 = op.launch_count()
     sampler = ClockSampler(local)
     sampler.start()
@@ -311,12 +310,19 @@ def main():
     sampler.stop_flag = True
     sampler.join()
     total_ms = sum(a.elapsed_time(b) for a, b in ev)
-    prof = op.profile(on=False)
     launches = op.launch_count() - launches0
     total_ms = max_over_ranks(total_ms)
     ms_per_step = total_ms / args.steps
     evals_rank = stages * nx * cfg.ns * cfg.ns
     value = whole_job_rate(evals_rank, world, ms_per_step)
+    # ---------------- the same steps once more with the library's per-launch CUDA events on (per-kernel times) -------
+    op.profile(on=True, reset=True)
+    for i in range(args.steps):
+        if flush is not None:
+            flush.fill_(i)
+        step_device()
+    barrier()
+    prof = op.profile(on=False)
 
     # ---------------- end to end: pinned host -> device -> step -> pinned host ----------------
     # homogeneous workloads: dgfs_collide_host (HOST pointers in and out; the library's own streams carry the copies

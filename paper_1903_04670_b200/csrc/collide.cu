@@ -77,6 +77,7 @@ int ensure_workspace(dgfs_ctx* c, size_t bytes, cudaStream_t st) {
     c->pool_set = true;
   }
   if (c->ev_last_set) cudaStreamWaitEvent(st, c->ev_last, 0);      // earlier calls on other streams still use the old block
+  drop_graphs_v1(c);                                               // captured graphs point into the old block
   if (c->ws) cudaFreeAsync(c->ws, st);
   c->ws = nullptr; c->ws_bytes = 0;
   int rc = check_cuda(c, cudaMallocAsync(&c->ws, bytes, st), "workspace allocation");

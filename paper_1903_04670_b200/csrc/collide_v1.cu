@@ -1188,7 +1188,7 @@ namespace dgfs {
 namespace {
 struct PlanV1 {
   int nbx, nbuf, tslots;
-  size_t off_fhat, off_fhh, off_nyqy, off_qg, off_gzr[2], off_gz0, off_nyq[2], off_s[2], off_t, off_tf, off_fp, nyq_bytes, qstride, total;
+  size_t off_fhat, off_fhh, off_nyqy, off_qg, off_gzr[2], off_gz0, off_nyq[2], off_s[2], off_t, off_tf, off_fp, off_gin, off_gout, nyq_bytes, qstride, total;
 };
 PlanV1 plan_v1(const dgfs_ctx* c, int nx) {
   PlanV1 pl{};
@@ -1230,6 +1230,10 @@ PlanV1 plan_v1(const dgfs_ctx* c, int nx) {
   // Tf: per-s forward-transformed planes of the full-table pairs
   pl.off_tf = take(c->any_full ? items * c->M * arr : 0);
   pl.off_fp = take(c->nyq_filter ? (size_t)nbx * c->ns * N3 * sizeof(double) : 0);     // filtered inputs
+  // small batches replayed from a CUDA graph: fixed input / output staging (run_collide_v1)
+  const bool small = nx * c->npairs <= c->v1_graph_items;
+  pl.off_gin = take(small ? (size_t)nx * c->ns * N3 * sizeof(double) : 0);
+  pl.off_gout = take(small ? (size_t)nx * c->npairs * N3 * sizeof(double) : 0);
   pl.total = off;
   return pl;
 }
@@ -1298,6 +1302,8 @@ int init_streams_v1(dgfs_ctx* c) {
   // shared memory of an SM on its own), same step time; at equal priority only the tails overlap, 1 % faster.
   // Off by default: one stream, per-kernel event times that add up.
   c->v1_overlap = (ov && atoi(ov) != 0);
+  const char* gi = getenv("DGFS_V1_GRAPH_ITEMS");
+  if (gi) c->v1_graph_items = atoi(gi) > 0 ? atoi(gi) : 0;
   const char* pk = getenv("DGFS_V1_PACK");
   c->v1_pack = (pk && atoi(pk) != 0);      // measured at c1 (N = 24): 119.5 against 113.2 ms of k_xy per 3 steps, off by default
   const char* xw = getenv("DGFS_V1_XYW");
@@ -1525,7 +1531,7 @@ static int collide_v1_impl(dgfs_ctx* c, const double* f, double* out, int nx, bo
   return check_cuda(c, cudaGetLastError(), "collide (v1) launch");
 }
 
-int run_collide_v1(dgfs_ctx* c, const double* f, double* out, int nx, bool pairs_out, cudaStream_t st) {
+static int dispatch_v1(dgfs_ctx* c, const double* f, double* out, int nx, bool pairs_out, cudaStream_t st) {
   switch (c->N) {
     case 8: return collide_v1_impl<8>(c, f, out, nx, pairs_out, st);
     case 16: return collide_v1_impl<16>(c, f, out, nx, pairs_out, st);
@@ -1534,6 +1540,59 @@ int run_collide_v1(dgfs_ctx* c, const double* f, double* out, int nx, bool pairs
     case 48: return collide_v1_impl<48>(c, f, out, nx, pairs_out, st);      // VHS pairs only (collide_v1_wide.cuh)
   }
   return set_error(c, DGFS_ENOSUP, "v1 pipeline: unsupported N");
+}
+
+void drop_graphs_v1(dgfs_ctx* c) {
+  for (auto& g : c->graphs) cudaGraphExecDestroy(g.exec);
+  c->graphs.clear();
+}
+void free_graph_stream_v1(dgfs_ctx* c) { if (c->cap_stream) cudaStreamDestroy(c->cap_stream); c->cap_stream = nullptr; }
+
+// Small batches (nx * pairs <= 64: config c0, single points of a test) are bound by launch latency: ~100 launches of a
+// few microseconds each.  Their whole call is captured once, on fixed staging buffers inside the workspace, into a CUDA
+// graph and replayed: copy f in, one graph launch, copy Q out.  Same kernels, same launch order, same bits.  Not
+// while the caller captures its own graph, nor with per-launch profiling on, nor with the three-stream schedule.
+int run_collide_v1(dgfs_ctx* c, const double* f, double* out, int nx, bool pairs_out, cudaStream_t st) {
+  cudaStreamCaptureStatus cap = cudaStreamCaptureStatusNone;
+  cudaStreamIsCapturing(st, &cap);
+  const bool small = nx * c->npairs <= c->v1_graph_items && !c->prof.on && !c->v1_overlap && cap == cudaStreamCaptureStatusNone;
+  if (!small) return dispatch_v1(c, f, out, nx, pairs_out, st);
+  const PlanV1 pl = plan_v1(c, nx);
+  int rc = ensure_workspace(c, pl.total, st);
+  if (rc) return rc;
+  double* gin = (double*)((char*)c->ws + pl.off_gin);
+  double* gout = (double*)((char*)c->ws + pl.off_gout);
+  const size_t in_bytes = (size_t)nx * c->ns * c->N3 * sizeof(double);
+  const size_t out_bytes = (size_t)nx * (pairs_out ? c->npairs : c->ns) * c->N3 * sizeof(double);
+  dgfs_ctx::SmallGraph* g = nullptr;
+  for (auto& e : c->graphs) if (e.nx == nx && e.pairs == pairs_out && e.ws == c->ws) g = &e;
+  if (!g) {
+    if (!c->v1_attr_done) {          // first call of the context: set the kernel attributes outside any capture
+      if ((rc = dispatch_v1(c, f, out, nx, pairs_out, st))) return rc;
+      return DGFS_OK;
+    }
+    const long long l0 = c->prof.total_launches;
+    cudaGraph_t graph = nullptr;
+    if (!c->cap_stream && (rc = check_cuda(c, cudaStreamCreateWithFlags(&c->cap_stream, cudaStreamNonBlocking), "stream create"))) return rc;
+    if ((rc = check_cuda(c, cudaStreamBeginCapture(c->cap_stream, cudaStreamCaptureModeThreadLocal), "graph capture"))) return rc;
+    rc = dispatch_v1(c, gin, gout, nx, pairs_out, c->cap_stream);
+    cudaError_t e = cudaStreamEndCapture(c->cap_stream, &graph);
+    const long long nl = c->prof.total_launches - l0;
+    c->prof.total_launches = l0;
+    if (rc) { if (graph) cudaGraphDestroy(graph); return rc; }
+    if ((rc = check_cuda(c, e, "graph capture"))) return rc;
+    cudaGraphExec_t exec = nullptr;
+    e = cudaGraphInstantiate(&exec, graph, 0);
+    cudaGraphDestroy(graph);
+    if ((rc = check_cuda(c, e, "graph instantiation"))) return rc;
+    c->graphs.push_back({nx, pairs_out, c->ws, exec, nl});
+    g = &c->graphs.back();
+  }
+  cudaMemcpyAsync(gin, f, in_bytes, cudaMemcpyDeviceToDevice, st);
+  if ((rc = check_cuda(c, cudaGraphLaunch(g->exec, st), "graph launch"))) return rc;
+  cudaMemcpyAsync(out, gout, out_bytes, cudaMemcpyDeviceToDevice, st);
+  c->prof.total_launches += g->launches;
+  return check_cuda(c, cudaGetLastError(), "collide (v1, graph) launch");
 }
 
 }  // namespace dgfs

@@ -616,6 +616,8 @@ extern "C" void dgfs_destroy(dgfs_ctx* c) {
   cudaFree(c->d_v0_sskip); cudaFree(c->d_v0_tsrc); cudaFree(c->d_v0_wfac); cudaFree(c->d_bref); cudaFree(c->d_bmap);
   for (auto p : c->h_bfull) cudaFree(p);
   cudaFree(c->ws); cudaFree(c->dg_ws);
+  drop_graphs_v1(c);
+  free_graph_stream_v1(c);
   free_tables_v1(c);
   free_streams_v1(c);
   if (c->ev_last) cudaEventDestroy(c->ev_last);

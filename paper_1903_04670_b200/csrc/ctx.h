@@ -182,6 +182,11 @@ struct dgfs_ctx {
   cudaEvent_t ev_last = nullptr;
   bool ev_last_set = false;
   bool pool_set = false;                 // release threshold of the stream-ordered allocator raised
+  // small batches (collide_v1.cu, run_collide_v1): the whole call captured once into a CUDA graph and replayed
+  struct SmallGraph { int nx; bool pairs; void* ws; cudaGraphExec_t exec; long long launches; };
+  std::vector<SmallGraph> graphs;
+  cudaStream_t cap_stream = nullptr;     // captures happen on a stream of the library (the legacy default stream cannot capture)
+  int v1_graph_items = 64;               // largest nx * pairs served that way (DGFS_V1_GRAPH_ITEMS; 0 = never)
   // workspace (grown on demand)
   void* ws = nullptr;
   size_t ws_bytes = 0;
@@ -220,6 +225,8 @@ int build_tables_v1(dgfs_ctx* c);
 void free_tables_v1(dgfs_ctx* c);
 int init_streams_v1(dgfs_ctx* c);
 void free_streams_v1(dgfs_ctx* c);
+void drop_graphs_v1(dgfs_ctx* c);
+void free_graph_stream_v1(dgfs_ctx* c);
 size_t workspace_bytes_v1(const dgfs_ctx* c, int nx);
 int run_collide_v1(dgfs_ctx* c, const double* f, double* out, int nx, bool pairs_out, cudaStream_t st);
 double flops_per_pair_eval_v1(const dgfs_ctx* c, int pair);
