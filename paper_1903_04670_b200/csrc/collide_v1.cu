@@ -1,4 +1,4 @@
-// collide_v1.cu -- v1 pipeline of dgfs_collide (N <= 32): Algorithm 2 of PAPER.md with the exact
+// collide_v1.cu -- v1 pipeline of dgfs_collide (N <= 32; N = 48 with collide_v1_wide.cuh): Algorithm 2 of PAPER.md with the exact
 // rearrangements of DESIGN.md section 5 (R-1 .. R-11).  The description below is the path of pairs whose b_rs
 // does not depend on s (VHS, table_mode 0); pairs with a full table share the first three kernels and take
 // k_xy_full / k_zfwd_full afterwards (described there).
@@ -20,12 +20,13 @@
 //   k_zshift  inverse z pass of h_z f^ for every DISTINCT z shift (the sphere rules share sigma_z values:
 //             18 arrays instead of 96 at c2), on the Hermitian half of the (lx,ly) plane (R-7)
 //   k_nyq1d / k_nyq2   the Nyquist-plane fields: three 1-D sums and three 2-D transforms per (pair, s)
-//   k_wterm   -sum_s Re W Im W
+//   k_wterm   -sum_s Re W Im W  (tables staged by TMA bulk copies)
 //   k_xy      per (pair, cz plane): for every s the inverse x,y passes of the packed field in one warp
 //             (lane = pencil, FFTs in registers, one transposition through shared memory), the product
 //             and the sum over s in registers, then the forward x,y passes of the real plane S_r(., ., cz)
 //   k_zfwd_acc  forward z pass, QG += w_r b_r .
-// Steps 1 and 10 reuse the v0 kernels.  Sphere points with a zero component (R-9) skip the fields and factors
+// Steps 1 and 10 reuse the v0 kernels.  dgfs_params::precision = 1 runs k_xy on float2 copies (k_xy<N, W, float2>).
+// Sphere points with a zero component (R-9) skip the fields and factors
 // that vanish; same-species pairs run one point per antipodal couple (R-10) and a transposed pair (q,p) reuses
 // the summed products of (p,q) (R-11): see build_tables_v1.
 #include <cmath>
