@@ -37,6 +37,9 @@
 
 namespace dgfs {
 
+// flags of V1Tables::jobs[].w beside the zero-component mask (bits 0-2)
+enum { JOB_FIRST = 8, JOB_LAST = 16, JOB_SLOT = 32 };
+
 // ---------------------------------------------------------------- create-time tables ------------
 static void split_factor(double theta, int N, double scale, cplx* h, double* s) {
   const int H = N / 2;
@@ -113,6 +116,12 @@ int build_tables_v1(dgfs_ctx* c) {
   {
     const char* ap = getenv("DGFS_V1_ANTIPODAL");
     const bool on = !(ap && atoi(ap) == 0);
+    // which point of a couple runs: the one whose first non-zero component in the order (z, x, y) is positive, so that
+    // the points kept are (sx, +-sy, sz) couples wherever the rule has them: they share their inverse x pass (R-12)
+    auto runs_first = [&](int a) {
+      for (int d : {2, 0, 1}) if (c->sigma[3 * a + d] != 0.0) return c->sigma[3 * a + d] > 0.0;
+      return true;
+    };
     for (int p = 0; on && p < ns; ++p) {
       const int pair = p * ns + p;
       if (c->full[pair]) continue;
@@ -122,10 +131,11 @@ int build_tables_v1(dgfs_ctx* c) {
           if (c->v1_sskip[(size_t)pair * M + s3]) continue;
           if (c->sigma[3 * s3] == -c->sigma[3 * s2] && c->sigma[3 * s3 + 1] == -c->sigma[3 * s2 + 1] &&
               c->sigma[3 * s3 + 2] == -c->sigma[3 * s2 + 2]) {
-            c->v1_sskip[(size_t)pair * M + s3] = 1;
-            const double fac = (c->w_sigma[s2] + c->w_sigma[s3]) / c->w_sigma[s2];
+            const int keep = runs_first(s2) ? s2 : s3, drop = keep == s2 ? s3 : s2;
+            c->v1_sskip[(size_t)pair * M + drop] = 1;
+            const double fac = (c->w_sigma[s2] + c->w_sigma[s3]) / c->w_sigma[keep];
             for (int r = 0; r < Nr; ++r) {
-              const size_t e = (((size_t)pair * Nr + r) * M + s2) * 2;        // side A
+              const size_t e = (((size_t)pair * Nr + r) * M + keep) * 2;        // side A
               for (int j = 0; j < N; ++j) { hxy[e * 2 * N + j].x *= fac; hxy[e * 2 * N + j].y *= fac; }
               sxy[e * 2] *= fac;
             }
@@ -206,15 +216,52 @@ int build_tables_v1(dgfs_ctx* c) {
   for (int s2 = 0; s2 < M; ++s2)
     for (int d = 0; d < 3; ++d)
       if (c->sigma[3 * s2 + d] == 0.0) c->v1_smask[s2] |= (unsigned char)(1 << d);
-  // the plane jobs of every pair as a list the kernels walk without further look-ups
+  // The plane jobs of every pair as a list the kernels walk without further look-ups, ordered in GROUPS of up to two
+  // sphere points that share their z jobs and their x factors on both sides (equal sigma_z and sigma_x: the points
+  // (sx, +-sy, sz) of the built-in rules): the inverse x pass of such points is the same transform of the same data
+  // and runs once per group (R-12, k_xy).  .w = smask | JOB_FIRST (opens a group) | JOB_LAST (closes it) | JOB_SLOT.
   c->v1_jobs.assign((size_t)np * M, make_int4(0, 0, 0, 0));
   c->v1_njobs.assign(np, 0);
-  for (int pr = 0; pr < np; ++pr) {
-    if (c->v1_tsrc[pr] != pr) continue;
-    for (int s2 = 0; s2 < M; ++s2) {
-      if (c->v1_sskip[(size_t)pr * M + s2]) continue;
-      c->v1_jobs[(size_t)pr * M + c->v1_njobs[pr]++] =
-          make_int4(s2, c->v1_zmap[((size_t)pr * M + s2) * 2], c->v1_zmap[((size_t)pr * M + s2) * 2 + 1], c->v1_smask[s2]);
+  c->v1_xyflops.assign(np, 0.0);
+  {
+    const char* gp = getenv("DGFS_V1_XSHARE");
+    const bool share = !(gp && atoi(gp) == 0) && N <= 32;       // the N = 48 job (collide_v1_wide.cuh) runs every x pass
+    const double fft1 = 5.0 * N * log2((double)N);
+    for (int pr = 0; pr < np; ++pr) {
+      if (c->v1_tsrc[pr] != pr) continue;
+      std::vector<int> run;
+      for (int s2 = 0; s2 < M; ++s2) if (!c->v1_sskip[(size_t)pr * M + s2]) run.push_back(s2);
+      std::vector<char> used(run.size(), 0);
+      auto zj = [&](int s2, int side) { return c->v1_zmap[((size_t)pr * M + s2) * 2 + side]; };
+      auto same_x = [&](int s2, int s3) {            // x factors (weights folded in) of both sides, every radial node
+        if (c->sigma[3 * s2] != c->sigma[3 * s3]) return false;
+        for (int r = 0; r < Nr; ++r) for (int side = 0; side < 2; ++side) {
+          const size_t e2 = ((((size_t)pr * Nr + r) * M + s2) * 2 + side), e3 = ((((size_t)pr * Nr + r) * M + s3) * 2 + side);
+          if (sxy[e2 * 2] != sxy[e3 * 2]) return false;
+          for (int j = 0; j < N; ++j)
+            if (hxy[e2 * 2 * N + j].x != hxy[e3 * 2 * N + j].x || hxy[e2 * 2 * N + j].y != hxy[e3 * 2 * N + j].y) return false;
+        }
+        return true;
+      };
+      auto push = [&](int s2, int flags) {
+        c->v1_jobs[(size_t)pr * M + c->v1_njobs[pr]++] = make_int4(s2, zj(s2, 0), zj(s2, 1), c->v1_smask[s2] | flags);
+        // flops of this job's y pass, factor, packing adds, product, Nyquist fixes; the x pass is counted per group
+        c->v1_xyflops[pr] += N * (N * fft1 + ((c->v1_smask[s2] & 2) ? 2.0 : 6.0) * N * N + 4.0 * N * N + 12.0 * N);
+        if (flags & JOB_FIRST) c->v1_xyflops[pr] += N * (N * fft1 + ((c->v1_smask[s2] & 1) ? 0.0 : 6.0) * N * N);
+      };
+      for (size_t i = 0; i < run.size(); ++i) {
+        if (used[i]) continue;
+        used[i] = 1;
+        size_t mate = run.size();
+        for (size_t k = i + 1; share && k < run.size() && mate == run.size(); ++k)
+          if (!used[k] && zj(run[k], 0) == zj(run[i], 0) && zj(run[k], 1) == zj(run[i], 1) && same_x(run[i], run[k])) mate = k;
+        if (mate < run.size()) {
+          used[mate] = 1;
+          push(run[i], JOB_FIRST);
+          push(run[mate], JOB_LAST | JOB_SLOT);
+        } else push(run[i], JOB_FIRST | JOB_LAST);
+      }
+      c->v1_xyflops[pr] += N * (N + 1.0) * fft1;       // forward y, x passes of the real plane, once per plane
     }
   }
   int rc;
@@ -635,6 +682,80 @@ __global__ void __launch_bounds__(32 * NW) k_nyq2(V1Tables t, DevTables tab, con
 //   pass 2: lane = cx rebuilds the N packed columns X[ly] = Y_A + i Y_B (mirror half by conjugation), inverse
 //           y pass: Z = a_r + i b_r;  acc[cy] += Re Z Im Z
 // in: S[item][cz][cy][cx] = -sum_s Re W Im W (k_wterm);  out: T[item][cz][kx][ky <= H] = fft_xy of S_r(., ., cz).
+// Shared memory of a k_xy warp: the tile, what a GROUP of jobs shares (x factors, x-Nyquist row correction) and what
+// each of its up to two jobs owns (y factors, y-Nyquist column correction, (H,H) scalar).
+template <int N>
+struct GroupSmem {
+  static constexpr int P = N + 1;
+  static constexpr int TILE = N * P;
+  static constexpr int TS = N + 1;
+  static constexpr int HI = TILE;             // [2][TS]  x factors per side
+  static constexpr int VYH = HI + 2 * TS;     // [N]      lane format
+  static constexpr int SLOT = VYH + N;        // per job of the group:
+  static constexpr int HM = 0;                //   [2][TS] y factors per side
+  static constexpr int VXP = 2 * TS;          //   [N]
+  static constexpr int VZP = 2 * TS + N;      //   [1]
+  static constexpr int SLOTW = 2 * TS + N + 2;
+  static constexpr int WORDS = SLOT + 2 * SLOTW;
+};
+
+// Inverse x pass of a group (lane = (side, m), column m of the Hermitian half): x factor, Nyquist row correction,
+// transform in registers, back into the tile WITHOUT the y factor (which differs between the jobs of the group).
+template <int N, class C>
+__device__ __forceinline__ void xpass_group(C* buf, int ln, int side, typename real_of<C>::type szs, C c1, bool unit_i) {
+  typedef GroupSmem<N> GS;
+  constexpr int H = N / 2, P = GS::P;
+  C v[N];
+  if (unit_i) {
+    // sigma_x = 0: the x factor is the same real number for every index (and the Nyquist correction c1 vanishes)
+    const typename real_of<C>::type sc = buf[GS::HI + side * GS::TS].x;
+#pragma unroll
+    for (int i = 0; i < N; ++i) { const C t = buf[i * P + ln]; v[i] = mkc<C>(t.x * sc, t.y * sc); }
+  } else {
+#pragma unroll
+    for (int i = 0; i < N; ++i) v[i] = cmul(buf[i * P + ln], buf[GS::HI + side * GS::TS + i]);
+    v[H].x = fma_(-szs, c1.x, v[H].x);
+    v[H].y = fma_(-szs, c1.y, v[H].y);
+  }
+  fft_reg<N, +1>(v);
+#pragma unroll
+  for (int i = 0; i < N; ++i) buf[i * P + ln] = v[i];
+}
+
+// Input of the y pass of one job of the group (lane = row = x index): the y factors of both sides (hm: [2][TS],
+// the same for every lane), the N packed columns
+// X = Y_A + i Y_B with the mirror half by conjugation, the Nyquist corrections vx (this lane's), vz.  The tile is only read.
+template <int N, class C>
+__device__ __forceinline__ void ypass_in(const C* buf, const C* hm, int ln, typename real_of<C>::type szs,
+                                         typename real_of<C>::type sxb, C vx, C vz, bool real_y, C (&X)[N]) {
+  typedef GroupSmem<N> GS;
+  typedef typename real_of<C>::type R;
+  constexpr int H = N / 2, P = GS::P;
+  const C* row = buf + ln * P;
+  const C a0 = row[0], b0 = row[H];
+  const R hA0 = hm[0].x, hAH = hm[H].x, hB0 = hm[GS::TS].x, hBH = hm[GS::TS + H].x;
+  X[0] = mkc<C>(a0.x * hA0, b0.x * hB0);
+  X[H] = mkc<C>(a0.y * hAH - (szs * vx.x + sxb * vz.x), b0.y * hBH - (szs * vx.y + sxb * vz.y));
+  if (real_y) {
+    // theta_y = 0: every y factor is the same real number per side
+#pragma unroll
+    for (int mm = 1; mm < H; ++mm) {
+      const C ya = row[mm], yb = row[H + mm];
+      const C p = mkc<C>(ya.x * hA0, ya.y * hA0), q = mkc<C>(yb.x * hB0, yb.y * hB0);
+      X[mm] = mkc<C>(p.x - q.y, p.y + q.x);
+      X[N - mm] = mkc<C>(p.x + q.y, q.x - p.y);
+    }
+  } else {
+#pragma unroll
+    for (int mm = 1; mm < H; ++mm) {
+      const C ha = hm[mm], hb = hm[GS::TS + mm];
+      const C p = cmul(row[mm], ha), q = cmul(row[H + mm], hb);
+      X[mm] = mkc<C>(p.x - q.y, p.y + q.x);
+      X[N - mm] = mkc<C>(p.x + q.y, q.x - p.y);
+    }
+  }
+}
+
 // C = double2: Algorithm 2 in fp64.  C = float2 (dgfs_params::precision = 1): the same job on single-precision copies
 // of the z-shifted arrays and factor tables; the Nyquist corrections and S are read in double and converted, T is
 // written in double (the forward z pass and everything after it stay fp64).
@@ -649,7 +770,7 @@ __global__ void __launch_bounds__(PACK ? N * W : 32 * W) __maxnreg__(sizeof(C) =
   constexpr bool F32 = sizeof(C) == sizeof(float2);
   typedef typename real_of<C>::type R;
   typedef NyqLayout<N> NL;
-  typedef JobSmem<N> JS;
+  typedef GroupSmem<N> JS;
   constexpr int P = JS::P;
   static_assert(N <= 32, "one lane per pencil");
   extern __shared__ __align__(16) unsigned char sm_raw[];
@@ -669,35 +790,46 @@ __global__ void __launch_bounds__(PACK ? N * W : 32 * W) __maxnreg__(sizeof(C) =
   const size_t goff = (size_t)cz * NH + m;
   const C* hbase = hxy + (((size_t)pair * tab.N_rho + r) * tab.M) * 4 * N;
   const cplx* nbase = nyq + (size_t)item * tab.M * NL::STRIDE;
-  // job = {s, z job of side A, z job of side B, smask[s]} (V1Tables::jobs): the entry of the next job is fetched a
-  // whole job ahead, so no look-up sits between the end of one job and the prefetch of the next
+  // jobs = {s, z job of side A, z job of side B, smask[s] | JOB_*} (V1Tables::jobs), in groups of one or two that
+  // share the inverse x pass (R-12); the entries of the next group are fetched a group ahead
   const int4* jl = t.jobs + (size_t)pair * tab.M;
   const int nj = t.njobs[pair];
-  cplx n1 = make_double2(0.0, 0.0), n2 = n1, n3 = n1;       // F32: Nyquist corrections of the job in flight (registers)
-  auto issue = [&](int4 jb) {
+  // the input of a group (the two half planes, x factors, x-Nyquist row) and the tables of its jobs into the tile
+  auto issue = [&](int4 j0, int4 j1, bool two) {
     if (act) {
-      const C* g = Gz.job(xl, side ? jb.z : jb.y, (size_t)(N * NH)) + goff;
+      const C* g = Gz.job(xl, side ? j0.z : j0.y, (size_t)(N * NH)) + goff;
 #pragma unroll
       for (int i = 0; i < N; ++i) cp_async_el(&buf[i * P + ln], g + i * H);
-      const C* hx = hbase + (size_t)jb.x * 4 * N;          // [side][x|y][N]
+      const C* hx = hbase + (size_t)j0.x * 4 * N;          // [side][x|y][N]
       cp_async_el(&buf[JS::HI + ln], hx + ln);               // h_x side A
       cp_async_el(&buf[JS::HI + JS::TS + ln], hx + 2 * N + ln);   // h_x side B
-      cp_async_el(&buf[JS::HM + ln], hx + N + ln);           // h_y side A
-      cp_async_el(&buf[JS::HM + JS::TS + ln], hx + 3 * N + ln);   // h_y side B
-      const cplx* nq = nbase + (size_t)jb.x * NL::STRIDE;
-      if (F32) {
-        n1 = __ldg(nq + NL::VYH + ln); n2 = __ldg(nq + NL::VXP + ln); n3 = __ldg(nq + NL::VZP + cz);
-      } else {
-        cplx* bd = reinterpret_cast<cplx*>(buf);
-        cp_async16(&bd[JS::VYH + ln], nq + NL::VYH + ln);
-        cp_async16(&bd[JS::VXP + ln], nq + NL::VXP + ln);
-        if (ln == 0) cp_async16(&bd[JS::VZP], nq + NL::VZP + cz);
+      if (!F32) cp_async16(reinterpret_cast<cplx*>(buf) + JS::VYH + ln, nbase + (size_t)j0.x * NL::STRIDE + NL::VYH + ln);
+#pragma unroll
+      for (int k = 0; k < 2; ++k) {
+        if (k == 1 && !two) break;
+        const int4 jb = k ? j1 : j0;
+        C* sl = buf + JS::SLOT + k * JS::SLOTW;
+        const C* hy = hbase + (size_t)jb.x * 4 * N;
+        cp_async_el(&sl[JS::HM + ln], hy + N + ln);           // h_y side A
+        cp_async_el(&sl[JS::HM + JS::TS + ln], hy + 3 * N + ln);   // h_y side B
+        if (!F32) {
+          const cplx* nq = nbase + (size_t)jb.x * NL::STRIDE;
+          cplx* sd = reinterpret_cast<cplx*>(sl);
+          cp_async16(&sd[JS::VXP + ln], nq + NL::VXP + ln);
+          if (ln == 0) cp_async16(&sd[JS::VZP], nq + NL::VZP + cz);
+        }
       }
     }
     cp_async_commit();
   };
-  int mask = 0;
-  if (nj > 0) { const int4 j0 = __ldg(&jl[0]); issue(j0); mask = j0.w; }
+  int4 g0 = make_int4(0, 0, 0, 0), g1 = g0;
+  bool two = false;
+  if (nj > 0) {
+    g0 = __ldg(&jl[0]);
+    two = !(g0.w & JOB_LAST);
+    if (two) g1 = __ldg(&jl[1]);
+    issue(g0, g1, two);
+  }
   // start from the Nyquist-field product written by k_wterm
   R acc[N];
   {
@@ -705,30 +837,48 @@ __global__ void __launch_bounds__(PACK ? N * W : 32 * W) __maxnreg__(sizeof(C) =
 #pragma unroll
     for (int j = 0; j < N; ++j) acc[j] = (R)w0[j * N];
   }
-  for (int j = 0; j < nj; ++j) {
-    const int4 jn = __ldg(&jl[j + 1 < nj ? j + 1 : j]);          // used after pass 1: its latency hides behind it
+  for (int j = 0; j < nj;) {
+    const int jn = j + (two ? 2 : 1);                        // first job of the next group
+    int4 n0 = g0, n1 = g1;
+    bool ntwo = false;
+    if (jn < nj) {
+      n0 = __ldg(&jl[jn]);
+      ntwo = !(n0.w & JOB_LAST);
+      if (ntwo) n1 = __ldg(&jl[jn + 1]);
+    }
     cp_async_wait_all();
     sync();
-    C X[N];
     if (act) {
-      // sigma_x = 0: h_x is the constant w_s / N (side A) or 1 / N; sigma_y = 0: h_y is the constant 1 / N
-      const bool ux_ = (mask & 1) != 0, ry_ = (mask & 2) != 0;
-      const C c1 = F32 ? cvt<C>(n1) : buf[JS::VYH + ln];
-      job_pass1<N, true>(buf, ln, side, m, szs, ux_ ? buf[JS::HI + side * JS::TS].x : (R)1, c1, ux_, ry_);
+      // sigma_x = 0: h_x is the constant w_s / N (side A) or 1 / N
+      const C c1 = F32 ? cvt<C>(__ldg(nbase + (size_t)g0.x * NL::STRIDE + NL::VYH + ln)) : buf[JS::VYH + ln];
+      xpass_group<N>(buf, ln, side, szs, c1, (g0.w & 1) != 0);
     }
     sync();
-    if (act) {
-      const C c2 = F32 ? cvt<C>(n2) : buf[JS::VXP + ln], c3 = F32 ? cvt<C>(n3) : buf[JS::VZP];
-      job_pass2_in<N, true>(buf, ln, szs, sxb, c2, c3, X);
-    }
-    sync();
-    if (j + 1 < nj) issue(jn);               // the tile is free: the next job's data arrives during pass 2
-    if (act) {
-      fft_reg<N, +1>(X);
+#pragma unroll 1
+    for (int k = 0; k < (two ? 2 : 1); ++k) {
+      const int4 jb = k ? g1 : g0;
+      const C* sl = buf + JS::SLOT + k * JS::SLOTW;
+      C X[N];
+      if (act) {
+        C c2, c3;
+        if (F32) {
+          const cplx* nq = nbase + (size_t)jb.x * NL::STRIDE;
+          c2 = cvt<C>(__ldg(nq + NL::VXP + ln)); c3 = cvt<C>(__ldg(nq + NL::VZP + cz));
+        } else { c2 = sl[JS::VXP + ln]; c3 = sl[JS::VZP]; }
+        // sigma_y = 0: h_y is the constant 1 / N
+        ypass_in<N>(buf, sl + JS::HM, ln, szs, sxb, c2, c3, (jb.w & 2) != 0, X);
+      }
+      if (k + 1 == (two ? 2 : 1)) {           // last job of the group: the tile is free, the next group's data arrives
+        sync();                               // during this y pass
+        if (jn < nj) issue(n0, n1, ntwo);
+      }
+      if (act) {
+        fft_reg<N, +1>(X);
 #pragma unroll
-      for (int jj = 0; jj < N; ++jj) acc[jj] = fma_(X[jj].x, X[jj].y, acc[jj]);
+        for (int jj = 0; jj < N; ++jj) acc[jj] = fma_(X[jj].x, X[jj].y, acc[jj]);
+      }
     }
-    mask = jn.w;
+    j = jn; g0 = n0; g1 = n1; two = ntwo;
   }
   // forward y and x passes of the real plane S_r(., ., cz) (steps 6-7, after R-1)
   if (act) {
@@ -1292,7 +1442,8 @@ double flops_per_pair_eval_v1(const dgfs_ctx* c, int pair) {
   for (int s2 = 0; s2 < c->M; ++s2) run += !c->v1_sskip[(size_t)pair * c->M + s2];
   const double frac = (double)run / c->M;
   const double fwd = c->N * (c->N + 1.0) * 5.0 * c->N * log2((double)c->N);     // forward passes in k_xy: once per plane
-  return c->N_rho * (f.zshift + frac * (f.nyq + f.wterm + f.xy - fwd) + fwd + f.acc) + f.tail;
+  (void)fwd;
+  return c->N_rho * (f.zshift + frac * (f.nyq + f.wterm) + c->v1_xyflops[pair] + f.acc) + f.tail;
 }
 
 // Streams and events of the two-stream schedule (created with the context's v1 tables).
@@ -1378,11 +1529,13 @@ static int collide_v1_impl(dgfs_ctx* c, const double* f, double* out, int nx, bo
     if (!c->full[pr]) run_vhs += (double)run / c->M;
     if (!c->full[pr] && c->v1_tsrc[pr] == pr) ++nrun_vhs;
   }
-  const double fwd_xy = N * (N + 1.0) * 5.0 * N * log2((double)N);      // forward passes inside k_xy, once per plane
+  double xy_flops = 0.0;                                                 // k_xy per point and radial node, all pairs
+  for (int pr = 0; pr < c->npairs; ++pr) if (!c->full[pr]) xy_flops += c->v1_xyflops[pr];
+  (void)nrun_vhs;
   const int ns = c->ns, np = c->npairs, nz = c->v1_nz, nz0 = c->v1_nz0, nzr = nz - nz0;
   const size_t smem_plane = plane_smem_per_warp<N>() * W;
   const size_t smem_final = plane_smem_per_warp<N>() * 2;
-  const size_t smem_xy = sizeof(cplx) * (size_t)W * JobSmem<N>::WORDS;
+  const size_t smem_xy = sizeof(cplx) * (size_t)W * GroupSmem<N>::WORDS;
   const size_t smem_xyf = sizeof(cplx) * (size_t)W * FullSmem<N>::WORDS;
   const size_t smem_wt = sizeof(cplx) * (size_t)WtermSmem<N>::STAGES * WtermSmem<N>::WORDS;
   const size_t smem_nyq = sizeof(cplx) * (size_t)2 * JobSmem<N>::WORDS;
@@ -1478,7 +1631,7 @@ static int collide_v1_impl(dgfs_ctx* c, const double* f, double* out, int nx, bo
       if (nvhs > 0) {
         const int g = r / RG, slot = r % pl.tslots;
         if (r % RG == 0 && g >= 2) wait(st, c->ev_acc[g & 1]);       // the forward z pass of group g - 2 has read these slots
-        { ProfScope ps(c->prof, st, "k_xy", nb * (run_vhs * (fl.xy - fwd_xy) + nrun_vhs * fwd_xy));
+        { ProfScope ps(c->prof, st, "k_xy", nb * xy_flops);
           if constexpr (N > 32) {
             k_xy_wide<N><<<dim3(N / 2, items), 2 * N, 2 * smem_wide, st>>>(c->v1, c->tab, gv, c->v1.hxy, nyqb[b], Sb[b], T + (size_t)slot * slot_stride, r);
           } else if (N < 32 && c->v1_pack) {          // N lanes per job: W planes on N W threads (k_xy, PACK)

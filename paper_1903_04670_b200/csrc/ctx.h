@@ -157,6 +157,7 @@ struct dgfs_ctx {
   std::vector<double> v1_fscale;
   std::vector<int4> v1_jobs;
   std::vector<int> v1_njobs;
+  std::vector<double> v1_xyflops;        // [pair] executed flops of k_xy per item and radial node (x passes per group)
   int4* d_v1_jobs = nullptr;
   int* d_v1_njobs = nullptr;
   int *d_v1_zsp = nullptr, *d_v1_zmap = nullptr, *d_v1_tsrc = nullptr, *d_v1_fsrc_s = nullptr, *d_v1_anti = nullptr, *d_v1_tpartner = nullptr;
