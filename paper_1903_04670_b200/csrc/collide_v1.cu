@@ -1,5 +1,5 @@
 // collide_v1.cu -- v1 pipeline of dgfs_collide (N <= 32; N = 48 with collide_v1_wide.cuh): Algorithm 2 of PAPER.md with the exact
-// rearrangements of DESIGN.md section 5 (R-1 .. R-11).  The description below is the path of pairs whose b_rs
+// rearrangements of DESIGN.md section 5 (R-1 .. R-12).  The description below is the path of pairs whose b_rs
 // does not depend on s (VHS, table_mode 0); pairs with a full table share the first three kernels and take
 // k_xy_full / k_zfwd_full afterwards (described there).
 //
