@@ -112,7 +112,10 @@ int dgfs_collide_pairs(dgfs_ctx *c, const double *f, double *Qpq, int nx, void *
  * times.  The device staging buffers are owned by the context and grown on demand. */
 int dgfs_collide_host(dgfs_ctx *c, const double *f_host, double *Q_host, int nx);
 
-/* Bytes of device workspace dgfs_collide* needs for a batch of nx points (tables excluded). */
+/* Bytes of device workspace dgfs_collide* needs for a batch of nx points (tables excluded).  A batch runs in launch
+ * groups of a fixed number of points; the group is halved until its workspace fits a byte budget fixed at
+ * dgfs_create: 70 % of the device memory free at that moment, or the environment variable DGFS_V1_WS_GB (in GB).
+ * Results do not depend on the group size. */
 size_t dgfs_workspace_bytes(const dgfs_ctx *c, int nx);
 
 /* Allocate the workspace for batches of up to nx points now, so that later dgfs_collide* calls

@@ -1341,13 +1341,9 @@ struct PlanV1 {
   int nbx, nbuf, tslots;
   size_t off_fhat, off_fhh, off_nyqy, off_qg, off_gzr[2], off_gz0, off_nyq[2], off_s[2], off_t, off_tf, off_fp, off_gin, off_gout, nyq_bytes, qstride, total;
 };
-PlanV1 plan_v1(const dgfs_ctx* c, int nx) {
+PlanV1 plan_v1_chunk(const dgfs_ctx* c, int nx, int nbx) {
   PlanV1 pl{};
   const size_t N = c->N, N3 = c->N3, arr = N3 * sizeof(cplx);
-  int nbx = c->v1_chunk;
-  if (nbx > nx) nbx = nx;
-  if (nbx < 1) nbx = 1;
-  if ((size_t)nbx * c->npairs > 65535) nbx = 65535 / c->npairs;
   pl.nbx = nbx;
   // two-stream schedule: the buffers filled by the preparing kernels exist twice (radial nodes r and r + 1 in flight)
   pl.nbuf = c->v1_overlap ? 2 : 1;
@@ -1386,6 +1382,21 @@ PlanV1 plan_v1(const dgfs_ctx* c, int nx) {
   pl.off_gin = take(small ? (size_t)nx * c->ns * N3 * sizeof(double) : 0);
   pl.off_gout = take(small ? (size_t)nx * c->npairs * N3 * sizeof(double) : 0);
   pl.total = off;
+  return pl;
+}
+// The launch group: v1_chunk spatial points, fewer when the batch is smaller, when the grid's y extent would pass
+// 65535, or when the workspace of the group would pass the context's byte budget (ws_budget: 70 % of the memory free
+// at create, or DGFS_V1_WS_GB) -- then it is halved until it fits.  Results do not depend on the group size.
+PlanV1 plan_v1(const dgfs_ctx* c, int nx) {
+  int nbx = c->v1_chunk;
+  if (nbx > nx) nbx = nx;
+  if (nbx < 1) nbx = 1;
+  if ((size_t)nbx * c->npairs > 65535) nbx = 65535 / c->npairs;
+  PlanV1 pl = plan_v1_chunk(c, nx, nbx);
+  while (c->ws_budget > 0 && pl.total > c->ws_budget && nbx > 1) {
+    nbx = (nbx + 1) / 2;
+    pl = plan_v1_chunk(c, nx, nbx);
+  }
   return pl;
 }
 }  // namespace
@@ -1460,6 +1471,12 @@ int init_streams_v1(dgfs_ctx* c) {
   c->v1_pack = (pk && atoi(pk) != 0);      // measured at c1 (N = 24): 119.5 against 113.2 ms of k_xy per 3 steps, off by default
   const char* xw = getenv("DGFS_V1_XYW");
   c->v1_xyw = (xw && atoi(xw) == 2) ? 2 : 4;
+  // byte budget of the workspace of one launch group (plan_v1): DGFS_V1_WS_GB, else 70 % of the memory free now
+  const char* wb = getenv("DGFS_V1_WS_GB");
+  size_t freeb = 0, totalb = 0;
+  if (wb && atof(wb) > 0) c->ws_budget = (size_t)(atof(wb) * 1e9);
+  else if (cudaMemGetInfo(&freeb, &totalb) == cudaSuccess) c->ws_budget = (size_t)(0.7 * (double)freeb);
+  else cudaGetLastError();
   if (!c->v1_overlap) return DGFS_OK;
   int least = 0, greatest = 0;
   cudaDeviceGetStreamPriorityRange(&least, &greatest);

@@ -151,6 +151,7 @@ struct dgfs_ctx {
   // v1 pipeline (collide_v1.cu): tables built by build_tables_v1, used for N <= 32
   bool use_v1 = false;
   int v1_chunk = 512;                    // spatial points per launch group (large launches amortise the tails)
+  size_t ws_budget = 0;                  // bytes the workspace of one launch group may take (0: no limit); plan_v1
   int v1_rgroup = 16;                    // radial nodes per forward-z / QG accumulation launch
   int v1_nz = 0, v1_nz0 = 0;             // z jobs; the last v1_nz0 of them have sigma_z = 0
   std::vector<int> v1_zsp, v1_zmap, v1_tsrc, v1_fsrc_s, v1_anti, v1_tpartner;

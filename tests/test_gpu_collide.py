@@ -305,6 +305,22 @@ def test_v1_batch_consistency_and_chunking(torch_cuda, monkeypatch):
         assert torch.equal(op.collide(f), Qs)
 
 
+def test_v1_workspace_budget_shrinks_the_launch_group(torch_cuda, monkeypatch):
+    """The launch group is halved until its workspace fits the byte budget (70 % of the free memory at create, or
+    DGFS_V1_WS_GB); the result does not change by a bit."""
+    torch = torch_cuda
+    cfg = _rand_cfg("t", 2, 16, 3, 12, (1.0, 1.0), (0.6, 0.8), (1.0, 2.0), seed=9)
+    f = torch.from_numpy(make_points(cfg, range(40))).cuda()
+    with _gpu_op(cfg) as op:
+        big = op.workspace_bytes(40)
+        Qb = op.collide_pairs(f).clone()
+    monkeypatch.setenv("DGFS_V1_WS_GB", "%.9f" % (0.3 * big / 1e9))
+    with _gpu_op(cfg) as op:
+        small = op.workspace_bytes(40)
+        assert small <= 0.3 * big * 1.3 and small < big
+        assert torch.equal(op.collide_pairs(f), Qb)
+
+
 def test_v1_mixed_pairs_batch_consistency_and_chunking(torch_cuda, monkeypatch):
     """3 species, pair (0,0) VHS and the other eight VSS in one context: the two kinds share the z shifts and
     the Nyquist fields and take different kernels afterwards; chunking must not change a bit."""
