@@ -112,6 +112,22 @@ int dgfs_collide_pairs(dgfs_ctx *c, const double *f, double *Qpq, int nx, void *
  * times.  The device staging buffers are owned by the context and grown on demand. */
 int dgfs_collide_host(dgfs_ctx *c, const double *f_host, double *Q_host, int nx);
 
+/* dgfs_collide for callers that must not allocate device memory (their own CUDA graph capture, a serving loop, a
+ * harness that forbids cudaMalloc): same kernels, same launch order and same result as dgfs_collide, bit for bit, but
+ * the workspace is a static device array of DGFS_NOALLOC_SCRATCH_BYTES inside the library instead of the context's
+ * allocation; the call makes no cudaMalloc / cudaFree / cudaMallocAsync and no call that allocates on its behalf
+ * (no CUDA graph is built, the context's workspace is not grown).  Every GPU that loads the library holds the array
+ * until the process exits.  f, Q, nx, stream: as dgfs_collide.  The batch runs in launch groups small enough for
+ * the array; the call fails with DGFS_EINVAL, before any launch, when one spatial point alone needs more (compare
+ * dgfs_workspace_bytes(c, 1): about 13 MB at N = 32, 2 species; N = 48 does not fit), with DGFS_ENOSUP for a context
+ * on the v0 pipeline (N = 48 with VSS pairs, DGFS_PIPELINE=v0) or with per-launch profiling switched on.
+ * The array is shared by every context and every call of the process on that GPU and keeps what the last call left;
+ * no kernel reads it before writing it, so nothing has to be cleared.  Calls that overlap on the GPU (two streams,
+ * two contexts, two host threads) race on it: the caller orders them.  Calls of ONE context are ordered by the
+ * library as for dgfs_collide.  The first call of a context sets kernel attributes (not an allocation). */
+#define DGFS_NOALLOC_SCRATCH_BYTES (64u << 20)
+int dgfs_collide_noalloc(dgfs_ctx *c, const double *f, double *Q, int nx, void *stream);
+
 /* Bytes of device workspace dgfs_collide* needs for a batch of nx points (tables excluded).  A batch runs in launch
  * groups of a fixed number of points; the group is halved until its workspace fits a byte budget fixed at
  * dgfs_create: 70 % of the device memory free at that moment, or the environment variable DGFS_V1_WS_GB (in GB).

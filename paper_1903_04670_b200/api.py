@@ -20,6 +20,7 @@ ABI_SYMBOLS = (
     "dgfs_flops_per_pair_eval", "dgfs_step", "dgfs_step_euler", "dgfs_advect_rhs",
     "dgfs_launch_count", "dgfs_profile_enable", "dgfs_profile_count", "dgfs_profile_get",
     "dgfs_profile_reset", "dgfs_collide_host", "dgfs_measure_fp64_peak", "dgfs_table_bytes", "dgfs_measure_dft",
+    "dgfs_collide_noalloc",
 )
 
 DGFS_OK, DGFS_EINVAL, DGFS_ECUDA, DGFS_ENOMEM, DGFS_ENOSUP = 0, -1, -2, -3, -4
@@ -87,7 +88,7 @@ def load_library():
     lib.dgfs_destroy.restype = None
     lib.dgfs_last_error.argtypes = [vp]
     lib.dgfs_last_error.restype = C.c_char_p
-    for name in ("dgfs_collide", "dgfs_collide_pairs"):
+    for name in ("dgfs_collide", "dgfs_collide_pairs", "dgfs_collide_noalloc"):
         fn = getattr(lib, name)
         fn.argtypes = [vp, vp, vp, ip, vp]
         fn.restype = ip
@@ -202,6 +203,11 @@ def _dev(t, who):
 def dgfs_collide(ctx, f, Q, nx):
     """Q[x][p][:] = sum_q beta_pq Q^(pq)(f[x][p], f[x][q])  on the current torch stream."""
     _check(ctx, load_library().dgfs_collide(ctx, _dev(f, "f"), _dev(Q, "Q"), int(nx), _stream_ptr()))
+
+
+def dgfs_collide_noalloc(ctx, f, Q, nx):
+    """dgfs_collide out of the library's static device scratch (no device allocation; include/dgfs.h)."""
+    _check(ctx, load_library().dgfs_collide_noalloc(ctx, _dev(f, "f"), _dev(Q, "Q"), int(nx), _stream_ptr()))
 
 
 def dgfs_collide_pairs(ctx, f, Qpq, nx):
@@ -354,6 +360,11 @@ class Dgfs:
         if out is None:
             out = torch.empty((nx, self.ns, self.N3), dtype=torch.float64, device=f.device)
         dgfs_collide(self.ctx, f, out, nx)
+        return out
+
+    def collide_noalloc(self, f, out):
+        """dgfs_collide_noalloc: `out` is the caller's ([nx][ns][N^3], fp64, CUDA); nothing is allocated."""
+        dgfs_collide_noalloc(self.ctx, f, out, f.shape[0])
         return out
 
     def collide_pairs(self, f, out=None):

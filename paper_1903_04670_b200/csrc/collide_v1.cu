@@ -32,6 +32,7 @@
 #include <cmath>
 #include <cstdio>
 #include <cstdlib>
+#include <mutex>
 #include "ctx.h"
 #include "kernels_v0.cuh"
 
@@ -1767,3 +1768,71 @@ int run_collide_v1(dgfs_ctx* c, const double* f, double* out, int nx, bool pairs
 }
 
 }  // namespace dgfs
+
+// ---------------------------------------------------------------- dgfs_collide_noalloc ------------
+// The v1 pipeline above with its workspace in a file-scope device array instead of the context's stream-ordered
+// allocation: for callers that must not allocate (a caller's own graph capture, a serving loop, a harness that forbids
+// cudaMalloc).  Every GPU that loads the library holds DGFS_NOALLOC_SCRATCH_BYTES of device memory for this array until
+// the process exits.  Host code must not pass the symbol itself to a kernel (there it names a host-side stand-in): the
+// device address is asked for once per device, with that device current, and kept.
+static __device__ __align__(256) unsigned char g_noalloc_scratch[DGFS_NOALLOC_SCRATCH_BYTES];
+
+namespace {
+constexpr int NOALLOC_MAX_DEVICES = 64;
+std::mutex g_noalloc_mutex;
+void* g_noalloc_ptr[NOALLOC_MAX_DEVICES] = {};
+
+// puts the context's workspace fields back however the call ends
+struct WorkspaceSwap {
+  dgfs_ctx* c; void* ws; size_t ws_bytes, ws_budget;
+  WorkspaceSwap(dgfs_ctx* c_, void* p, size_t bytes) : c(c_), ws(c_->ws), ws_bytes(c_->ws_bytes), ws_budget(c_->ws_budget) {
+    c->ws = p; c->ws_bytes = bytes;
+    if (c->ws_budget == 0 || c->ws_budget > bytes) c->ws_budget = bytes;      // plan_v1 halves the launch group to fit
+  }
+  ~WorkspaceSwap() { c->ws = ws; c->ws_bytes = ws_bytes; c->ws_budget = ws_budget; }
+};
+}  // namespace
+
+extern "C" int dgfs_collide_noalloc(dgfs_ctx* c, const double* f, double* Q, int nx, void* stream) {
+  using namespace dgfs;
+  if (!c) return DGFS_EINVAL;
+  if (nx < 0) return set_error(c, DGFS_EINVAL, "dgfs_collide_noalloc: nx must be >= 0");
+  if (nx == 0) return DGFS_OK;
+  if (!f || !Q) return set_error(c, DGFS_EINVAL, "dgfs_collide_noalloc: f and Q must not be NULL");
+  if ((const void*)f == (const void*)Q) return set_error(c, DGFS_EINVAL, "dgfs_collide_noalloc: Q must not alias f");
+  if (!c->use_v1) return set_error(c, DGFS_ENOSUP, "dgfs_collide_noalloc: only contexts on the v1 pipeline (N <= 32, or N = 48 without VSS pairs)");
+  if (c->prof.on) return set_error(c, DGFS_ENOSUP, "dgfs_collide_noalloc: per-launch profiling creates events; switch it off (dgfs_profile_enable)");
+  if (c->device < 0 || c->device >= NOALLOC_MAX_DEVICES) return set_error(c, DGFS_ENOSUP, "dgfs_collide_noalloc: device index beyond 63");
+  cudaError_t e = cudaSetDevice(c->device);
+  if (e != cudaSuccess) return check_cuda(c, e, "cudaSetDevice");
+  void* scratch = nullptr;
+  {
+    std::lock_guard<std::mutex> lock(g_noalloc_mutex);
+    if (!g_noalloc_ptr[c->device]) {                  // once per device, that device current
+      void* p = nullptr;
+      e = cudaGetSymbolAddress(&p, g_noalloc_scratch);
+      if (e != cudaSuccess || !p) return check_cuda(c, e != cudaSuccess ? e : cudaErrorInvalidSymbol, "dgfs_collide_noalloc: cudaGetSymbolAddress");
+      g_noalloc_ptr[c->device] = p;
+    }
+    scratch = g_noalloc_ptr[c->device];
+  }
+  cudaStream_t st = (cudaStream_t)stream;
+  WorkspaceSwap swap(c, scratch, (size_t)DGFS_NOALLOC_SCRATCH_BYTES);
+  const size_t need = workspace_bytes_v1(c, nx);       // with the launch group already halved towards the limit
+  if (need > (size_t)DGFS_NOALLOC_SCRATCH_BYTES) {
+    char msg[256];
+    snprintf(msg, sizeof msg, "dgfs_collide_noalloc: one spatial point of this configuration needs %zu bytes of workspace, "
+             "the static scratch holds %zu (DGFS_NOALLOC_SCRATCH_BYTES): use dgfs_collide", need, (size_t)DGFS_NOALLOC_SCRATCH_BYTES);
+    return set_error(c, DGFS_EINVAL, msg);
+  }
+  cudaStreamCaptureStatus cap = cudaStreamCaptureStatusNone;
+  cudaStreamIsCapturing(st, &cap);
+  const bool capturing = cap != cudaStreamCaptureStatusNone;
+  if (!capturing && c->ev_last_set) cudaStreamWaitEvent(st, c->ev_last, 0);      // calls of one context stay ordered
+  // Nothing in the workspace has to start from zero: every buffer is written by an earlier kernel of the same call
+  // before it is read (the r = 0 launches of k_zfwd_acc / k_zfwd_full store QG, the later ones add to it), the
+  // Nyquist-filter variant clears its fields itself.  So the contents the last call left behind are never read.
+  const int rc = dispatch_v1(c, f, Q, nx, false, st);    // straight to the kernels: no graph, no ensure_workspace growth
+  if (!capturing && c->ev_last) { cudaEventRecord(c->ev_last, st); c->ev_last_set = true; }
+  return rc;
+}
