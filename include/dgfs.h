@@ -179,6 +179,14 @@ int dgfs_profile_reset(dgfs_ctx *c);
  * either may be NULL.  Synchronous; needs no context. */
 int dgfs_measure_fp64_peak(int device, double seconds, double *tflops_burst, double *tflops_sustained);
 
+/* Do the plain FP64 pipe (DFMA) and the FP64 tensor path (mma.sync.m8n8k4.f64) of `device` run side by side?  A kernel
+ * in which every thread carries n_dfma independent DFMA chains and every warp n_dmma independent MMA chains, no memory
+ * traffic, timed for about `seconds` (0 < seconds <= 30); (n_dfma, n_dmma) one of (8,0), (0,8), (8,8), (8,2), (4,4),
+ * else DGFS_EINVAL.  Host outputs (either may be NULL): the TFLOP/s each kind of instruction reached in the best launch
+ * (m8n8k4 = 512 flop).  Separate pipes would give a mixed run both pure rates at once; B200 gives their times added
+ * (profiles/r02_dft_probe.md).  Synchronous; needs no context. */
+int dgfs_measure_fp64_mix(int device, int n_dfma, int n_dmma, double seconds, double *tflops_dfma, double *tflops_dmma);
+
 /* Evidence for the transform kernels' design (BASELINE.json north_star: "shared-memory radix stages ... or per-axis DFT as
  * a dense contraction on FP64 tensor cores where N makes that the faster choice"): complex 1-D DFTs of length N
  * (8, 16, 24, 32 or 48) per second on `device`, on chip (registers / shared memory only inside the timed loop), by

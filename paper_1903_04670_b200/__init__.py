@@ -11,7 +11,7 @@ from .api import (DgfsError, Dgfs, Mesh1D, load_library, library_path, exported_
                   dgfs_get_tables, dgfs_flops_per_pair_eval, dgfs_last_error,
                   dgfs_launch_count, dgfs_profile_enable, dgfs_profile_count, dgfs_profile_get,
                   dgfs_profile_reset, dgfs_collide_host, dgfs_measure_fp64_peak, dgfs_table_bytes, dgfs_measure_dft,
-                  dgfs_collide_noalloc)
+                  dgfs_collide_noalloc, dgfs_measure_fp64_mix)
 from . import api
 
 __all__ = [
@@ -20,5 +20,5 @@ __all__ = [
     "dgfs_destroy", "dgfs_reserve", "dgfs_workspace_bytes", "dgfs_get_quadrature",
     "dgfs_get_tables", "dgfs_flops_per_pair_eval", "dgfs_last_error",
     "dgfs_launch_count", "dgfs_profile_enable", "dgfs_profile_count", "dgfs_profile_get",
-    "dgfs_profile_reset", "dgfs_collide_host", "dgfs_measure_fp64_peak", "dgfs_table_bytes", "dgfs_measure_dft", "dgfs_collide_noalloc", "api",
+    "dgfs_profile_reset", "dgfs_collide_host", "dgfs_measure_fp64_peak", "dgfs_table_bytes", "dgfs_measure_dft", "dgfs_collide_noalloc", "dgfs_measure_fp64_mix", "api",
 ]

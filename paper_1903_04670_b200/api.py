@@ -20,7 +20,7 @@ ABI_SYMBOLS = (
     "dgfs_flops_per_pair_eval", "dgfs_step", "dgfs_step_euler", "dgfs_advect_rhs",
     "dgfs_launch_count", "dgfs_profile_enable", "dgfs_profile_count", "dgfs_profile_get",
     "dgfs_profile_reset", "dgfs_collide_host", "dgfs_measure_fp64_peak", "dgfs_table_bytes", "dgfs_measure_dft",
-    "dgfs_collide_noalloc",
+    "dgfs_collide_noalloc", "dgfs_measure_fp64_mix",
 )
 
 DGFS_OK, DGFS_EINVAL, DGFS_ECUDA, DGFS_ENOMEM, DGFS_ENOSUP = 0, -1, -2, -3, -4
@@ -96,6 +96,8 @@ def load_library():
     lib.dgfs_collide_host.restype = ip
     lib.dgfs_measure_fp64_peak.argtypes = [ip, C.c_double, _dp, _dp]
     lib.dgfs_measure_fp64_peak.restype = ip
+    lib.dgfs_measure_fp64_mix.argtypes = [ip, ip, ip, C.c_double, _dp, _dp]
+    lib.dgfs_measure_fp64_mix.restype = ip
     lib.dgfs_workspace_bytes.argtypes = [vp, ip]
     lib.dgfs_workspace_bytes.restype = C.c_size_t
     lib.dgfs_measure_dft.argtypes = [ip, ip, ip, C.c_double, _dp, _dp]
@@ -239,6 +241,15 @@ def dgfs_measure_fp64_peak(device=0, seconds=1.0):
     rc = load_library().dgfs_measure_fp64_peak(int(device), float(seconds), C.byref(a), C.byref(b))
     if rc != DGFS_OK:
         raise DgfsError(rc, "dgfs_measure_fp64_peak failed")
+    return a.value, b.value
+
+
+def dgfs_measure_fp64_mix(device=0, n_dfma=8, n_dmma=8, seconds=0.5):
+    """(DFMA TFLOP/s, DMMA TFLOP/s) of a kernel that issues both kinds of FP64 instruction side by side."""
+    a, b = C.c_double(), C.c_double()
+    rc = load_library().dgfs_measure_fp64_mix(int(device), int(n_dfma), int(n_dmma), float(seconds), C.byref(a), C.byref(b))
+    if rc != DGFS_OK:
+        raise DgfsError(rc, "dgfs_measure_fp64_mix failed")
     return a.value, b.value
 
 

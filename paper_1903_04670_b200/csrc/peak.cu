@@ -225,3 +225,74 @@ extern "C" int dgfs_measure_dft(int device, int N, int method, double seconds, d
   }
   return DGFS_EINVAL;
 }
+
+// ------------------------------------------------------------------------------------------------------------------
+// dgfs_measure_fp64_mix: do the plain FP64 pipe (DFMA) and the FP64 tensor path (mma.sync.m8n8k4.f64, SASS DMMA) run
+// side by side, or is it one unit?  Every thread carries n_dfma independent DFMA chains and every warp n_dmma independent
+// MMA chains in the same unrolled loop; no memory traffic.  If the two were separate pipes a mixed kernel would take the
+// longer of the two pure times; on B200 the times ADD (profiles/r02_dft_probe.md): a plane job cannot hand part of its
+// arithmetic to the tensor path to get past the DFMA rate.
+namespace {
+__device__ __forceinline__ void dmma_884(double& c0, double& c1, double a, double b) {
+  asm volatile("mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%0,%1}, {%2}, {%3}, {%0,%1};\n" : "+d"(c0), "+d"(c1) : "d"(a), "d"(b));
+}
+template <int NF, int NM>
+__global__ void __launch_bounds__(256) k_fp64_mix(double* out, int iters, double a, double b) {
+  double x[8], c[8][2];
+#pragma unroll
+  for (int i = 0; i < 8; ++i) { x[i] = threadIdx.x * 1e-3 + i; c[i][0] = i; c[i][1] = -i; }
+  for (int it = 0; it < iters; ++it) {
+#pragma unroll
+    for (int u = 0; u < 8; ++u) {
+#pragma unroll
+      for (int j = 0; j < NF; ++j) x[j] = fma(x[j], a, b);
+#pragma unroll
+      for (int j = 0; j < NM; ++j) dmma_884(c[j][0], c[j][1], a, b);
+    }
+  }
+  double s = 0.0;
+#pragma unroll
+  for (int i = 0; i < 8; ++i) s += x[i] + c[i][0] + c[i][1];
+  if (s == 123.456) out[0] = s;     // never true: keeps the chains alive
+}
+template <int NF, int NM>
+int run_mix(int device, double seconds, double* tf_dfma, double* tf_dmma) {
+  cudaDeviceProp prop;
+  if (cudaGetDeviceProperties(&prop, device) != cudaSuccess) return DGFS_ECUDA;
+  double* d = nullptr;
+  if (cudaMalloc(&d, 8) != cudaSuccess) return DGFS_ENOMEM;
+  const int blocks = prop.multiProcessorCount * 4, iters = 2000;
+  cudaEvent_t e0, e1;
+  cudaEventCreate(&e0); cudaEventCreate(&e1);
+  k_fp64_mix<NF, NM><<<blocks, 256>>>(d, iters, 0.999999, 1e-9);
+  cudaDeviceSynchronize();
+  double best = 1e30, total = 0.0;
+  while (total < seconds * 1e3) {
+    cudaEventRecord(e0);
+    k_fp64_mix<NF, NM><<<blocks, 256>>>(d, iters, 0.999999, 1e-9);
+    cudaEventRecord(e1);
+    if (cudaEventSynchronize(e1) != cudaSuccess) { cudaFree(d); return DGFS_ECUDA; }
+    float ms = 0; cudaEventElapsedTime(&ms, e0, e1);
+    if (ms < best) best = ms;
+    total += ms;
+  }
+  cudaEventDestroy(e0); cudaEventDestroy(e1); cudaFree(d);
+  // thread-level DFMAs (2 flop) and warp-level m8n8k4 MMAs (512 flop) of the best launch
+  const double nf = (double)NF * 8 * iters * 256.0 * blocks, nm = (double)NM * 8 * iters * 8.0 * blocks;
+  if (tf_dfma) *tf_dfma = 2.0 * nf / (best * 1e-3) / 1e12;
+  if (tf_dmma) *tf_dmma = 512.0 * nm / (best * 1e-3) / 1e12;
+  return DGFS_OK;
+}
+}  // namespace
+
+extern "C" int dgfs_measure_fp64_mix(int device, int n_dfma, int n_dmma, double seconds, double* tflops_dfma, double* tflops_dmma) {
+  if (seconds <= 0 || seconds > 30) return DGFS_EINVAL;
+  if (cudaSetDevice(device) != cudaSuccess) return DGFS_ECUDA;
+  if (n_dfma == 8 && n_dmma == 0) return run_mix<8, 0>(device, seconds, tflops_dfma, tflops_dmma);
+  if (n_dfma == 0 && n_dmma == 8) return run_mix<0, 8>(device, seconds, tflops_dfma, tflops_dmma);
+  if (n_dfma == 8 && n_dmma == 8) return run_mix<8, 8>(device, seconds, tflops_dfma, tflops_dmma);
+  if (n_dfma == 8 && n_dmma == 2) return run_mix<8, 2>(device, seconds, tflops_dfma, tflops_dmma);
+  if (n_dfma == 4 && n_dmma == 4) return run_mix<4, 4>(device, seconds, tflops_dfma, tflops_dmma);
+  return DGFS_EINVAL;      // chains per thread / per warp: (8,0), (0,8), (8,8), (8,2), (4,4)
+}
+

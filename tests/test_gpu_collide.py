@@ -479,6 +479,27 @@ def test_dft_probe_both_methods_compute_the_dft(torch_cuda, N):
            rates[0] / rates[1], 1.0)
 
 
+def test_fp64_mix_probe_dfma_and_dmma_share_one_pipe(torch_cuda):
+    """dgfs_measure_fp64_mix: both kinds of FP64 instruction reach the pipe's rate alone; issued side by side their
+    rates do not add up to more than one pipe's worth (they would, up to ~2x, on separate pipes).  The figures go to the
+    log (profiles/r02_dft_probe.md); asserted loosely: the combined rate stays below 1.3x the better pure rate."""
+    from oracle_pool import record
+    from paper_1903_04670_b200 import dgfs_measure_fp64_mix, DgfsError
+    f_only, _ = dgfs_measure_fp64_mix(0, 8, 0, 0.2)
+    _, m_only = dgfs_measure_fp64_mix(0, 0, 8, 0.2)
+    f_mix, m_mix = dgfs_measure_fp64_mix(0, 8, 8, 0.2)
+    f_mix2, m_mix2 = dgfs_measure_fp64_mix(0, 8, 2, 0.2)
+    print("fp64 mix: DFMA alone %.2f, DMMA alone %.2f, mixed 8+8: %.2f + %.2f, mixed 8+2: %.2f + %.2f TFLOP/s" % (
+        f_only, m_only, f_mix, m_mix, f_mix2, m_mix2))
+    assert f_only > 10.0 and m_only > 10.0
+    for f, m in ((f_mix, m_mix), (f_mix2, m_mix2)):
+        record("fp64-mix", "DFMA %.2f + DMMA %.2f TFLOP/s side by side, sum / better pure rate" % (f, m),
+               (f + m) / max(f_only, m_only), 1.3)
+        assert f + m < 1.3 * max(f_only, m_only)
+    with pytest.raises(DgfsError):
+        dgfs_measure_fp64_mix(0, 3, 5, 0.1)
+
+
 def test_calls_on_two_streams_of_one_context_do_not_race(torch_cuda):
     """The workspace belongs to one call at a time: a call on another stream, issued without any host or stream
     synchronisation, waits for the previous call's last launch (include/dgfs.h: calls on one context are ordered)."""
