@@ -1024,32 +1024,65 @@ __global__ void __launch_bounds__(32 * W) k_xy_full(V1Tables t, DevTables tab, G
 //   QG[partner item]  += w_r f b^(qp)_rs' u                    the transposed pair, which ran nothing (R-11)
 // with f = fscale of the target (ratio of sphere weights).  Thread pair per pencil as in k_zfwd_acc; the sums
 // over s stay in registers.  b is read in SPEC layout [r][s][kz][kx][ky].
+template <int N>
+struct ZaccSmem {
+  static constexpr int PB = 64, STAGES = 3, WORDS = N * PB;
+};
+// The rows of Tf (64 pencils x N values of z per sphere point) are staged in shared memory by cp.async, a ring of three
+// stages over the sphere points that ran, as k_zfwd_acc stages the radial nodes of T: the loads of the next two points are
+// in flight while the current one is transformed, and both threads of a pencil read each element from the stage.
 template <int N, bool FIRST>
-__global__ void __launch_bounds__(256, N <= 24 ? 2 : 1) k_zfwd_full(DevTables tab, V1Tables t, const cplx* __restrict__ Tf,
+__global__ void __launch_bounds__(128) k_zfwd_full(DevTables tab, V1Tables t, const cplx* __restrict__ Tf,
                                                    cplx* __restrict__ QG, size_t qstride, int r) {
   constexpr int H = N / 2, N2 = N * N, N3 = N2 * N;
-  const int par = threadIdx.x >> 7;
-  const int pid = blockIdx.x * 128 + (threadIdx.x & 127);
+  typedef ZaccSmem<N> ZS;
+  constexpr int PB = ZS::PB, NS = ZS::STAGES;
+  extern __shared__ cplx sm[];
+  const int par = threadIdx.x >> 6, pl = threadIdx.x & 63;
+  const int pid0 = blockIdx.x * PB, pid = pid0 + pl;
   const int item = blockIdx.y, pair = item % tab.npairs;
-  if (pid >= N2 || !tab.full[pair] || t.tsrc[pair] != pair) return;
+  if (!tab.full[pair] || t.tsrc[pair] != pair) return;      // uniform per block
   const int M = tab.M;
   const int partner = t.tpartner[pair];                 // pair that reads this one's products, or -1
-  const int kxs = sfreq(pid / N, N), kys = sfreq(pid % N, N);
   const unsigned char* skip = t.sskip + (size_t)pair * M;
+  auto next_s = [&](int s) { while (s < M && skip[s]) ++s; return s; };
+  const cplx* tbase = Tf + (size_t)item * M * N3 + pid0;
+  auto issue = [&](int s, int slot) {
+    cplx* dstb = sm + (size_t)slot * ZS::WORDS;
+    const cplx* srcb = tbase + (size_t)s * N3;
+#pragma unroll
+    for (int q = threadIdx.x; q < N * PB; q += 128) {
+      const int jj = q / PB, col = q % PB;
+      if (pid0 + col < N2) cp_async16(&dstb[q], srcb + (size_t)jj * N2 + col);
+    }
+  };
+  int s_iss = next_s(0);
+#pragma unroll
+  for (int k = 0; k < NS - 1; ++k) {
+    if (s_iss < M) { issue(s_iss, k); s_iss = next_s(s_iss + 1); }
+    cp_async_commit();
+  }
+  const bool live = pid < N2;
+  const int pc = live ? pid : 0;
+  const int kxs = sfreq(pc / N, N), kys = sfreq(pc % N, N);
   const double scale = tab.w_rho[r];
   cplx acc[H], acc2[H];
 #pragma unroll
   for (int k = 0; k < H; ++k) acc[k] = acc2[k] = make_double2(0.0, 0.0);
-  for (int s = 0; s < M; ++s) {
-    if (skip[s]) continue;
-    const cplx* src = Tf + ((size_t)item * M + s) * N3 + pid;
+  for (int s = next_s(0), j = 0; s < M; s = next_s(s + 1), ++j) {
+    cp_async_wait_pending<NS - 2>();
+    __syncthreads();                            // stage j has landed; the stage of j - 1 is free
+    if (s_iss < M) { issue(s_iss, (j + NS - 1) % NS); s_iss = next_s(s_iss + 1); }
+    cp_async_commit();
+    if (!live) continue;
+    const cplx* src = sm + (size_t)(j % NS) * ZS::WORDS + pl;
     cplx u[H];
     if (par == 0) {
 #pragma unroll
-      for (int j = 0; j < H; ++j) u[j] = cadd(src[(size_t)j * N2], src[(size_t)(j + H) * N2]);
+      for (int jj = 0; jj < H; ++jj) u[jj] = cadd(src[jj * PB], src[(jj + H) * PB]);
     } else {
 #pragma unroll
-      for (int j = 0; j < H; ++j) u[j] = twiddle_mul<N, -1>(csub(src[(size_t)j * N2], src[(size_t)(j + H) * N2]), j);
+      for (int jj = 0; jj < H; ++jj) u[jj] = twiddle_mul<N, -1>(csub(src[jj * PB], src[(jj + H) * PB]), jj);
     }
     fft_reg<H, -1>(u);
     const int sa = t.anti[s];
@@ -1071,6 +1104,7 @@ __global__ void __launch_bounds__(256, N <= 24 ? 2 : 1) k_zfwd_full(DevTables ta
       if (partner >= 0) { const cplx b3v = b3.p[zi * b3.sz]; acc2[k] = cfma(make_double2(fp * b3v.x, fp * b3v.y), u[k], acc2[k]); }
     }
   }
+  if (!live) return;
   cplx* dst = QG + (size_t)item * qstride + pid;
   cplx* dst2 = QG + (size_t)(item - pair + (partner >= 0 ? partner : pair)) * qstride + pid;
 #pragma unroll
@@ -1226,10 +1260,6 @@ __global__ void __launch_bounds__(WtermSmem<N>::THREADS, N > 32 ? 1 : 2) k_wterm
 // The rows of T (64 pencils x N values of z per radial node) are staged in shared memory by cp.async, a ring of three
 // stages: the loads of the next two radial nodes are in flight while the current one is transformed, without holding
 // registers, and every element of T is fetched once (the two threads of a pencil read it from the stage).
-template <int N>
-struct ZaccSmem {
-  static constexpr int PB = 64, STAGES = 3, WORDS = N * PB;
-};
 template <int N, bool FIRST>
 __global__ void __launch_bounds__(128) k_zfwd_acc(DevTables tab, const int* __restrict__ tsrc, const cplx* __restrict__ T,
                                                   size_t slot_stride, cplx* __restrict__ QGh, size_t qstride, int r0, int nr) {
@@ -1581,6 +1611,10 @@ static int collide_v1_impl(dgfs_ctx* c, const double* f, double* out, int nx, bo
     cudaFuncSetAttribute(k_wterm<N>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_wt);
     cudaFuncSetAttribute(k_zshift<N, cplx>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_zs);
     cudaFuncSetAttribute(k_zshift<N, cplxf>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_zs);
+    if constexpr (N <= 32) {
+      cudaFuncSetAttribute(k_zfwd_full<N, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_zacc);
+      cudaFuncSetAttribute(k_zfwd_full<N, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_zacc);
+    }
     cudaFuncSetAttribute(k_zfwd_acc<N, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_zacc);
     cudaFuncSetAttribute(k_zfwd_acc<N, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_zacc);
     c->v1_attr_done = true;
@@ -1672,8 +1706,9 @@ static int collide_v1_impl(dgfs_ctx* c, const double* f, double* out, int nx, bo
         { ProfScope ps(c->prof, st, "k_xy_full", nb * (run_all - run_vhs) * fl.xy_full);
           k_xy_full<N, W><<<dim3((N + W - 1) / W, items), 32 * W, smem_xyf, st>>>(c->v1, c->tab, gv, nyqb[b], Tf, r); }
         { ProfScope ps(c->prof, st, "k_zfwd_full", nb * nfull * fl.acc_full);
-          if (r == 0) k_zfwd_full<N, true><<<dim3(pen_blocks, items), 256, 0, st>>>(c->tab, c->v1, Tf, QG, qstride, r);
-          else k_zfwd_full<N, false><<<dim3(pen_blocks, items), 256, 0, st>>>(c->tab, c->v1, Tf, QG, qstride, r); }
+          const int fp_blocks = (N2 + ZaccSmem<N>::PB - 1) / ZaccSmem<N>::PB;
+          if (r == 0) k_zfwd_full<N, true><<<dim3(fp_blocks, items), 128, smem_zacc, st>>>(c->tab, c->v1, Tf, QG, qstride, r);
+          else k_zfwd_full<N, false><<<dim3(fp_blocks, items), 128, smem_zacc, st>>>(c->tab, c->v1, Tf, QG, qstride, r); }
       }
       record(c->ev_xy[b], st);
       // ---- forward z pass and QG accumulation of a finished group of radial nodes (stream sz)
