@@ -378,6 +378,7 @@ def report(args, cfg, op, prof, nx, world, stages, ms_per_step, value, e2e_ms, n
     # (its intermediates) is reported beside it with its own floor, which at c2 is of the same size as the flops floor.
     bound = "alu" if flops_floor_ms >= alg_bytes_floor_ms else "hbm"
     top_traffic = tj["dram_bytes_per_launch"].get(top["name"]) if (tj and dram_step) else None
+    clk = sampler.summary()
     roofline = {
         "bound": bound,
         # the WHOLE step: executed-algorithm flops of every kernel of the call / step time / nominal FP64 peak
@@ -394,6 +395,10 @@ def report(args, cfg, op, prof, nx, world, stages, ms_per_step, value, e2e_ms, n
         "step_dram_gbs": dram_step / (ms_per_step * 1e-3) / 1e9 if dram_step else None,
         "hbm_gbs": hbm_gbs, "hbm_source": hbm_src,
         "frac_of_measured_dfma_peak": step_tflops / peak_meas,
+        # the same fraction against the pipe's rate at the SM clock the timed steps actually ran at (median NVML sample;
+        # under the power cap the step runs below sm_max_mhz): secondary, "frac" stays against the nominal clock
+        "frac_at_sm_clock": (step_tflops / (FP64_PEAK_NOMINAL_TFLOPS * clk["sm_mhz"] / clk["sm_max_mhz"])
+                             if clk.get("sm_mhz") and clk.get("sm_max_mhz") else None),
         "measured_dfma_peak": peak_meas,
         "measured_dfma_peak_how": "dgfs_measure_fp64_peak: dependency-free DFMA chains, 2 s sustained, same box",
         # the dominant kernel class, from the library's per-launch CUDA events on the launching stream
@@ -428,7 +433,7 @@ def report(args, cfg, op, prof, nx, world, stages, ms_per_step, value, e2e_ms, n
                             "(N, N_rho, M) operating point, BKW workload; context, not the target",
         "dtype": args.precision, "data": "synthetic",
         "config": dict(workload_desc(cfg, nx, world, stages), **variant),
-        "clocks": sampler.summary(),
+        "clocks": clk,
         "e2e": {"value": evals_step / (e2e_ms * 1e-3), "unit": UNIT, "ms_per_step": e2e_ms,
                 "h2d_bytes_per_step": nbytes, "d2h_bytes_per_step": nbytes,
                 "call": ("state host -> device, one step, device -> host (pinned buffers, host clock)" if is_dg else
