@@ -1252,6 +1252,92 @@ __global__ void __launch_bounds__(WtermSmem<N>::THREADS, N > 32 ? 1 : 2) k_wterm
       *reinterpret_cast<double2*>(o + (size_t)b * N2 + i * N) = make_double2(-acc[i][b][0], -acc[i][b][1]);
 }
 
+// k_wterm with the uy plane of a sphere point fetched ONCE per item: the N / CYB blocks of an item (its cy slabs) form a
+// thread-block cluster; block rank 0 issues one bulk copy of the plane with .multicast::cluster, which lands at the same
+// shared-memory offset of every block of the cluster and counts its bytes on each block's own mbarrier; every block
+// still fetches its own rows of ux' and uz.  A slot is refilled only after EVERY block of the cluster has finished with
+// it: the block barrier of k_wterm becomes a cluster barrier, split into arrive (after a job's arithmetic) and wait
+// (before the next refill is issued).
+__device__ __forceinline__ unsigned cluster_ctarank() { unsigned r; asm volatile("mov.u32 %0, %%cluster_ctarank;\n" : "=r"(r)); return r; }
+__device__ __forceinline__ void cluster_arrive() { asm volatile("barrier.cluster.arrive.release.aligned;\n" ::: "memory"); }
+__device__ __forceinline__ void cluster_wait() { asm volatile("barrier.cluster.wait.acquire.aligned;\n" ::: "memory"); }
+__device__ __forceinline__ void tma_bulk_g2s_mc(void* smem, const void* gmem, unsigned bytes, unsigned long long* bar, unsigned short mask) {
+  asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes.multicast::cluster [%0], [%1], %2, [%3], %4;\n"
+               ::"r"(smem_u32(smem)), "l"(gmem), "r"(bytes), "r"(smem_u32(bar)), "h"(mask) : "memory");
+}
+template <int N>
+__global__ void __launch_bounds__(WtermSmem<N>::THREADS, 2) k_wterm_mc(const cplx* __restrict__ nyq, int M, double* __restrict__ S, const unsigned char* __restrict__ full, int npairs,
+        const unsigned char* __restrict__ smask, const unsigned char* __restrict__ sskip, const int* __restrict__ tsrc) {
+  constexpr int N2 = N * N, N3 = N2 * N, H = N / 2;
+  typedef NyqLayout<N> NL;
+  typedef WtermSmem<N> WS;
+  constexpr int CYB = WS::CYB, NT = WS::THREADS, NS = WS::STAGES, NC = N / CYB;
+  extern __shared__ cplx sm[];
+  // uniform per cluster (one item): nothing to do
+  if (full[blockIdx.y % npairs] || tsrc[blockIdx.y % npairs] != (int)(blockIdx.y % npairs)) return;
+  const int tx = threadIdx.x % H, tz = threadIdx.x / H;
+  const unsigned rank = cluster_ctarank();
+  const int cy0 = blockIdx.x * CYB;
+  const cplx* nbase = nyq + (size_t)blockIdx.y * M * NL::STRIDE;
+  const unsigned char* skip = sskip + (size_t)(blockIdx.y % npairs) * M;
+  __shared__ unsigned char mk_s[256];
+  __shared__ unsigned long long bar[NS];
+  for (int i = threadIdx.x; i < M && i < 256; i += NT) mk_s[i] = skip[i] ? 7 : smask[i];
+  if (threadIdx.x == 0) {
+    for (int k = 0; k < NS; ++k) mbar_init(&bar[k], 1);
+    fence_mbar_init();
+  }
+  __syncthreads();
+  cluster_arrive();                                  // every block's barriers exist before anyone multicasts onto them
+  cluster_wait();
+  auto mk = [&](int s) -> int { return s < 256 ? (int)mk_s[s] : (skip[s] ? 7 : (int)smask[s]); };
+  auto next_a = [&](int s) { while (s < M && mk(s) == 7) ++s; return s; };
+  auto issue = [&](int s, int slot) {
+    cplx* dst = sm + (size_t)slot * WS::WORDS;
+    const cplx* nq = nbase + (size_t)s * NL::STRIDE;
+    const int mask = mk(s);
+    const unsigned bu = (mask & 1) ? 0u : (unsigned)(CYB * N * sizeof(cplx));
+    const unsigned by = (mask & 2) ? 0u : (unsigned)(N2 * sizeof(cplx));
+    const unsigned bz = (mask & 4) ? 0u : (unsigned)(CYB * N * sizeof(cplx));
+    mbar_expect_tx(&bar[slot], bu + by + bz);         // by arrives by multicast from block rank 0
+    if (by && rank == 0) tma_bulk_g2s_mc(dst + WS::Y, nq + NL::UY, by, &bar[slot], (unsigned short)((1u << NC) - 1));
+    if (bz) tma_bulk_g2s(dst + WS::Z, nq + NL::UZ + (size_t)cy0 * N, bz, &bar[slot]);
+    if (bu) tma_bulk_g2s(dst + WS::U, nq + NL::UXP + (size_t)cy0 * N, bu, &bar[slot]);
+  };
+  double acc[CYB][2][2];
+#pragma unroll
+  for (int i = 0; i < CYB; ++i) acc[i][0][0] = acc[i][0][1] = acc[i][1][0] = acc[i][1][1] = 0.0;
+  int s_issue = next_a(0), j_issue = 0;
+  if (threadIdx.x == 0) {
+    for (int k = 0; k < NS - 1 && s_issue < M; ++k) { issue(s_issue, j_issue % NS); s_issue = next_a(s_issue + 1); ++j_issue; }
+  }
+  cluster_arrive();                                  // matches the wait of the first iteration (no job before it)
+  for (int s = next_a(0), j = 0; s < M; s = next_a(s + 1), ++j) {
+    mbar_wait(&bar[j % NS], (unsigned)((j / NS) & 1));       // the bulk copies of job j have landed
+    cluster_wait();                                            // every block of the item is done with job j - 1
+    if (threadIdx.x == 0 && s_issue < M) { issue(s_issue, j_issue % NS); s_issue = next_a(s_issue + 1); ++j_issue; }
+    const cplx* b_ = sm + (size_t)(j % NS) * WS::WORDS;
+    switch (mk(s)) {
+      case 0: wterm_rows<N, 0>(b_, tx, tz, acc); break;
+      case 1: wterm_rows<N, 1>(b_, tx, tz, acc); break;
+      case 2: wterm_rows<N, 2>(b_, tx, tz, acc); break;
+      case 3: wterm_rows<N, 3>(b_, tx, tz, acc); break;
+      case 4: wterm_rows<N, 4>(b_, tx, tz, acc); break;
+      case 5: wterm_rows<N, 5>(b_, tx, tz, acc); break;
+      case 6: wterm_rows<N, 6>(b_, tx, tz, acc); break;
+      default: break;
+    }
+    cluster_arrive();
+  }
+  cluster_wait();                                    // the last arrive; no block leaves while a neighbour still multicasts
+  double* o = S + (size_t)blockIdx.y * N3 + (size_t)(2 * tz) * N2 + (size_t)cy0 * N + 2 * tx;
+#pragma unroll
+  for (int i = 0; i < CYB; ++i)
+#pragma unroll
+    for (int b = 0; b < 2; ++b)
+      *reinterpret_cast<double2*>(o + (size_t)b * N2 + i * N) = make_double2(-acc[i][b][0], -acc[i][b][1]);
+}
+
 // Forward z pass and steps 7-8 for a group of nr radial nodes r0 .. r0+nr-1:
 //   QGh[item][kz][kx][ky <= H] (+)= sum_r w_r b_r(|k|^2) fft_z( T_r[item][.][kx][ky] ).
 // Thread pair per (kx,ky) pencil: parity 0 computes the even kz, parity 1 the odd kz (one radix-2
@@ -1502,6 +1588,8 @@ int init_streams_v1(dgfs_ctx* c) {
   c->v1_pack = (pk && atoi(pk) != 0);      // measured at c1 (N = 24): 119.5 against 113.2 ms of k_xy per 3 steps, off by default
   const char* xw = getenv("DGFS_V1_XYW");
   c->v1_xyw = (xw && atoi(xw) == 2) ? 2 : 4;
+  const char* wm = getenv("DGFS_V1_WTERM_MC");
+  c->v1_wterm_mc = (wm && atoi(wm) != 0);
   // byte budget of the workspace of one launch group (plan_v1): DGFS_V1_WS_GB, else 70 % of the memory free now
   const char* wb = getenv("DGFS_V1_WS_GB");
   size_t freeb = 0, totalb = 0;
@@ -1609,6 +1697,7 @@ static int collide_v1_impl(dgfs_ctx* c, const double* f, double* out, int nx, bo
       cudaFuncSetAttribute(k_nyq2_wide<N>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_wide);
     }
     cudaFuncSetAttribute(k_wterm<N>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_wt);
+    if constexpr (N == 32) cudaFuncSetAttribute(k_wterm_mc<N>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_wt);
     cudaFuncSetAttribute(k_zshift<N, cplx>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_zs);
     cudaFuncSetAttribute(k_zshift<N, cplxf>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_zs);
     if constexpr (N <= 32) {
@@ -1674,6 +1763,20 @@ static int collide_v1_impl(dgfs_ctx* c, const double* f, double* out, int nx, bo
         else k_nyq2_wide<N><<<dim3(3, items), 64, smem_wide, sa>>>(c->v1, c->tab, fhh, nyqy, nyqb[b], r); }
       if (nvhs > 0)
         { ProfScope ps(c->prof, sa, "k_wterm", nb * run_vhs * fl.wterm);
+          bool mc = false;
+          if constexpr (N == 32) mc = c->v1_wterm_mc != 0;
+          if (mc) {
+            if constexpr (N == 32) {
+              cudaLaunchConfig_t lc{};
+              lc.gridDim = dim3(N / WtermSmem<N>::CYB, items); lc.blockDim = dim3(WtermSmem<N>::THREADS);
+              lc.dynamicSmemBytes = smem_wt; lc.stream = sa;
+              cudaLaunchAttribute at[1];
+              at[0].id = cudaLaunchAttributeClusterDimension;
+              at[0].val.clusterDim.x = N / WtermSmem<N>::CYB; at[0].val.clusterDim.y = 1; at[0].val.clusterDim.z = 1;
+              lc.attrs = at; lc.numAttrs = 1;
+              cudaLaunchKernelEx(&lc, k_wterm_mc<N>, (const cplx*)nyqb[b], (int)c->M, Sb[b], c->tab.full, np, c->v1.smask, c->v1.sskip, c->v1.tsrc);
+            }
+          } else
           k_wterm<N><<<dim3(N / WtermSmem<N>::CYB, items), WtermSmem<N>::THREADS, smem_wt, sa>>>(nyqb[b], c->M, Sb[b], c->tab.full, np, c->v1.smask, c->v1.sskip, c->v1.tsrc); }
       }
       record(c->ev_prep[b], sa);

@@ -175,6 +175,7 @@ struct dgfs_ctx {
   // the caller's stream; double-buffered intermediates, ordered by these events
   int v1_pack = 0;                       // DGFS_V1_PACK=1, N < 32: plane jobs dealt out N lanes each instead of one per warp
   int v1_xyw = 4;                        // warps per k_xy block (DGFS_V1_XYW)
+  int v1_wterm_mc = 0;                   // DGFS_V1_WTERM_MC=1 (N = 32): k_wterm as clusters of 4 blocks, uy plane by TMA multicast
   int v1_overlap = 0;                    // DGFS_V1_OVERLAP=1: three streams (default: everything on the caller's stream)
   cudaStream_t aux = nullptr, aux2 = nullptr;
   bool v1_attr_done = false, v0_attr_done = false;   // dynamic shared-memory opt-in, once per context (= per device)

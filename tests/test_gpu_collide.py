@@ -321,6 +321,24 @@ def test_v1_workspace_budget_shrinks_the_launch_group(torch_cuda, monkeypatch):
         assert torch.equal(op.collide_pairs(f), Qb)
 
 
+def test_k_wterm_cluster_multicast_variant_is_bit_equal(torch_cuda, monkeypatch):
+    """DGFS_V1_WTERM_MC=1 (N = 32): k_wterm as clusters of four blocks, the uy plane of a sphere point fetched once per
+    item by a TMA multicast (measured slower than the default, profiles/r02_wterm.md; kept as a switch): same sums in
+    the same order, so the results equal the default's bit for bit; white-noise inputs so that the Nyquist fields count."""
+    torch = torch_cuda
+    cfg = _rand_cfg("t", 2, 32, 3, 12, (1.0, 1.0), (0.6, 0.8), (1.0, 2.0), seed=23)
+    rng = np.random.default_rng(5)
+    f = make_points(cfg, range(6)) * (1.0 + 0.4 * rng.uniform(-1, 1, (6, cfg.ns, cfg.N ** 3)))
+    fd = torch.from_numpy(f).cuda()
+    with _gpu_op(cfg) as op:
+        Q0 = op.collide_pairs(fd).clone()
+    monkeypatch.setenv("DGFS_V1_WTERM_MC", "1")
+    with _gpu_op(cfg) as op:
+        Q1 = op.collide_pairs(fd).clone()
+        Q2 = op.collide_pairs(fd)
+        assert torch.equal(Q1, Q0) and torch.equal(Q2, Q0)
+
+
 def test_v1_mixed_pairs_batch_consistency_and_chunking(torch_cuda, monkeypatch):
     """3 species, pair (0,0) VHS and the other eight VSS in one context: the two kinds share the z shifts and
     the Nyquist fields and take different kernels afterwards; chunking must not change a bit."""
