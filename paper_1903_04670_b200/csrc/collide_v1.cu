@@ -1031,27 +1031,100 @@ struct ZaccSmem {
 // The rows of Tf (64 pencils x N values of z per sphere point) are staged in shared memory by cp.async, a ring of three
 // stages over the sphere points that ran, as k_zfwd_acc stages the radial nodes of T: the loads of the next two points are
 // in flight while the current one is transformed, and both threads of a pencil read each element from the stage.
+// One sphere point's contribution for the thread's quarter QTR of the outputs, kz = 4 k + QTR: one radix-4 decimation-in-
+// frequency step on the staged row, u_j = (x_j + w^QTR x_{j+Q} + w^{2 QTR} x_{j+2Q} + w^{3 QTR} x_{j+3Q}) W_N^{j QTR}
+// (w = -i, Q = N / 4), then a length-Q transform in registers.
+template <int N, int QTR>
+__device__ __forceinline__ void zfull_quarter(const cplx* __restrict__ src, int PB, const BSweep& b1, const BSweep& b2,
+                                              const BSweep& b3, bool sym, bool twin, bool has_partner, double ft, double fp,
+                                              cplx (&acc)[N / 4], cplx (&acc2)[N / 4]) {
+  constexpr int Q = N / 4, H = N / 2;
+  cplx u[Q];
+#pragma unroll
+  for (int j = 0; j < Q; ++j) {
+    const cplx x0 = src[j * PB], x1 = src[(j + Q) * PB], x2 = src[(j + 2 * Q) * PB], x3 = src[(j + 3 * Q) * PB];
+    cplx v;
+    if (QTR == 0) v = cadd(cadd(x0, x2), cadd(x1, x3));
+    else if (QTR == 2) v = csub(cadd(x0, x2), cadd(x1, x3));
+    else {
+      // QTR = 1: x0 - i x1 - x2 + i x3 = (x0 - x2) - i (x1 - x3);  QTR = 3: (x0 - x2) + i (x1 - x3)
+      const cplx a = csub(x0, x2), d = csub(x1, x3);
+      v = (QTR == 1) ? make_double2(a.x + d.y, a.y - d.x) : make_double2(a.x - d.y, a.y + d.x);
+    }
+    u[j] = twiddle_mul<N, -1>(v, j * QTR);
+  }
+  fft_reg<Q, -1>(u);
+#pragma unroll
+  for (int k = 0; k < Q; ++k) {
+    const int iz = 4 * k + QTR, kzs = iz - (iz >= H ? N : 0);
+    const long zi = sym ? kzs : iz;
+    cplx b = b1.p[zi * b1.sz];
+    if (twin) { const cplx bb = b2.p[zi * b2.sz]; b.x = fma(ft, bb.x, b.x); b.y = fma(ft, bb.y, b.y); }
+    acc[k] = cfma(b, u[k], acc[k]);
+    if (has_partner) { const cplx b3v = b3.p[zi * b3.sz]; acc2[k] = cfma(make_double2(fp * b3v.x, fp * b3v.y), u[k], acc2[k]); }
+  }
+}
+template <int N>
+struct ZfullSmem {
+  static constexpr int PB = 64, STAGES = 3, WORDS = N * PB;
+};
+// The rows of Tf (64 pencils x N values of z per sphere point) are staged in shared memory by cp.async, a ring of three
+// stages over the sphere points that ran, as k_zfwd_acc stages the radial nodes of T.  FOUR threads per pencil, each
+// with a quarter of the outputs (N / 4 + N / 4 accumulators): ~130 registers, so that enough warps are resident to hide
+// the L2 latency of the three sweeps over the b tables (with two threads per pencil and 255 registers, 8 warps per SM,
+// every sweep's round trip was exposed).
 template <int N, bool FIRST>
-__global__ void __launch_bounds__(128) k_zfwd_full(DevTables tab, V1Tables t, const cplx* __restrict__ Tf,
+__global__ void __launch_bounds__(256, 2) k_zfwd_full(DevTables tab, V1Tables t, const cplx* __restrict__ Tf,
                                                    cplx* __restrict__ QG, size_t qstride, int r) {
-  constexpr int H = N / 2, N2 = N * N, N3 = N2 * N;
-  typedef ZaccSmem<N> ZS;
+  constexpr int Q = N / 4, N2 = N * N, N3 = N2 * N;
+  typedef ZfullSmem<N> ZS;
   constexpr int PB = ZS::PB, NS = ZS::STAGES;
   extern __shared__ cplx sm[];
-  const int par = threadIdx.x >> 6, pl = threadIdx.x & 63;
+  const int qtr = threadIdx.x >> 6, pl = threadIdx.x & 63;          // warp-uniform quarter
   const int pid0 = blockIdx.x * PB, pid = pid0 + pl;
   const int item = blockIdx.y, pair = item % tab.npairs;
   if (!tab.full[pair] || t.tsrc[pair] != pair) return;      // uniform per block
   const int M = tab.M;
   const int partner = t.tpartner[pair];                 // pair that reads this one's products, or -1
   const unsigned char* skip = t.sskip + (size_t)pair * M;
-  auto next_s = [&](int s) { while (s < M && skip[s]) ++s; return s; };
+  // What the loop needs to know about a sphere point (its antipode, the weight ratios, where its three sweeps over the b
+  // tables start and how they stride), gathered ONCE per block by one thread per sphere point and kept in shared
+  // memory: looked up inside the loop these are chains of four or five dependent global loads per sphere point, and
+  // that latency, not the sweeps or the staging, was what the kernel waited for (long scoreboard 6.2 per issue).
+  constexpr int MAXJ = 64;
+  struct ZJob { int run, twin; double ft, fp; long b1, b2, b3; int m1[3], m2[3], m3[3]; };
+  __shared__ ZJob jobs[MAXJ];
+  const bool sym = tab.bsym != 0;
+  auto sweep_of = [&](int s2, long& base, int (&m)[3]) {
+    if (sym) {
+      const int4 mm = tab.bmap[s2];
+      const long E = N + 1;
+      base = (long)r * tab.nref * (E * E * E) + mm.x; m[0] = mm.y; m[1] = mm.z; m[2] = mm.w;
+    } else { base = ((long)r * M + s2) * N3; m[0] = N; m[1] = 1; m[2] = N2; }
+  };
+  auto make_job = [&](int s2) {
+    ZJob jb;
+    jb.run = !skip[s2];
+    const int sa = t.anti[s2];
+    jb.twin = jb.run && sa >= 0 && skip[sa] && t.fsrc_s[(size_t)pair * M + sa] == s2;     // same-species pair: s also stands for its antipode
+    jb.ft = jb.twin ? t.fscale[(size_t)pair * M + sa] : 0.0;
+    jb.fp = (partner >= 0 && sa >= 0) ? t.fscale[(size_t)partner * M + sa] : 0.0;
+    sweep_of(s2, jb.b1, jb.m1);
+    sweep_of(jb.twin ? sa : s2, jb.b2, jb.m2);
+    sweep_of(partner >= 0 && sa >= 0 ? sa : s2, jb.b3, jb.m3);
+    return jb;
+  };
+  for (int s2 = threadIdx.x; s2 < M && s2 < MAXJ; s2 += 256) jobs[s2] = make_job(s2);
+  const cplx* bf_own = tab.bfull[pair];
+  const cplx* bf_par = tab.bfull[partner >= 0 ? partner : pair];
+  __syncthreads();
+  auto next_s = [&](int s) { while (s < M && (s < MAXJ ? !jobs[s].run : (bool)skip[s])) ++s; return s; };
   const cplx* tbase = Tf + (size_t)item * M * N3 + pid0;
   auto issue = [&](int s, int slot) {
     cplx* dstb = sm + (size_t)slot * ZS::WORDS;
     const cplx* srcb = tbase + (size_t)s * N3;
 #pragma unroll
-    for (int q = threadIdx.x; q < N * PB; q += 128) {
+    for (int q = threadIdx.x; q < N * PB; q += 256) {
       const int jj = q / PB, col = q % PB;
       if (pid0 + col < N2) cp_async16(&dstb[q], srcb + (size_t)jj * N2 + col);
     }
@@ -1064,11 +1137,12 @@ __global__ void __launch_bounds__(128) k_zfwd_full(DevTables tab, V1Tables t, co
   }
   const bool live = pid < N2;
   const int pc = live ? pid : 0;
-  const int kxs = sfreq(pc / N, N), kys = sfreq(pc % N, N);
+  // index of the pencil in a table: signed frequencies on the extended grid of the orbit tables, else plain indices
+  const int kxu = sym ? sfreq(pc / N, N) : pc / N, kyu = sym ? sfreq(pc % N, N) : pc % N;
   const double scale = tab.w_rho[r];
-  cplx acc[H], acc2[H];
+  cplx acc[Q], acc2[Q];
 #pragma unroll
-  for (int k = 0; k < H; ++k) acc[k] = acc2[k] = make_double2(0.0, 0.0);
+  for (int k = 0; k < Q; ++k) acc[k] = acc2[k] = make_double2(0.0, 0.0);
   for (int s = next_s(0), j = 0; s < M; s = next_s(s + 1), ++j) {
     cp_async_wait_pending<NS - 2>();
     __syncthreads();                            // stage j has landed; the stage of j - 1 is free
@@ -1076,40 +1150,25 @@ __global__ void __launch_bounds__(128) k_zfwd_full(DevTables tab, V1Tables t, co
     cp_async_commit();
     if (!live) continue;
     const cplx* src = sm + (size_t)(j % NS) * ZS::WORDS + pl;
-    cplx u[H];
-    if (par == 0) {
-#pragma unroll
-      for (int jj = 0; jj < H; ++jj) u[jj] = cadd(src[jj * PB], src[(jj + H) * PB]);
-    } else {
-#pragma unroll
-      for (int jj = 0; jj < H; ++jj) u[jj] = twiddle_mul<N, -1>(csub(src[jj * PB], src[(jj + H) * PB]), jj);
-    }
-    fft_reg<H, -1>(u);
-    const int sa = t.anti[s];
-    // same-species pair: s also stands for its antipode
-    const bool twin = sa >= 0 && skip[sa] && t.fsrc_s[(size_t)pair * M + sa] == s;
-    const double ft = twin ? t.fscale[(size_t)pair * M + sa] : 0.0;
-    const double fp = (partner >= 0) ? t.fscale[(size_t)partner * M + sa] : 0.0;
-    const bool sym = tab.bsym != 0;
-    const BSweep b1 = bfull_sweep(tab, pair, r, s, kxs, kys);
-    const BSweep b2 = bfull_sweep(tab, pair, r, twin ? sa : s, kxs, kys);
-    const BSweep b3 = bfull_sweep(tab, partner >= 0 ? partner : pair, r, partner >= 0 ? sa : s, kxs, kys);
-#pragma unroll
-    for (int k = 0; k < H; ++k) {
-      const int iz = 2 * k + par, kzs = iz - (iz >= H ? N : 0);
-      const long zi = sym ? kzs : iz;
-      cplx b = b1.p[zi * b1.sz];
-      if (twin) { const cplx bb = b2.p[zi * b2.sz]; b.x = fma(ft, bb.x, b.x); b.y = fma(ft, bb.y, b.y); }
-      acc[k] = cfma(b, u[k], acc[k]);
-      if (partner >= 0) { const cplx b3v = b3.p[zi * b3.sz]; acc2[k] = cfma(make_double2(fp * b3v.x, fp * b3v.y), u[k], acc2[k]); }
+    const ZJob jb = (s < MAXJ) ? jobs[s] : make_job(s);
+    const bool twin = jb.twin != 0;
+    const double ft = jb.ft, fp = jb.fp;
+    const BSweep b1{bf_own + jb.b1 + (long)kxu * jb.m1[0] + (long)kyu * jb.m1[1], (long)jb.m1[2]};
+    const BSweep b2{bf_own + jb.b2 + (long)kxu * jb.m2[0] + (long)kyu * jb.m2[1], (long)jb.m2[2]};
+    const BSweep b3{bf_par + jb.b3 + (long)kxu * jb.m3[0] + (long)kyu * jb.m3[1], (long)jb.m3[2]};
+    switch (qtr) {
+      case 0: zfull_quarter<N, 0>(src, PB, b1, b2, b3, sym, twin, partner >= 0, ft, fp, acc, acc2); break;
+      case 1: zfull_quarter<N, 1>(src, PB, b1, b2, b3, sym, twin, partner >= 0, ft, fp, acc, acc2); break;
+      case 2: zfull_quarter<N, 2>(src, PB, b1, b2, b3, sym, twin, partner >= 0, ft, fp, acc, acc2); break;
+      default: zfull_quarter<N, 3>(src, PB, b1, b2, b3, sym, twin, partner >= 0, ft, fp, acc, acc2); break;
     }
   }
   if (!live) return;
   cplx* dst = QG + (size_t)item * qstride + pid;
   cplx* dst2 = QG + (size_t)(item - pair + (partner >= 0 ? partner : pair)) * qstride + pid;
 #pragma unroll
-  for (int k = 0; k < H; ++k) {
-    const size_t o = (size_t)(2 * k + par) * N2;
+  for (int k = 0; k < Q; ++k) {
+    const size_t o = (size_t)(4 * k + qtr) * N2;
     const cplx q1 = FIRST ? make_double2(0.0, 0.0) : dst[o];
     dst[o] = make_double2(fma(scale, acc[k].x, q1.x), fma(scale, acc[k].y, q1.y));
     if (partner >= 0) {
@@ -1810,8 +1869,8 @@ static int collide_v1_impl(dgfs_ctx* c, const double* f, double* out, int nx, bo
           k_xy_full<N, W><<<dim3((N + W - 1) / W, items), 32 * W, smem_xyf, st>>>(c->v1, c->tab, gv, nyqb[b], Tf, r); }
         { ProfScope ps(c->prof, st, "k_zfwd_full", nb * nfull * fl.acc_full);
           const int fp_blocks = (N2 + ZaccSmem<N>::PB - 1) / ZaccSmem<N>::PB;
-          if (r == 0) k_zfwd_full<N, true><<<dim3(fp_blocks, items), 128, smem_zacc, st>>>(c->tab, c->v1, Tf, QG, qstride, r);
-          else k_zfwd_full<N, false><<<dim3(fp_blocks, items), 128, smem_zacc, st>>>(c->tab, c->v1, Tf, QG, qstride, r); }
+          if (r == 0) k_zfwd_full<N, true><<<dim3(fp_blocks, items), 256, smem_zacc, st>>>(c->tab, c->v1, Tf, QG, qstride, r);
+          else k_zfwd_full<N, false><<<dim3(fp_blocks, items), 256, smem_zacc, st>>>(c->tab, c->v1, Tf, QG, qstride, r); }
       }
       record(c->ev_xy[b], st);
       // ---- forward z pass and QG accumulation of a finished group of radial nodes (stream sz)
