@@ -910,13 +910,18 @@ __global__ void __launch_bounds__(PACK ? N * W : 32 * W) __maxnreg__(sizeof(C) =
 //   P = (a_r b_r - a_i b_i) + i (a_r b_i + a_i b_r),   W = a_i + i b_i from the Nyquist fields (file header).
 // Same block / warp mapping and prefetch as k_xy; the warp's shared memory also holds the uz plane and the
 // ux', uy columns of the job.  out: Tf[item][s][cz][kx][ky] = fft_xy of P_s(., ., cz).
+// The uz plane of a job does not depend on cz: the W warps (planes) of a block share ONE copy, staged a quarter each and
+// guarded by two block barriers per job (all warps of a block walk the same job list), instead of one copy per warp: 101
+// instead of 150 KB per block at N = 32, i.e. two blocks (eight warps) per SM instead of one.
 template <int N>
 struct FullSmem {
   typedef JobSmem<N> JS;
-  static constexpr int UZ = JS::WORDS;          // [cy][cx]
-  static constexpr int UX = JS::WORDS + N * N;  // [cy]   ux'(cy, cz)
+  static constexpr bool SHARE = N > 24;         // (N = 24: two blocks per SM either way, and the barriers cost 10 %: one copy per warp)
+  static constexpr int UX = JS::WORDS;          // [cy]   ux'(cy, cz)
   static constexpr int UY = UX + N;             // [cx]   uy(cx, cz)
-  static constexpr int WORDS = UY + N;
+  static constexpr int UZ = UY + N;             // [cy][cx] per warp (not SHARE)
+  static constexpr int WORDS = UY + N + (SHARE ? 0 : N * N);      // per warp
+  static constexpr int UZW = SHARE ? N * N : 0; // per block: [cy][cx], after the W warps' regions (SHARE)
 };
 template <int N, int W>
 __global__ void __launch_bounds__(32 * W) k_xy_full(V1Tables t, DevTables tab, GzView Gz,
@@ -933,6 +938,9 @@ __global__ void __launch_bounds__(32 * W) k_xy_full(V1Tables t, DevTables tab, G
   const int pair = item % tab.npairs, xl = item / tab.npairs;
   if (cz >= N || !tab.full[pair] || t.tsrc[pair] != pair) return;     // (q,p) reads the products of (p,q)
   cplx* buf = sm + (size_t)warp * FS::WORDS;
+  cplx* uzs = FS::SHARE ? sm + (size_t)W * FS::WORDS : buf + FS::UZ;      // the block's (or the warp's) copy of the uz plane
+  static_assert(N % W == 0, "every warp of a block has a plane (block barriers in the job loop)");
+  auto sync = [&]() { if (FS::SHARE) __syncthreads(); else __syncwarp(); };
   const bool act = lane < N;
   const int ln = act ? lane : 0;
   const int side = ln / H, m = ln % H;
@@ -957,7 +965,7 @@ __global__ void __launch_bounds__(32 * W) k_xy_full(V1Tables t, DevTables tab, G
       cp_async16(&buf[JS::VXP + ln], nq + NL::VXP + ln);
       if (ln == 0) cp_async16(&buf[JS::VZP], nq + NL::VZP + cz);
 #pragma unroll
-      for (int j = 0; j < N; ++j) cp_async16(&buf[FS::UZ + j * N + ln], nq + NL::UZ + j * N + ln);
+      for (int j = FS::SHARE ? warp : 0; j < N; j += FS::SHARE ? W : 1) cp_async16(&uzs[j * N + ln], nq + NL::UZ + j * N + ln);   // (this warp's rows)
       cp_async16(&buf[FS::UX + ln], nq + NL::UXP + ln * N + cz);
       cp_async16(&buf[FS::UY + ln], nq + NL::UY + ln * N + cz);
     }
@@ -970,7 +978,7 @@ __global__ void __launch_bounds__(32 * W) k_xy_full(V1Tables t, DevTables tab, G
   while (s < tab.M) {
     const int sn = next_s(s + 1);
     cp_async_wait_all();
-    __syncwarp();
+    sync();                                                // every warp's rows of the uz plane have landed
     cplx X[N];
     if (act) {
       // sigma_x = 0: h_x is the constant w_s / N (side A) or 1 / N; sigma_y = 0: h_y is the constant 1 / N
@@ -985,7 +993,7 @@ __global__ void __launch_bounds__(32 * W) k_xy_full(V1Tables t, DevTables tab, G
       const cplx uyv = buf[FS::UY + ln];
 #pragma unroll
       for (int j = 0; j < N; ++j) {
-        const cplx ux = buf[FS::UX + j], uz = buf[FS::UZ + j * N + ln];
+        const cplx ux = buf[FS::UX + j], uz = uzs[j * N + ln];
         const double syj = (j & 1) ? -1.0 : 1.0;
         const double ai = fma(sxb, ux.x, fma(szs, uz.x, syj * uyv.x));
         const double bi = fma(sxb, ux.y, fma(szs, uz.y, syj * uyv.y));
@@ -1004,7 +1012,7 @@ __global__ void __launch_bounds__(32 * W) k_xy_full(V1Tables t, DevTables tab, G
 #pragma unroll
       for (int i = 0; i < N; ++i) X[i] = buf[ln * P + i];          // lane = ky
     }
-    __syncwarp();
+    sync();                                                // every warp of the block is done with the uz plane
     if (sn < tab.M) issue(sn);                             // tile and tables are free again
     if (act) {
       fft_reg<N, -1>(X);                                   // forward x pass
@@ -1731,7 +1739,7 @@ static int collide_v1_impl(dgfs_ctx* c, const double* f, double* out, int nx, bo
   const size_t smem_plane = plane_smem_per_warp<N>() * W;
   const size_t smem_final = plane_smem_per_warp<N>() * 2;
   const size_t smem_xy = sizeof(cplx) * (size_t)W * GroupSmem<N>::WORDS;
-  const size_t smem_xyf = sizeof(cplx) * (size_t)W * FullSmem<N>::WORDS;
+  const size_t smem_xyf = sizeof(cplx) * ((size_t)W * FullSmem<N>::WORDS + FullSmem<N>::UZW);
   const size_t smem_wt = sizeof(cplx) * (size_t)WtermSmem<N>::STAGES * WtermSmem<N>::WORDS;
   const size_t smem_nyq = sizeof(cplx) * (size_t)2 * JobSmem<N>::WORDS;
   const size_t smem_zacc = sizeof(cplx) * (size_t)ZaccSmem<N>::STAGES * ZaccSmem<N>::WORDS;
