@@ -77,3 +77,34 @@ def test_random_contexts_batches_and_streams(seed, monkeypatch):
                 assert c is None or torch.equal(c, ref), what
                 assert np.array_equal(h, ref.cpu().numpy()), what
     assert ran_noalloc > 0
+
+
+def test_launch_group_at_the_grid_limit(monkeypatch):
+    """Maximum sizes of the launch geometry: a launch group asked to be larger than the grid's y extent allows
+    (65535 rows = points x pairs) is clipped to it, and a batch larger than one group is split with a ragged tail; v1 (20 000
+    points of N = 8, 2 species: groups of 16 383 + 3 617) and the v0 pipeline's own limit.  Sampled points against
+    single-point calls, bit for bit; no point left unwritten."""
+    import torch
+    if not torch.cuda.is_available():
+        pytest.fail("GPU tests need a CUDA device: there is no CPU fallback")
+    from paper_1903_04670_b200 import Dgfs
+    torch.cuda.set_device(0)
+    cfg = Config("g", 77, (1.0, 1.7), _mean_matrix((0.6, 0.8)), _mean_matrix((1.0, 1.0)),
+                 N=8, L=5.5, N_rho=2, M=6, nx=3, kind="bimaxwell")
+    nx = 20000
+    base = torch.from_numpy(make_points(cfg, range(50))).cuda()
+    scale = 1.0 + 0.5 * torch.rand(nx, 1, 1, dtype=torch.float64, device="cuda", generator=torch.Generator("cuda").manual_seed(5))
+    f = (base[torch.arange(nx, device="cuda") % 50] * scale).contiguous()
+    sample = [0, 1, 16382, 16383, 16384, 19998, 19999]
+    for pipeline, chunk_env in (("v1", "DGFS_V1_CHUNK"), ("v0", "DGFS_SCRATCH_MB")):
+        monkeypatch.delenv("DGFS_PIPELINE", raising=False)
+        if pipeline == "v0":
+            monkeypatch.setenv("DGFS_PIPELINE", "v0")
+        monkeypatch.setenv(chunk_env, "40000")
+        with Dgfs.from_config(cfg, device=0) as op:
+            out = torch.full((nx, cfg.ns, cfg.N ** 3), float("nan"), dtype=torch.float64, device="cuda")
+            op.collide(f, out=out)
+            assert bool(torch.isfinite(out).all()), pipeline
+            for x in sample:
+                assert torch.equal(op.collide(f[x:x + 1].contiguous())[0], out[x]), (pipeline, x)
+        monkeypatch.delenv(chunk_env, raising=False)
