@@ -99,6 +99,37 @@ def test_c2_full_batch_16_points_both_halves_all_pairs(torch_cuda):
     assert es.max() < TOL, es
 
 
+def test_c2_full_batch_bilinearity_on_every_point(torch_cuda):
+    """Properties that hold at any size, checked on ALL 4096 points of the headline batch.  Q^(pq) is bilinear (Eq. 1,
+    P:51) and scaling by a power of two is exact in floating point: with the whole state doubled every value of every
+    Q^(pq) is exactly 4x, bit for bit (every step of the path is linear in each argument).  With species 0 alone doubled
+    Q^(11) does not change by a bit, Q^(00) is exactly 4x, and the cross pairs, whose two fields share one complex
+    transform, are 2x to round-off (< 1e-11 of max|Q| per point and pair; 7e-13 measured, the near-equilibrium half).  A zero state gives exactly zero."""
+    torch = torch_cuda
+    from paper_1903_04670_b200 import Dgfs
+    cfg = get_config("c2")
+    f = torch.from_numpy(make_points(cfg, range(cfg.nx))).cuda()
+    with Dgfs.from_config(cfg, device=0) as op:
+        Q = op.collide_pairs(f).clone()
+        assert float(Q.abs().amax(dim=(1, 2, 3)).min()) > 0.0          # no point was left out
+        f *= 2.0
+        Q2 = op.collide_pairs(f)
+        assert torch.equal(Q2, 4.0 * Q)
+        f[:, 1, :] *= 0.5                                               # species 0 doubled, species 1 as at the start
+        Q2 = op.collide_pairs(f)
+        assert torch.equal(Q2[:, 0, 0], 4.0 * Q[:, 0, 0])
+        assert torch.equal(Q2[:, 1, 1], Q[:, 1, 1])
+        for (p, q) in ((0, 1), (1, 0)):
+            err = (Q2[:, p, q] - 2.0 * Q[:, p, q]).abs().amax(dim=1) / Q[:, p, q].abs().amax(dim=1) / 2.0
+            record(cfg.name, "bilinearity, all 4096 points, pair (%d,%d): species 0 doubled" % (p, q), float(err.max()), 1e-11,
+                   points=cfg.nx)
+            assert float(err.max()) < 1e-11
+        del Q, Q2
+        f.zero_()
+        Z = op.collide(f)
+        assert float(Z.abs().max()) == 0.0
+
+
 def test_c3_collision_term_all_dof_all_pairs(torch_cuda):
     """c3's collide call: 3 species, 8 of 9 pairs VSS (full b tables), all 64 spatial DOF against the oracle."""
     torch = torch_cuda
