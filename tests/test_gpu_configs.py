@@ -130,6 +130,26 @@ def test_c2_full_batch_bilinearity_on_every_point(torch_cuda):
         assert float(Z.abs().max()) == 0.0
 
 
+@pytest.mark.parametrize("name", ["c1", "c4"])
+def test_full_batch_exact_scaling_on_every_point(torch_cuda, name):
+    """The same exact property on every point of the other homogeneous batches (c1: N = 24; c4: N = 48, the wide plane
+    jobs): the state times 2 gives every Q^(pq) times 4, bit for bit, and no point is left unwritten."""
+    torch = torch_cuda
+    from paper_1903_04670_b200 import Dgfs
+    cfg = get_config(name)
+    f = torch.from_numpy(make_points(cfg, range(cfg.nx))).cuda()
+    with Dgfs.from_config(cfg, device=0) as op:
+        Q = torch.full((cfg.nx, cfg.ns, cfg.ns, cfg.N ** 3), float("nan"), dtype=torch.float64, device="cuda")
+        op.collide_pairs(f, out=Q)
+        assert bool(torch.isfinite(Q).all()) and float(Q.abs().amax(dim=(1, 2, 3)).min()) > 0.0
+        f *= 2.0
+        Q2 = op.collide_pairs(f)
+        Q *= 4.0
+        assert torch.equal(Q2, Q)
+    del Q, Q2, f
+    torch.cuda.empty_cache()
+
+
 def test_c3_collision_term_all_dof_all_pairs(torch_cuda):
     """c3's collide call: 3 species, 8 of 9 pairs VSS (full b tables), all 64 spatial DOF against the oracle."""
     torch = torch_cuda
