@@ -1153,12 +1153,13 @@ __global__ void __launch_bounds__(256, 2) k_zfwd_full(DevTables tab, V1Tables t,
   for (int k = 0; k < Q; ++k) acc[k] = acc2[k] = make_double2(0.0, 0.0);
   for (int s = next_s(0), j = 0; s < M; s = next_s(s + 1), ++j) {
     cp_async_wait_pending<NS - 2>();
+    if (s >= MAXJ && threadIdx.x == 0) jobs[s % MAXJ] = make_job(s);      // (M > 64: the slot of a point long done)
     __syncthreads();                            // stage j has landed; the stage of j - 1 is free
     if (s_iss < M) { issue(s_iss, (j + NS - 1) % NS); s_iss = next_s(s_iss + 1); }
     cp_async_commit();
     if (!live) continue;
     const cplx* src = sm + (size_t)(j % NS) * ZS::WORDS + pl;
-    const ZJob jb = (s < MAXJ) ? jobs[s] : make_job(s);
+    const ZJob& jb = jobs[s % MAXJ];                    // read in place (a copy of the struct ends up in local memory)
     const bool twin = jb.twin != 0;
     const double ft = jb.ft, fp = jb.fp;
     const BSweep b1{bf_own + jb.b1 + (long)kxu * jb.m1[0] + (long)kyu * jb.m1[1], (long)jb.m1[2]};
