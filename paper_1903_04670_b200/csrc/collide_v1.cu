@@ -1047,6 +1047,18 @@ __device__ __forceinline__ void zfull_quarter(const cplx* __restrict__ src, int 
                                               const BSweep& b3, bool sym, bool twin, bool has_partner, double ft, double fp,
                                               cplx (&acc)[N / 4], cplx (&acc2)[N / 4]) {
   constexpr int Q = N / 4, H = N / 2;
+  // N <= 24: the sweep over the point's own table is issued first, its L2 round trip runs under the transform (c3: 81.3 ->
+  // 72.5 ms per three steps).  Not at N = 32, and not the other two sweeps as well: at the 128-register cap the values
+  // are spilled and the kernel gets slower (measured both).
+  constexpr bool PRE = N <= 24;
+  cplx bo[PRE ? Q : 1];
+  if (PRE) {
+#pragma unroll
+    for (int k = 0; k < Q; ++k) {
+      const int iz = 4 * k + QTR, kzs = iz - (iz >= H ? N : 0);
+      bo[PRE ? k : 0] = b1.p[(sym ? (long)kzs : (long)iz) * b1.sz];
+    }
+  }
   cplx u[Q];
 #pragma unroll
   for (int j = 0; j < Q; ++j) {
@@ -1066,7 +1078,7 @@ __device__ __forceinline__ void zfull_quarter(const cplx* __restrict__ src, int 
   for (int k = 0; k < Q; ++k) {
     const int iz = 4 * k + QTR, kzs = iz - (iz >= H ? N : 0);
     const long zi = sym ? kzs : iz;
-    cplx b = b1.p[zi * b1.sz];
+    cplx b = PRE ? bo[PRE ? k : 0] : b1.p[zi * b1.sz];
     if (twin) { const cplx bb = b2.p[zi * b2.sz]; b.x = fma(ft, bb.x, b.x); b.y = fma(ft, bb.y, b.y); }
     acc[k] = cfma(b, u[k], acc[k]);
     if (has_partner) { const cplx b3v = b3.p[zi * b3.sz]; acc2[k] = cfma(make_double2(fp * b3v.x, fp * b3v.y), u[k], acc2[k]); }
